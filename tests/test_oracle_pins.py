@@ -1,0 +1,395 @@
+"""Pins P1-P10 of SURVEY.md §8(c): the oracle against what the paper and the
+mathematics fix (closed forms, fixed points, invariants, brute force).
+
+None of these re-types the oracle's formula as the expectation: every expected
+value comes from an independent route (long-double libm, an analytic closed
+form, a dense matrix power, an RK4 integration of the ODE of PAPER.md Eq. (1)).
+"""
+from math import factorial
+
+import numpy as np
+import pytest
+
+from gen import Network, make_toy
+from gen.network import _pack
+from oracle import Oracle, OracleParams
+
+
+def toy_with_coefs(A, reactions, coefs):
+    return _pack(A, reactions, coefs, "toy", {})
+
+
+# ---------------------------------------------------------------- P1: rates
+def test_p1_rate_constant_coefficients():
+    """a1..a6 = 0  =>  R = p * rho^(n-1) * exp(a0), p = 1/prod(m!)  (S:Q1, Q2)."""
+    A = [1, 1, 2, 3, 4]
+    reactions = [
+        ((0,), (1,)),          # 1-body, p = 1
+        ((0, 1), (2,)),        # 2-body distinct, p = 1
+        ((0, 0), (2,)),        # 2-body identical, p = 1/2
+        ((0, 0, 0), (3,)),     # 3-body identical, p = 1/6
+        ((0, 0, 2), (4,)),     # 3-body, one pair, p = 1/2
+        ((0, 1, 2), (4,)),     # 3-body distinct, p = 1
+    ]
+    a0 = [0.3, -1.2, 2.0, 0.7, -0.4, 1.1]
+    coefs = [(a, 0, 0, 0, 0, 0, 0) for a in a0]
+    o = Oracle(toy_with_coefs(A, reactions, coefs))
+    rho = 3.0e7
+    R = o.rates(T9=2.7, rho=rho)
+    pref = [1, 1, 1 / 2, 1 / 6, 1 / 2, 1]
+    nre = [1, 2, 2, 3, 3, 3]
+    expect = np.array([p * rho ** (n - 1) * np.exp(a) for p, n, a in zip(pref, nre, a0)])
+    np.testing.assert_allclose(R, expect, rtol=1e-14)
+
+
+def test_p1_rate_T9_one_and_eight():
+    """T9 = 1: ln R = a0+..+a5.  T9 = 8: T9^(1/3) = 2 and T9^(5/3) = 32 exactly."""
+    a = (0.5, -0.25, 0.125, 1.0, -0.5, 0.0625, 1.5)
+    o = Oracle(toy_with_coefs([1, 1], [((0,), (1,))], [a]))
+    R1 = o.rates(T9=1.0, rho=123.0)[0]
+    assert R1 == pytest.approx(np.exp(sum(a[:6])), rel=1e-15)
+    R8 = o.rates(T9=8.0, rho=123.0)[0]
+    ln8 = a[0] + a[1] / 8 + a[2] / 2 + a[3] * 2 + a[4] * 8 + a[5] * 32 + a[6] * np.log(8.0)
+    assert R8 == pytest.approx(np.exp(ln8), rel=4e-15)
+
+
+def test_p1_rate_vs_long_double(hub150):
+    """Cross-check O2 against 80-bit powl/expl/logl on the real tables."""
+    o = Oracle(hub150)
+    L = np.longdouble
+    third = L(1) / L(3)
+    for T9, rho in ((1.0, 1e7), (3.3, 2.2e8), (7.0, 1e8), (10.0, 3.1e9)):
+        R = o.rates(T9, rho)
+        T = L(T9)
+        a = hub150.coef.astype(L)
+        terms = np.stack([
+            a[:, 0], a[:, 1] / T, a[:, 2] * T ** (-third), a[:, 3] * T ** third, a[:, 4] * T,
+            a[:, 5] * T ** (L(5) * third), a[:, 6] * np.log(T),
+        ], axis=1)
+        lnp = np.array([
+            -sum(np.log(L(factorial(list(re[:n]).count(s)))) for s in set(re[:n]))
+            for re, n in zip(hub150.react, hub150.n_react)
+        ], dtype=L)
+        dens = (hub150.n_react.astype(L) - 1) * np.log(L(rho))
+        expect = np.exp(terms.sum(axis=1) + lnp + dens)
+        # one rounding (2^-53) per term of the exponent, amplified by its size
+        scale = np.abs(terms).sum(axis=1) + np.abs(lnp) + np.abs(dens) + 1
+        rel = np.abs((R.astype(L) - expect) / expect).astype(np.float64)
+        assert (rel <= 8 * 2.0**-53 * scale.astype(np.float64)).all(), rel.max()
+
+
+# ------------------------------------------------------ P2/P3: single decay
+def decay_net(k):
+    return make_toy([1, 1], [((0,), (1,))], [k])
+
+
+@pytest.mark.parametrize("k,dt,branch", [(1.0, 0.25, "euler"), (1.0, 1.0, "asym"),
+                                          (1.0, 4.0, "asym"), (2.0, 0.25, "euler")])
+def test_p2_single_decay_discrete_closed_forms(k, dt, branch):
+    """A -> B, F+_A = 0: Euler gives Y0 (1 - k dt)^n, Eq. (3) gives Y0/(1 + k dt)^n.
+    k dt = 1 exactly must take the asymptotic branch ('>=')."""
+    o = Oracle(decay_net(k))
+    n, Y0 = 40, 0.75
+    out = o.integrate_fixed(1.0, 1.0, [Y0, 0.0], dt, n)
+    YA, YB = out["Y"][0]
+    a = k * dt
+    if branch == "euler":
+        assert a < 1
+        assert YA == pytest.approx(Y0 * (1 - a) ** n, rel=1e-13)
+        assert YA + YB == pytest.approx(Y0, rel=1e-14)  # Euler conserves exactly
+        assert out["n_asym"][0] == 0
+    else:
+        assert a >= 1
+        assert YA == pytest.approx(Y0 / (1 + a) ** n, rel=1e-13)
+        # B is fed from the OLD Y_A each step (explicit):
+        # Y_B(n) = a Y0 sum_{j<n} (1+a)^-j
+        q = 1 / (1 + a)
+        assert YB == pytest.approx(a * Y0 * (1 - q**n) / (1 - q), rel=1e-13)
+        assert out["n_asym"][0] == n  # species A every step, species B never (k_B = 0)
+
+
+def test_p3_single_decay_continuum():
+    """Y0 exp(-k t) at k dt = 1e-4, t = 1/k: first-order error ~ k dt / 2."""
+    k = 1.0
+    o = Oracle(decay_net(k))
+    out = o.integrate_fixed(1.0, 1.0, [1.0, 0.0], 1e-4, 10_000)
+    rel = abs(out["Y"][0, 0] / np.exp(-1.0) - 1)
+    assert 4e-5 < rel < 6e-5
+
+
+# ------------------------------------------------- P4: two-species fixed point
+@pytest.mark.parametrize("dt", [1e-3, 0.5, 10.0, 1e3])
+def test_p4_two_species_equilibrium_ratio(dt):
+    """A <-> B: Y_A/Y_B = k_r/k_f is a fixed point of both branches at any dt."""
+    kf, kr = 3.0, 1.0
+    o = Oracle(make_toy([1, 1], [((0,), (1,)), ((1,), (0,))], [kf, kr]))
+    Y = np.array([[0.9, 0.1]])
+    for _ in range(60):
+        Y = o.integrate_fixed(1.0, 1.0, Y, dt, 1000)["Y"]
+    assert Y[0, 0] / Y[0, 1] == pytest.approx(kr / kf, rel=1e-12)
+
+
+def test_p4_total_drift_shrinks_with_eps():
+    """With the controller on and t long enough to enter the asymptotic branch,
+    |Y_A + Y_B - 1| is a bounded diagnostic, not an identity (Eq. (3) does not
+    conserve): small, and smaller at the tighter eps_Y."""
+    kf, kr = 3.0, 1.0
+    net = make_toy([1, 1], [((0,), (1,)), ((1,), (0,))], [kf, kr])
+    drift = []
+    for eps in (0.05, 0.0125):
+        o = Oracle(net, OracleParams(eps_y=eps))
+        out = o.integrate(1.0, 1.0, [[0.9, 0.1]], 10.0)
+        assert out["n_asym"][0] > 0
+        drift.append(abs(out["Y"].sum() - 1.0))
+    assert 1e-6 < drift[0] < 1e-2 and drift[1] < drift[0]
+
+
+# ------------------------------------------------------- P5: A-conservation
+def test_p5_nucleon_number_euler_regime(g16):
+    """Config 1 is all-Euler: sum(A_i Y_i) stays 1 to rounding over 1e4 steps."""
+    o = Oracle(g16)
+    Y0 = np.zeros(16)
+    Y0[0], Y0[1] = 0.5 / 4, 0.5 / 8
+    out = o.integrate_fixed(3.0, 1e8, Y0, 1e-10, 10_000)
+    assert out["n_asym"][0] == 0
+    assert abs((out["Y"][0] * g16.A).sum() - 1.0) < 1e-12
+
+
+def test_p5_every_family_conserves(hub150):
+    """Tiny Euler steps from a state with every species populated: any wrong
+    edge, sign or multiplicity in any reaction family breaks sum(A Y)."""
+    o = Oracle(hub150)
+    rng = np.random.default_rng(5)
+    Y0 = rng.uniform(0.5, 1.5, 150)
+    Y0 /= (Y0 * hub150.A).sum()
+    out = o.integrate_fixed(4.0, 1e8, Y0, 1e-16, 50)
+    assert out["n_asym"][0] == 0
+    assert not np.allclose(out["Y"][0], Y0, rtol=1e-9)  # something did happen
+    assert abs((out["Y"][0] * hub150.A).sum() - 1.0) < 1e-13
+
+
+# ----------------------------------------------------------- P6: positivity
+def test_p6_positivity(hub150):
+    o = Oracle(hub150)
+    rng = np.random.default_rng(6)
+    z = 6
+    T9 = rng.uniform(1, 10, z)
+    rho = 10 ** rng.uniform(7, 9.5, z)
+    Y0 = np.zeros((z, 150))
+    Y0[:, 3], Y0[:, 15] = 0.5 / 12, 0.5 / 16
+    Y = Y0
+    for dt in (1e-12, 1e-9, 1e-7, 1e-6):  # from all-Euler to mixed (1e-3 overflows: Eq. (3) does not conserve)
+        Y = o.integrate_fixed(T9, rho, Y, dt, 200)["Y"]
+        assert (Y >= 0).all() and np.isfinite(Y).all()
+    out = o.integrate(T9, rho, Y0, 1e-7)
+    assert (out["Y"] >= 0).all() and (out["status"] == 0).all()
+
+
+# ---------------------------------------------------------- P7: brute force
+def ode_rhs(net: Network, R, Y):
+    """dY/dt of Eq. (1) straight from the reaction list (independent of the
+    oracle's edge list): each reaction moves rate = R prod(Y) from its
+    reactants to its products, one unit per occurrence."""
+    d = np.zeros_like(Y)
+    for r in range(net.n_reactions):
+        re = net.react[r, : net.n_react[r]]
+        pr = net.prod[r, : net.n_prod[r]]
+        rate = R[r] * np.prod(Y[re])
+        for s in re:
+            d[s] -= rate
+        for s in pr:
+            d[s] += rate
+    return d
+
+
+def rk4(net, R, Y, t_end, n):
+    h = t_end / n
+    for _ in range(n):
+        k1 = ode_rhs(net, R, Y)
+        k2 = ode_rhs(net, R, Y + 0.5 * h * k1)
+        k3 = ode_rhs(net, R, Y + 0.5 * h * k2)
+        k4 = ode_rhs(net, R, Y + h * k3)
+        Y = Y + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    return Y
+
+
+def tiny_net():
+    # species: a(A=1) b(A=1) c(A=2) d(A=3) e(A=4) g(A=4)
+    A = [1, 1, 2, 3, 4, 4]
+    reactions = [
+        ((0,), (1,)),            # a -> b
+        ((1,), (0,)),            # b -> a
+        ((0, 1), (2,)),          # a + b -> c
+        ((2,), (0, 1)),          # c -> a + b
+        ((0, 0), (2,)),          # a + a -> c      (identical pair)
+        ((0, 1, 2), (4,)),       # a + b + c -> e  (3-body)
+        ((0, 0, 0), (3,)),       # 3a -> d         (3-body identical)
+        ((3, 0), (5,)),          # d + a -> g
+        ((5,), (4,)),            # g -> e
+        ((4,), (2, 2)),          # e -> c + c      (identical products)
+    ]
+    rates = [2.0, 1.0, 30.0, 0.5, 8.0, 200.0, 90.0, 40.0, 3.0, 0.7]
+    return make_toy(A, reactions, rates)
+
+
+def test_p7_brute_force_tiny_network():
+    net = tiny_net()
+    Y0 = np.array([0.5, 0.3, 0.1, 0.0, 0.0, 0.0])
+    Y0 /= (Y0 * net.A).sum()
+    t_end = 0.8
+    o = Oracle(net)
+    R = o.rates(1.0, 1.0)
+    ref = rk4(net, R, Y0.copy(), t_end, 8_000)
+    assert abs((ref * net.A).sum() - 1.0) < 1e-12
+    errs = []
+    for eps in (0.04, 0.01, 0.0025):
+        out = Oracle(net, OracleParams(eps_y=eps)).integrate(1.0, 1.0, Y0, t_end)
+        X, Xr = out["Y"][0] * net.A, ref * net.A
+        m = Xr > 1e-6
+        errs.append(np.abs(X[m] / Xr[m] - 1).max())
+    assert errs[0] < 4e-2                       # O(eps_Y)
+    assert errs[1] < 0.45 * errs[0] and errs[2] < 0.45 * errs[1]  # ~linear in eps_Y
+
+
+def test_p7_fixed_small_dt_matches_forward_euler_exactly():
+    """In the all-Euler regime the oracle IS forward Euler on Eq. (1)."""
+    net = tiny_net()
+    Y0 = np.array([0.5, 0.3, 0.1, 0.01, 0.02, 0.03])
+    o = Oracle(net)
+    R = o.rates(1.0, 1.0)
+    dt, n = 1e-4, 300
+    Y = Y0.copy()
+    for _ in range(n):
+        Y = Y + dt * ode_rhs(net, R, Y)
+    out = o.integrate_fixed(1.0, 1.0, Y0, dt, n)
+    assert out["n_asym"][0] == 0
+    np.testing.assert_allclose(out["Y"][0], Y, rtol=1e-12)
+
+
+# ------------------------------------------------------ P8: linear networks
+def test_p8_linear_network_dense_matrix_power():
+    """All 1-body reactions, Euler regime: Y_n = (I + dt K)^n Y0."""
+    rng = np.random.default_rng(8)
+    n_light, n_heavy = 6, 3  # A = 1 species and A = 2 species
+    N = n_light + n_heavy
+    A = [1] * n_light + [2] * n_heavy
+    reactions, rates = [], []
+    for _ in range(24):
+        i, j = rng.choice(n_light, 2, replace=False)
+        reactions.append(((int(i),), (int(j),)))
+        rates.append(float(rng.uniform(0.1, 5.0)))
+    for h in range(n_heavy):  # heavy -> j + j (nu = 2 on the product side) and -> j + j'
+        j = int(rng.integers(0, n_light))
+        reactions.append(((n_light + h,), (j, j)))
+        rates.append(float(rng.uniform(0.1, 5.0)))
+        j2 = (j + 1 + int(rng.integers(0, n_light - 1))) % n_light
+        reactions.append(((n_light + h,), (j, j2)))
+        rates.append(float(rng.uniform(0.1, 5.0)))
+    net = make_toy(A, reactions, rates)
+    K = np.zeros((N, N))
+    for (re, pr), k in zip(reactions, rates):
+        K[re[0], re[0]] -= k
+        for s in pr:
+            K[s, re[0]] += k
+    dt, n = 5e-3, 400
+    Y0 = rng.uniform(0.1, 1.0, N)
+    expect = np.linalg.matrix_power(np.eye(N) + dt * K, n) @ Y0
+    out = Oracle(net).integrate_fixed(1.0, 1.0, Y0, dt, n)
+    assert out["n_asym"][0] == 0
+    np.testing.assert_allclose(out["Y"][0], expect, rtol=1e-12)
+
+
+# ------------------------------------------------- P9: permutation invariance
+def test_p9_permutation_invariance(hub150):
+    net2, sigma = hub150.permuted(seed=99)
+    o1, o2 = Oracle(hub150), Oracle(net2)
+    Y0 = np.zeros(150)
+    Y0[3], Y0[15] = 0.5 / 12, 0.5 / 16
+    Y0p = np.zeros(150)
+    Y0p[sigma] = Y0
+    a = o1.integrate_fixed(6.0, 5e8, Y0, 1e-9, 500)["Y"][0]
+    b = o2.integrate_fixed(6.0, 5e8, Y0p, 1e-9, 500)["Y"][0][sigma]
+    X = a * hub150.A
+    m = X > 1e-12
+    assert m.sum() > 10
+    assert np.abs(b[m] / a[m] - 1).max() < 1e-10
+    ra = o1.integrate(6.0, 5e8, Y0, 1e-7)
+    rb = o2.integrate(6.0, 5e8, Y0p, 1e-7)
+    a, b = ra["Y"][0], rb["Y"][0][sigma]
+    m = a * hub150.A > 1e-12
+    assert np.abs(b[m] / a[m] - 1).max() < 1e-7
+    assert abs(int(ra["n_steps"][0]) - int(rb["n_steps"][0])) <= max(1, ra["n_steps"][0] // 100)
+
+
+# ------------------------------------------------ P10: 3-body multiplicity
+def test_p10_three_alpha_multiplicity():
+    """3a -> C with raw rate Rraw: f = Rraw Ya^3 / 6, F-_a = 3 f, F+_C = f."""
+    Rraw, Ya = 7.0, 0.2
+    net = toy_with_coefs([4, 12], [((0, 0, 0), (1,)), ((1,), (0, 0, 0))],
+                         [(np.log(Rraw), 0, 0, 0, 0, 0, 0), (np.log(0.5), 0, 0, 0, 0, 0, 0)])
+    o = Oracle(net)
+    R = o.rates(1.0, 1.0)
+    assert R[0] == pytest.approx(Rraw / 6, rel=1e-15)
+    f, Fp, Fm = o.rhs(R, [Ya, 0.0])
+    assert f[0] == pytest.approx(Rraw * Ya**3 / 6, rel=1e-15)
+    assert Fm[0] == pytest.approx(3 * Rraw * Ya**3 / 6, rel=1e-15) and Fp[1] == f[0]
+    # reverse: C -> 3a feeds alpha three times
+    f, Fp, Fm = o.rhs(R, [0.0, 0.1])
+    assert Fp[0] == pytest.approx(3 * 0.5 * 0.1, rel=1e-15) and Fm[1] == pytest.approx(0.05, rel=1e-15)
+    # first Euler step
+    dt = 1e-3
+    Y = o.integrate_fixed(1.0, 1.0, [Ya, 0.0], dt, 1)["Y"][0]
+    assert Y[0] == pytest.approx(Ya - dt * 3 * Rraw * Ya**3 / 6, rel=1e-15)
+    assert Y[1] == pytest.approx(dt * Rraw * Ya**3 / 6, rel=1e-15)
+
+
+# ------------------------------------------- controller and call contract
+def test_dt_controller_contract():
+    """O3/O6/O8-O9 (S:Q7, Q9-Q11) on a single decay where every step is known.
+
+    A -> B with k = 1, Y_A = 1, Y_B = 100, eps = 0.05: c_A = eps Y_A/(k Y_A) =
+    0.05 and c_B = eps Y_B/(k Y_A) >= 5, so dt_ctrl = 0.05 every step once the
+    growth cap allows; t_hydro = 1 takes exactly 20 steps (the last one clamped
+    through the 1e-12 guard) and the returned dt is the unclamped 0.05."""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.05, growth=2.0))
+    Y0 = [1.0, 100.0]
+    out = o.integrate(1.0, 1.0, Y0, 1.0)
+    assert out["n_steps"][0] == 20 and out["status"][0] == 0
+    assert out["dt"][0] == pytest.approx(0.05, rel=1e-12)
+    assert out["Y"][0, 0] == pytest.approx(0.95**20, rel=1e-12)
+    # trial dt honoured with the growth cap: dt_in = 0.01 -> 0.02, 0.04, then 0.05 ...
+    out = o.integrate(1.0, 1.0, Y0, 1.0, dt=[0.01])
+    # t after 2 steps = 0.06; remaining 0.94 / 0.05 = 18.8 -> 19 more steps
+    assert out["n_steps"][0] == 21
+    assert out["Y"][0, 0] == pytest.approx(0.98 * 0.96 * 0.95**18 * (1 - 0.04), rel=1e-12)
+    # a short clamped final step does not poison the returned dt (S:Q10)
+    assert out["dt"][0] == pytest.approx(0.05, rel=1e-12)
+    # max_steps -> status bit 1
+    o2 = Oracle(decay_net(1.0), OracleParams(eps_y=0.05, max_steps=5))
+    out = o2.integrate(1.0, 1.0, Y0, 1.0)
+    assert out["n_steps"][0] == 5 and out["status"][0] == 1
+    # t_hydro <= 0: nothing happens
+    out = o.integrate(1.0, 1.0, Y0, 0.0, dt=[0.3])
+    assert out["n_steps"][0] == 0 and out["dt"][0] == 0.3 and out["Y"][0, 0] == 1.0
+
+
+def test_zero_abundance_species_use_euler():
+    """S:Q8: Y_i = 0 => k_i = 0 => Euler: Y_i' = dt F+_i, however large dt is."""
+    o = Oracle(make_toy([1, 1, 1], [((0,), (1,)), ((1,), (2,))], [2.0, 1e6]))
+    Y = o.integrate_fixed(1.0, 1.0, [1.0, 0.0, 0.0], 10.0, 1)["Y"][0]
+    assert Y[1] == pytest.approx(10.0 * 2.0 * 1.0, rel=1e-15)  # fed from old Y_0
+    assert Y[0] == pytest.approx(1.0 / 21.0, rel=1e-15)        # k dt = 20 -> Eq. (3)
+    assert Y[2] == 0.0                                           # old Y_1 was 0
+
+
+def test_fp32_variant_tracks_fp64(hub150):
+    """P12 (PARITY UNPINNED: the paper gives no bound) - sanity only."""
+    o = Oracle(hub150)
+    Y0 = np.zeros((1, 150))
+    Y0[0, 3], Y0[0, 15] = 0.5 / 12, 0.5 / 16
+    a = o.integrate(7.0, 1e8, Y0, 1e-7, precision=64)
+    b = o.integrate(7.0, 1e8, Y0, 1e-7, precision=32)
+    X = a["Y"][0] * hub150.A
+    m = X > 1e-12
+    assert np.abs(b["Y"][0][m] / a["Y"][0][m] - 1).max() < 1e-2
+    assert abs(int(a["n_steps"][0]) - int(b["n_steps"][0])) <= max(2, a["n_steps"][0] // 50)
