@@ -1,0 +1,175 @@
+/*
+ * kinnet.h -- C ABI of the B200 batched explicit-asymptotic network integrator.
+ *
+ * One opaque net_t holds one reaction network (species/reaction tables, the
+ * compiled gather schedule and their device copies).  net_integrate advances
+ * `zones` independent copies of that network, each at its own fixed (T9, rho),
+ * over one hydro step with the explicit asymptotic method of
+ *   Brock, Belt, Billings, Guidry, "Explicit Integration with GPU Acceleration
+ *   for Large Kinetic Networks":
+ *   Eq. (1)  dy_i/dt = F+_i - F-_i = F+_i - k_i y_i
+ *   Eq. (3)  y_n = (y_{n-1} + F+ dt) / (1 + k dt)
+ *   branch   k_i dt < kappa -> forward Euler, else Eq. (3)
+ *   rates computed once per network integration, fluxes and F+/F- sums every
+ *   step, all inside one kernel
+ * The adaptive-dt controller and every reading of a point the paper leaves
+ * open are in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - All functions return NET_OK (0) or a negative NET_E* code; the message is
+ *     available from net_last_error() (thread-local).  No exception crosses the
+ *     ABI.  Per-zone numerical trouble is reported in status[z], not as a call
+ *     failure.
+ *   - "host" / "device" below says where a pointer must live.  The caller owns
+ *     every array it passes.  net_create copies the host tables; the net_t owns
+ *     its device copies.  net_integrate* allocate nothing, are asynchronous on
+ *     `cuda_stream` (a cudaStream_t cast to void*, NULL = default stream) and
+ *     never synchronise.  net_integrate_host is the synchronous end-to-end
+ *     variant taking host buffers.
+ *   - Y is zone-major [zones * n_species], molar abundances Y_i = X_i / A_i
+ *     (Eq. (2) with X the mass fraction); double when the net was
+ *     created with precision 64, float with precision 32 (the paper's
+ *     single-precision study).
+ *   - T9 = T / 1e9 K, rho in g cm^-3, times in s.
+ */
+#ifndef KINNET_H
+#define KINNET_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NET_OK 0
+#define NET_EINVAL (-1) /* bad argument or table (index out of range, n_react not in 1..3,
+                           n_prod not in 1..4, reaction not conserving A, size over limit) */
+#define NET_ENOMEM (-2)
+#define NET_ECUDA (-3)   /* CUDA runtime error, or no device copy (net_create_host) */
+
+#define NET_MAX_REACT 3
+#define NET_MAX_PROD 4
+#define NET_N_COEF 7
+#define NET_MAX_SPECIES 1024   /* one thread per species, one CTA per zone */
+#define NET_MAX_REACTIONS 65535
+
+#define NET_STATUS_MAX_STEPS 1 /* status bit: max_steps sub-steps taken before t_hydro */
+#define NET_STATUS_NONFINITE 2 /* status bit: a non-finite abundance was produced    */
+
+typedef struct net net_t;
+
+typedef struct {
+    double kappa;        /* branch threshold on k*dt (kappa = 1)            */
+    double eps_y;        /* dt control: max relative explicit change per step (0.05)      */
+    double y_floor;      /* dt control: abundance floor (1e-10)                           */
+    double growth;       /* dt control: dt may grow by at most this factor per step (2)   */
+    long long max_steps; /* per call and zone (1e7)                                       */
+    int precision;       /* 64 (default) or 32                                            */
+    int reserved;
+} net_params_t;
+
+/* Fill *p with the defaults listed above. */
+int net_default_params(net_params_t *p);
+
+/*
+ * Compile a network and upload it to the current CUDA device.
+ *   A        host [n_species]      mass numbers
+ *   n_react  host [n_reactions]    reactants per reaction, 1..3
+ *   react    host [n_reactions*3]  reactant species, repeats allowed, unused = -1
+ *   n_prod   host [n_reactions]    products per reaction, 1..4
+ *   prod     host [n_reactions*4]  product species, repeats allowed, unused = -1
+ *   coef     host [n_reactions*7]  a0..a6 of  ln R = a0 + a1/T9 + a2 T9^(-1/3)
+ *                                  + a3 T9^(1/3) + a4 T9 + a5 T9^(5/3) + a6 ln T9
+ *   params   host, NULL = defaults
+ * The full rate is R = p * rho^(n_react-1) * exp(ln R) with the statistical
+ * factor p = 1/prod(m!) over repeated reactants derived here (rate evaluation
+ * "from library parameters ... once for each network integration", PAPER.md
+ * L104, L197, L202).  This call also builds the host half of the hot path: the
+ * flux-slot layout and the deterministic species-to-reaction gather schedule
+ * (the flux sums of PAPER.md L197, L215-216; no atomics).
+ */
+int net_create(net_t **out, int n_species, const int *A, int n_reactions, const int *n_react,
+               const int *react, const int *n_prod, const int *prod, const double *coef,
+               const net_params_t *params);
+
+/* Same compile without touching CUDA (no device copy; net_integrate* on the
+ * result fail with NET_ECUDA).  For schedule inspection on machines without a GPU. */
+int net_create_host(net_t **out, int n_species, const int *A, int n_reactions,
+                    const int *n_react, const int *react, const int *n_prod, const int *prod,
+                    const double *coef, const net_params_t *params);
+
+void net_destroy(net_t *net);
+
+/*
+ * One hydro step of length t_hydro for every zone, adaptive network timestep
+ * (in = abundances, T, rho, dt_hydro, trial dt;
+ * out = abundances, final dt).
+ *   T9, rho  device [zones]          held constant over the step (operator split)
+ *   Y        device [zones*N]        in/out
+ *   dt       device [zones] or NULL  in: trial dt (<= 0 or NULL -> t_hydro);
+ *                                    out: last unclamped controller dt
+ *   n_steps  device [zones] or NULL  out: sub-steps taken
+ *   status   device [zones] or NULL  out: NET_STATUS_* bits
+ */
+int net_integrate(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                  double t_hydro, double *dt, int *n_steps, int *status, void *cuda_stream);
+
+/* Exactly n_steps sub-steps of size dt_fixed for every zone (parity mode). */
+int net_integrate_fixed(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                        double dt_fixed, long long n_steps, void *cuda_stream);
+
+/*
+ * End-to-end variant: every array is a HOST buffer (pinned for full copy
+ * speed).  Copies inputs to net-owned device scratch, integrates, copies the
+ * results back and synchronises before returning (the 154-in / 152-out float
+ * exchange of PAPER.md L106-110, batched).  Scratch grows on demand.
+ */
+int net_integrate_host(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                       double t_hydro, double *dt, int *n_steps, int *status);
+
+/* Rate evaluation alone: R device [zones * n_reactions] (reaction order), double. */
+int net_rates(net_t *net, int zones, const double *T9, const double *rho, double *R,
+              void *cuda_stream);
+
+/* Fluxes and sums alone for the given state: Fplus, Fminus device [zones*N],
+ * same type as Y (Eq. (1) terms). */
+int net_rhs(net_t *net, int zones, const double *T9, const double *rho, const void *Y,
+            void *Fplus, void *Fminus, void *cuda_stream);
+
+/* Shape of the compiled schedule (all host-side facts). */
+typedef struct {
+    int n_species, n_reactions;
+    int threads;         /* threads per zone (= CTA size), multiple of 32            */
+    int flux_slots;      /* flux slots per thread                                    */
+    int slots_2body;     /* slots [0, slots_2body) multiply a 2nd reactant           */
+    int slots_3body;     /* slots [0, slots_3body) multiply a 3rd reactant           */
+    int n_entries;       /* gather entries = sum over reactions of reactants+products */
+    int n_big_species;   /* species whose sums are reduced across the CTA            */
+    int n_entries_big;   /* entries served by own-slot readback                      */
+    int small_max;       /* longest per-thread small-row gather list                 */
+    int readback_max;    /* longest per-thread readback list                         */
+    int smem_bytes;      /* dynamic shared memory per zone at this precision         */
+    int zones_per_sm;    /* co-resident CTAs per SM (0 without a device)             */
+} net_schedule_info_t;
+
+int net_schedule_info(const net_t *net, net_schedule_info_t *info);
+
+/*
+ * Copy one schedule table into out (host, capacity in ints); returns the
+ * number of ints the table holds (call with cap = 0 to size), negative on error.
+ *   "flux_rxn"    [flux_slots*threads]     reaction of slot j of thread t, -1 = empty
+ *   "flux_react"  [flux_slots*threads*3]   its reactant species, n_species = the constant 1
+ *   "owner"       [threads]                species owned by thread t, -1 = none
+ *   "small_plus"  [threads]                F+ small-row entries of thread t
+ *   "small_minus" [threads]                F- small-row entries
+ *   "small_src"   [small_max*threads]      entry e of thread t = flux index slot*threads+thread
+ *   "big_species" [n_big_species]
+ *   "big_cnt"     [2*n_big_species*threads] readback entries of thread t for row 2*s+{0:+,1:-}
+ *   "big_slot"    [readback_max*threads]   own flux slot of readback entry e of thread t
+ */
+int net_schedule_table(const net_t *net, const char *name, int *out, int cap);
+
+const char *net_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KINNET_H */

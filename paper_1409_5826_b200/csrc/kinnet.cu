@@ -1,0 +1,660 @@
+// kinnet.cu -- sm_100a kernels and the C ABI of include/kinnet.h.
+//
+// One CTA integrates one zone over the whole hydro step (PAPER.md L104-110,
+// Fig. 3: rates once, then the sub-step loop entirely on the GPU); the whole
+// batch of zones is ONE launch instead of the paper's one asynchronous launch
+// per network from OpenMP threads.
+//
+// Sub-step (Eq. (1), Eq. (3)), three barriers:
+//   flux     f[j*T+t] = R * Y[a] * Y[b] * Y[c]        every thread, rs slots
+//   ---------------------------------------------------------------- barrier
+//   sums     small rows: the owner thread gathers F+_i, F-_i from f
+//            big rows:   own-column readback + warp butterfly -> red[warp][row]
+//   dt       candidate eps*max(Y,floor)/|F+ - F-| , warp min -> redmin[warp]
+//   ---------------------------------------------------------------- barrier
+//   finalize every warp redundantly: min over warps and big species -> dt
+//   update   k dt >= kappa ? (Y + dt F+)/(1 + k dt) : Y + dt (F+ - F-)
+//   ---------------------------------------------------------------- barrier
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/kinnet.h"
+#include "schedule.h"
+
+namespace {
+
+using kinnet::Schedule;
+
+thread_local std::string g_last_error;
+
+int fail(int code, const std::string& msg) {
+    g_last_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                      \
+    do {                                                                                    \
+        cudaError_t e_ = (expr);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(NET_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));     \
+    } while (0)
+
+constexpr int kMaxBig = kinnet::kMaxBigSpecies;
+constexpr int kRedStride = 2 * kMaxBig;
+
+enum Mode { kAdaptive = 0, kFixed = 1, kRhs = 2, kRates = 3 };
+
+struct KParams {
+    // schedule
+    int N, M, T, W, rs, j2, j3, nbs;
+    int big_species[kMaxBig];
+    const int32_t* flux_rxn;
+    const ushort4* flux_react;
+    const double* coef;
+    const int32_t* owner;
+    const uint16_t* small_plus;
+    const uint16_t* small_minus;
+    const uint16_t* small_src;
+    const uint8_t* big_cnt;
+    const uint8_t* big_slot;
+    // zones
+    const double* T9;
+    const double* rho;
+    void* Y;
+    double* dt;
+    int* n_steps;
+    int* status;
+    void* Fplus;
+    void* Fminus;
+    double* Rout;
+    double t_hydro, dt_fixed;
+    long long n_fixed;
+    // integrator parameters
+    double kappa, eps_y, y_floor, growth;
+    long long max_steps;
+};
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Minimum over the warp of non-negative doubles (or +inf; NaN loses): the bit
+// patterns order like unsigned integers, so two REDUX.MIN do it.
+__device__ __forceinline__ double warp_min_pos(double c) {
+    const unsigned hi = static_cast<unsigned>(__double2hiint(c));
+    const unsigned mh = __reduce_min_sync(0xffffffffu, hi);
+    const unsigned lo = (hi == mh) ? static_cast<unsigned>(__double2loint(c)) : 0xffffffffu;
+    const unsigned ml = __reduce_min_sync(0xffffffffu, lo);
+    return __hiloint2double(static_cast<int>(mh), static_cast<int>(ml));
+}
+
+__host__ __device__ inline int real_words_before_flux(int N) { return (N + 1 + 3) & ~3; }
+
+template <typename real>
+size_t smem_bytes(const Schedule& S) {
+    return 64 * sizeof(double) +
+           sizeof(real) * (static_cast<size_t>(real_words_before_flux(S.N)) +
+                           2 * static_cast<size_t>(S.rs) * S.T +
+                           static_cast<size_t>(S.W) * kRedStride);
+}
+
+template <typename real, int MODE, int TB>
+__global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int T = p.T, N = p.N, W = p.W, rs = p.rs, slots = rs * T, nbs = p.nbs;
+    const int z = blockIdx.x;
+
+    double* redmin = reinterpret_cast<double*>(smem_raw);            // [32] per-warp dt minima
+    double* ybig = redmin + 32;                                      // [kMaxBig] start-of-step Y of big species
+    real* Ybuf = reinterpret_cast<real*>(redmin + 64);               // [N] + constant one
+    real* Rbuf = Ybuf + real_words_before_flux(N);                   // [rs*T]
+    real* fbuf = Rbuf + slots;                                       // [rs*T]
+    real* red = fbuf + slots;                                        // [W][kRedStride]
+
+    // ---- S1: rates, once per zone per call -----
+    {
+        const double T9 = p.T9[z], rho = p.rho[z];
+        const double t13 = cbrt(T9);
+        const double t53 = T9 * t13 * t13;
+        const double lnT = log(T9), lnrho = log(rho);
+        for (int j = 0; j < rs; ++j) {
+            const int idx = j * T + tid;
+            const double* c = p.coef + idx;
+            const double lnR = c[0] + c[1 * (size_t)slots] / T9 + c[2 * (size_t)slots] / t13 +
+                               c[3 * (size_t)slots] * t13 + c[4 * (size_t)slots] * T9 +
+                               c[5 * (size_t)slots] * t53 + c[6 * (size_t)slots] * lnT;
+            const double R = exp(c[7 * (size_t)slots] * lnrho + lnR);
+            if (MODE == kRates) {
+                const int r = p.flux_rxn[idx];
+                if (r >= 0) p.Rout[(size_t)z * p.M + r] = R;
+            } else {
+                Rbuf[idx] = static_cast<real>(R);
+            }
+        }
+        if (MODE == kRates) return;
+    }
+
+    // ---- S6: zone state in ----------------------------------------------
+    real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
+    for (int i = tid; i < N; i += T) Ybuf[i] = Yg[i];
+    if (tid == 0) Ybuf[N] = static_cast<real>(1);
+    const int own = p.owner[tid];
+    const int np = p.small_plus[tid], nm = p.small_minus[tid];
+    const bool is_big = (tid >= W && tid < W + nbs);
+    unsigned bigcnt[2 * kMaxBig];
+#pragma unroll
+    for (int b = 0; b < 2 * kMaxBig; ++b)
+        bigcnt[b] = (b < 2 * nbs) ? p.big_cnt[(size_t)b * T + tid] : 0u;
+    __syncthreads();
+    real y = (own >= 0) ? Ybuf[own] : static_cast<real>(0);
+
+    const real kappa = static_cast<real>(p.kappa);
+    const real eps_y = static_cast<real>(p.eps_y);
+    const real y_floor = static_cast<real>(p.y_floor);
+
+    double t = 0.0, dt_prev = 0.0;
+    long long steps = 0;
+    int status = 0;
+    bool run = true;
+    if (MODE == kAdaptive) {
+        const double dt_in = p.dt ? p.dt[z] : 0.0;
+        dt_prev = (dt_in > 0.0) ? dt_in : p.t_hydro;
+        run = p.t_hydro > 0.0;
+        if (!run) dt_prev = dt_in;  // nothing to do: the trial dt is returned unchanged
+    } else if (MODE == kFixed) {
+        run = p.n_fixed > 0;
+    }
+
+    while (run) {
+        // ---- S2: fluxes ------------------------------------
+        for (int j = 0; j < rs; ++j) {
+            const int idx = j * T + tid;
+            const ushort4 re = __ldg(p.flux_react + idx);
+            real v = Rbuf[idx] * Ybuf[re.x];
+            if (j < p.j2) v = v * Ybuf[re.y];
+            if (j < p.j3) v = v * Ybuf[re.z];
+            fbuf[idx] = v;
+        }
+        __syncthreads();
+
+        // ---- S3: sums F+_i, F-_i (Eq. (1)) --------
+        real Fp = 0, Fm = 0;
+        {
+            int e = 0;
+            for (; e < np; ++e) Fp += fbuf[__ldg(p.small_src + (size_t)e * T + tid)];
+            for (; e < np + nm; ++e) Fm += fbuf[__ldg(p.small_src + (size_t)e * T + tid)];
+        }
+        if (nbs > 0) {
+            int e = 0;
+#pragma unroll
+            for (int b = 0; b < 2 * kMaxBig; ++b) {
+                if (b < 2 * nbs) {
+                    real acc = 0;
+                    for (unsigned q = 0; q < bigcnt[b]; ++q, ++e)
+                        acc += fbuf[(int)__ldg(p.big_slot + (size_t)e * T + tid) * T + tid];
+                    acc = warp_sum(acc);
+                    if (lane == 0) red[warp * kRedStride + b] = acc;
+                }
+            }
+        }
+        // ---- S5: dt candidates of the small species ------------------------
+        if (MODE == kAdaptive) {
+            double c = INFINITY;
+            if (own >= 0 && !is_big) {
+                real a = Fp - Fm;
+                a = a < 0 ? -a : a;
+                if (a > 0) c = static_cast<double>(eps_y * (y > y_floor ? y : y_floor) / a);
+            }
+            c = warp_min_pos(c);
+            if (lane == 0) redmin[warp] = c;
+            // Ybuf[big species] is overwritten by its owner right after the barrier
+            // while other warps still need the old value: hand it over separately.
+            if (is_big) ybig[tid - W] = static_cast<double>(y);
+        }
+        __syncthreads();
+
+        // ---- finalize: big species sums, zone-wide dt -----------------------
+        real bFp = 0, bFm = 0;
+        double cand = INFINITY;
+        if (lane >= W && lane < W + nbs) {
+            const int s = lane - W;
+            for (int w = 0; w < W; ++w) {  // fixed order over warps
+                bFp += red[w * kRedStride + 2 * s];
+                bFm += red[w * kRedStride + 2 * s + 1];
+            }
+            if (MODE == kAdaptive) {
+                const real yb = static_cast<real>(ybig[s]);
+                real a = bFp - bFm;
+                a = a < 0 ? -a : a;
+                if (a > 0) cand = static_cast<double>(eps_y * (yb > y_floor ? yb : y_floor) / a);
+            }
+        } else if (MODE == kAdaptive && lane < W) {
+            cand = redmin[lane];
+        }
+        if (is_big) {  // warp 0, lane == tid: this lane just summed its own rows
+            Fp = bFp;
+            Fm = bFm;
+        }
+        if (MODE == kRhs) {
+            if (own >= 0) {
+                reinterpret_cast<real*>(p.Fplus)[(size_t)z * N + own] = Fp;
+                reinterpret_cast<real*>(p.Fminus)[(size_t)z * N + own] = Fm;
+            }
+            return;
+        }
+
+        double dts;
+        bool last;
+        if (MODE == kAdaptive) {
+            const double cmin = warp_min_pos(cand);
+            double dt_ctrl = p.growth * dt_prev;
+            if (cmin < dt_ctrl) dt_ctrl = cmin;
+            const double rem = p.t_hydro - t;
+            if (dt_ctrl >= rem * (1.0 - 1e-12)) {
+                dts = rem;
+                last = true;
+            } else {
+                dts = dt_ctrl;
+                last = false;
+            }
+            dt_prev = dt_ctrl;
+        } else {
+            dts = p.dt_fixed;
+            last = (steps + 1 >= p.n_fixed);
+        }
+
+        // ---- S4: update (Eq. (3)) -------------------------
+        if (own >= 0) {
+            const real h = static_cast<real>(dts);
+            const real k = (y > 0) ? Fm / y : static_cast<real>(0);
+            const real kdt = k * h;
+            if (kdt >= kappa)
+                y = (y + h * Fp) / (static_cast<real>(1) + kdt);
+            else
+                y = y + h * (Fp - Fm);
+            Ybuf[own] = y;
+        }
+        t = last ? p.t_hydro : t + dts;
+        ++steps;
+        if (last) run = false;
+        else if (MODE == kAdaptive && steps >= p.max_steps) {
+            status |= NET_STATUS_MAX_STEPS;
+            run = false;
+        }
+        __syncthreads();
+    }
+
+    // ---- S6: zone state out ----------------------------------------------
+    const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
+    if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    for (int i = tid; i < N; i += T) Yg[i] = Ybuf[i];
+    if (tid == 0) {
+        if (MODE == kAdaptive && p.dt) p.dt[z] = dt_prev;
+        if (p.n_steps) p.n_steps[z] = static_cast<int>(steps);
+        if (p.status) p.status[z] = status;
+    }
+}
+
+struct DeviceTables {
+    int32_t* flux_rxn = nullptr;
+    ushort4* flux_react = nullptr;
+    double* coef = nullptr;
+    int32_t* owner = nullptr;
+    uint16_t* small_plus = nullptr;
+    uint16_t* small_minus = nullptr;
+    uint16_t* small_src = nullptr;
+    uint8_t* big_cnt = nullptr;
+    uint8_t* big_slot = nullptr;
+};
+
+}  // namespace
+
+struct net {
+    Schedule S;
+    net_params_t P;
+    bool has_device = false;
+    int device = -1;
+    int zones_per_sm = 0;
+    DeviceTables D;
+    // scratch of net_integrate_host
+    cudaStream_t host_stream = nullptr;
+    int scratch_zones = 0;
+    double *sT9 = nullptr, *srho = nullptr, *sdt = nullptr;
+    void* sY = nullptr;
+    int *ssteps = nullptr, *sstatus = nullptr;
+};
+
+namespace {
+
+template <typename T>
+int upload(T** dst, const void* src, size_t count) {
+    CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(dst), std::max<size_t>(count, 1) * sizeof(T)));
+    if (count) CUDA_TRY(cudaMemcpy(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice));
+    return NET_OK;
+}
+
+typedef void (*kernel_fn)(const KParams);
+
+template <typename real, int MODE>
+kernel_fn pick_block(int T) {
+    if (T <= 256) return zone_kernel<real, MODE, 256>;
+    if (T <= 512) return zone_kernel<real, MODE, 512>;
+    return zone_kernel<real, MODE, 1024>;
+}
+
+template <int MODE>
+kernel_fn pick_kernel(const net* n) {
+    if (MODE == kRates) return pick_block<double, MODE>(n->S.T);
+    return n->P.precision == 32 ? pick_block<float, MODE>(n->S.T) : pick_block<double, MODE>(n->S.T);
+}
+
+size_t net_smem(const net* n) {
+    return n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
+}
+
+int prepare_kernels(net* n) {
+    const size_t smem = net_smem(n);
+    kernel_fn fns[4] = {pick_kernel<kAdaptive>(n), pick_kernel<kFixed>(n), pick_kernel<kRhs>(n),
+                        pick_kernel<kRates>(n)};
+    for (kernel_fn f : fns) {
+        const size_t need = (f == fns[3]) ? smem_bytes<double>(n->S) : smem;
+        CUDA_TRY(cudaFuncSetAttribute(reinterpret_cast<const void*>(f),
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      static_cast<int>(need)));
+    }
+    int nb = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+        &nb, reinterpret_cast<const void*>(fns[0]), n->S.T, smem));
+    n->zones_per_sm = nb;
+    return NET_OK;
+}
+
+void fill_params(const net* n, KParams& k) {
+    const Schedule& S = n->S;
+    std::memset(&k, 0, sizeof(k));
+    k.N = S.N; k.M = S.M; k.T = S.T; k.W = S.W; k.rs = S.rs; k.j2 = S.j2; k.j3 = S.j3;
+    k.nbs = S.nbs;
+    for (int s = 0; s < S.nbs; ++s) k.big_species[s] = S.big_species[s];
+    k.flux_rxn = n->D.flux_rxn;
+    k.flux_react = n->D.flux_react;
+    k.coef = n->D.coef;
+    k.owner = n->D.owner;
+    k.small_plus = n->D.small_plus;
+    k.small_minus = n->D.small_minus;
+    k.small_src = n->D.small_src;
+    k.big_cnt = n->D.big_cnt;
+    k.big_slot = n->D.big_slot;
+    k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
+    k.growth = n->P.growth; k.max_steps = n->P.max_steps;
+}
+
+template <int MODE>
+int launch(net* n, int zones, KParams& k, void* stream) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+    if (zones == 0) return NET_OK;
+    if (!k.T9 || !k.rho) return fail(NET_EINVAL, "null T9/rho");
+    const size_t smem = (MODE == kRates) ? smem_bytes<double>(n->S) : net_smem(n);
+    kernel_fn f = pick_kernel<MODE>(n);
+    f<<<zones, n->S.T, smem, static_cast<cudaStream_t>(stream)>>>(k);
+    CUDA_TRY(cudaGetLastError());
+    return NET_OK;
+}
+
+int create_common(net_t** out, int N, const int* A, int M, const int* n_react, const int* react,
+                  const int* n_prod, const int* prod, const double* coef,
+                  const net_params_t* params, bool device) {
+    if (!out) return fail(NET_EINVAL, "null out pointer");
+    *out = nullptr;
+    net* n = new (std::nothrow) net();
+    if (!n) return fail(NET_ENOMEM, "out of host memory");
+    if (params) n->P = *params; else net_default_params(&n->P);
+    if (n->P.precision == 0) n->P.precision = 64;
+    if (n->P.precision != 64 && n->P.precision != 32) {
+        delete n;
+        return fail(NET_EINVAL, "precision must be 64 or 32");
+    }
+    if (!(n->P.kappa > 0) || !(n->P.eps_y > 0) || !(n->P.y_floor > 0) || !(n->P.growth > 1) ||
+        n->P.max_steps < 1 || n->P.max_steps > 2000000000LL) {
+        delete n;
+        return fail(NET_EINVAL, "bad integrator parameter");
+    }
+    std::string err;
+    int rc;
+    try {
+        rc = kinnet::build_schedule(N, A, M, n_react, react, n_prod, prod, coef, n->S, err);
+    } catch (const std::bad_alloc&) {
+        delete n;
+        return fail(NET_ENOMEM, "out of host memory");
+    }
+    if (rc != NET_OK) {
+        delete n;
+        return fail(rc, err);
+    }
+    if (net_smem(n) > 227 * 1024) {
+        delete n;
+        return fail(NET_EINVAL, "network too large for one CTA's shared memory");
+    }
+    if (device) {
+        const Schedule& S = n->S;
+        rc = NET_OK;
+        if (cudaGetDevice(&n->device) != cudaSuccess) rc = fail(NET_ECUDA, "no CUDA device");
+        if (rc == NET_OK) rc = upload(&n->D.flux_rxn, S.flux_rxn.data(), S.flux_rxn.size());
+        if (rc == NET_OK)
+            rc = upload(&n->D.flux_react, S.flux_react.data(), S.flux_react.size() / 4);
+        if (rc == NET_OK) rc = upload(&n->D.coef, S.coef.data(), S.coef.size());
+        if (rc == NET_OK) rc = upload(&n->D.owner, S.owner.data(), S.owner.size());
+        if (rc == NET_OK) rc = upload(&n->D.small_plus, S.small_plus.data(), S.small_plus.size());
+        if (rc == NET_OK) rc = upload(&n->D.small_minus, S.small_minus.data(), S.small_minus.size());
+        if (rc == NET_OK) rc = upload(&n->D.small_src, S.small_src.data(), S.small_src.size());
+        if (rc == NET_OK) rc = upload(&n->D.big_cnt, S.big_cnt.data(), S.big_cnt.size());
+        if (rc == NET_OK) rc = upload(&n->D.big_slot, S.big_slot.data(), S.big_slot.size());
+        if (rc == NET_OK) {
+            n->has_device = true;
+            rc = prepare_kernels(n);
+        }
+        if (rc != NET_OK) {
+            std::string keep = g_last_error;
+            net_destroy(n);
+            g_last_error = keep;
+            return rc;
+        }
+    }
+    *out = n;
+    return NET_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int net_default_params(net_params_t* p) {
+    if (!p) return fail(NET_EINVAL, "null params");
+    p->kappa = 1.0;
+    p->eps_y = 0.05;
+    p->y_floor = 1e-10;
+    p->growth = 2.0;
+    p->max_steps = 10000000LL;
+    p->precision = 64;
+    p->reserved = 0;
+    return NET_OK;
+}
+
+int net_create(net_t** out, int n_species, const int* A, int n_reactions, const int* n_react,
+               const int* react, const int* n_prod, const int* prod, const double* coef,
+               const net_params_t* params) {
+    return create_common(out, n_species, A, n_reactions, n_react, react, n_prod, prod, coef,
+                         params, true);
+}
+
+int net_create_host(net_t** out, int n_species, const int* A, int n_reactions,
+                    const int* n_react, const int* react, const int* n_prod, const int* prod,
+                    const double* coef, const net_params_t* params) {
+    return create_common(out, n_species, A, n_reactions, n_react, react, n_prod, prod, coef,
+                         params, false);
+}
+
+void net_destroy(net_t* n) {
+    if (!n) return;
+    if (n->has_device) {
+        cudaFree(n->D.flux_rxn); cudaFree(n->D.flux_react); cudaFree(n->D.coef);
+        cudaFree(n->D.owner); cudaFree(n->D.small_plus); cudaFree(n->D.small_minus);
+        cudaFree(n->D.small_src); cudaFree(n->D.big_cnt); cudaFree(n->D.big_slot);
+        cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
+        cudaFree(n->ssteps); cudaFree(n->sstatus);
+        if (n->host_stream) cudaStreamDestroy(n->host_stream);
+    }
+    delete n;
+}
+
+int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                  double t_hydro, double* dt, int* n_steps, int* status, void* stream) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
+    if (!(t_hydro == t_hydro)) return fail(NET_EINVAL, "t_hydro is NaN");
+    KParams k;
+    fill_params(n, k);
+    k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
+    k.t_hydro = t_hydro;
+    return launch<kAdaptive>(n, zones, k, stream);
+}
+
+int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                        double dt_fixed, long long n_steps, void* stream) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
+    if (n_steps < 0) return fail(NET_EINVAL, "n_steps < 0");
+    KParams k;
+    fill_params(n, k);
+    k.T9 = T9; k.rho = rho; k.Y = Y;
+    k.dt_fixed = dt_fixed; k.n_fixed = n_steps;
+    return launch<kFixed>(n, zones, k, stream);
+}
+
+int net_rates(net_t* n, int zones, const double* T9, const double* rho, double* R, void* stream) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (zones > 0 && !R) return fail(NET_EINVAL, "null R");
+    KParams k;
+    fill_params(n, k);
+    k.T9 = T9; k.rho = rho; k.Rout = R;
+    return launch<kRates>(n, zones, k, stream);
+}
+
+int net_rhs(net_t* n, int zones, const double* T9, const double* rho, const void* Y, void* Fplus,
+            void* Fminus, void* stream) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (zones > 0 && (!Y || !Fplus || !Fminus)) return fail(NET_EINVAL, "null Y/Fplus/Fminus");
+    KParams k;
+    fill_params(n, k);
+    k.T9 = T9; k.rho = rho; k.Y = const_cast<void*>(Y); k.Fplus = Fplus; k.Fminus = Fminus;
+    return launch<kRhs>(n, zones, k, stream);
+}
+
+int net_integrate_host(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                       double t_hydro, double* dt, int* n_steps, int* status) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+    if (zones == 0) return NET_OK;
+    if (!T9 || !rho || !Y) return fail(NET_EINVAL, "null T9/rho/Y");
+    const size_t ysz = (n->P.precision == 32 ? sizeof(float) : sizeof(double)) * (size_t)n->S.N;
+    if (!n->host_stream) CUDA_TRY(cudaStreamCreateWithFlags(&n->host_stream, cudaStreamNonBlocking));
+    if (zones > n->scratch_zones) {
+        cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
+        cudaFree(n->ssteps); cudaFree(n->sstatus);
+        n->sT9 = n->srho = n->sdt = nullptr; n->sY = nullptr; n->ssteps = n->sstatus = nullptr;
+        n->scratch_zones = 0;
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->sT9), sizeof(double) * zones));
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->srho), sizeof(double) * zones));
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->sdt), sizeof(double) * zones));
+        CUDA_TRY(cudaMalloc(&n->sY, ysz * zones));
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->ssteps), sizeof(int) * zones));
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->sstatus), sizeof(int) * zones));
+        n->scratch_zones = zones;
+    }
+    cudaStream_t s = n->host_stream;
+    CUDA_TRY(cudaMemcpyAsync(n->sT9, T9, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaMemcpyAsync(n->srho, rho, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaMemcpyAsync(n->sY, Y, ysz * zones, cudaMemcpyHostToDevice, s));
+    if (dt) CUDA_TRY(cudaMemcpyAsync(n->sdt, dt, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
+    else CUDA_TRY(cudaMemsetAsync(n->sdt, 0, sizeof(double) * zones, s));
+    int rc = net_integrate(n, zones, n->sT9, n->srho, n->sY, t_hydro, n->sdt, n->ssteps,
+                           n->sstatus, s);
+    if (rc != NET_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(Y, n->sY, ysz * zones, cudaMemcpyDeviceToHost, s));
+    if (dt) CUDA_TRY(cudaMemcpyAsync(dt, n->sdt, sizeof(double) * zones, cudaMemcpyDeviceToHost, s));
+    if (n_steps)
+        CUDA_TRY(cudaMemcpyAsync(n_steps, n->ssteps, sizeof(int) * zones, cudaMemcpyDeviceToHost, s));
+    if (status)
+        CUDA_TRY(cudaMemcpyAsync(status, n->sstatus, sizeof(int) * zones, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return NET_OK;
+}
+
+int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
+    if (!n || !info) return fail(NET_EINVAL, "null argument");
+    const Schedule& S = n->S;
+    info->n_species = S.N;
+    info->n_reactions = S.M;
+    info->threads = S.T;
+    info->flux_slots = S.rs;
+    info->slots_2body = S.j2;
+    info->slots_3body = S.j3;
+    info->n_entries = S.n_entries;
+    info->n_big_species = S.nbs;
+    info->n_entries_big = S.n_entries_big;
+    info->small_max = S.small_max;
+    info->readback_max = S.readback_max;
+    info->smem_bytes = static_cast<int>(net_smem(n));
+    info->zones_per_sm = n->zones_per_sm;
+    return NET_OK;
+}
+
+int net_schedule_table(const net_t* n, const char* name, int* out, int cap) {
+    if (!n || !name) return fail(NET_EINVAL, "null argument");
+    const Schedule& S = n->S;
+    const std::string key(name);
+    int count = -1;
+    auto emit = [&](auto const& vec, size_t stride, size_t take) {
+        // copies `take` of every `stride` elements
+        const size_t groups = stride ? vec.size() / stride : 0;
+        count = static_cast<int>(groups * take);
+        if (out && cap >= count)
+            for (size_t g = 0, o = 0; g < groups; ++g)
+                for (size_t q = 0; q < take; ++q) out[o++] = static_cast<int>(vec[g * stride + q]);
+    };
+    if (key == "flux_rxn") emit(S.flux_rxn, 1, 1);
+    else if (key == "flux_react") emit(S.flux_react, 4, 3);
+    else if (key == "owner") emit(S.owner, 1, 1);
+    else if (key == "small_plus") emit(S.small_plus, 1, 1);
+    else if (key == "small_minus") emit(S.small_minus, 1, 1);
+    else if (key == "small_src") {
+        if (S.small_max == 0) count = 0; else emit(S.small_src, 1, 1);
+    } else if (key == "big_species") emit(S.big_species, 1, 1);
+    else if (key == "big_cnt") {
+        if (S.nbs == 0) count = 0; else emit(S.big_cnt, 1, 1);
+    } else if (key == "big_slot") {
+        if (S.readback_max == 0) count = 0; else emit(S.big_slot, 1, 1);
+    } else return fail(NET_EINVAL, "unknown schedule table '" + key + "'");
+    if (out && cap < count) return fail(NET_EINVAL, "output buffer too small");
+    return count;
+}
+
+const char* net_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

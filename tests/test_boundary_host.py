@@ -1,0 +1,167 @@
+"""CPU-only checks of the C-ABI library: it loads, exports what include/kinnet.h
+declares, rejects bad tables, and its compiled schedule (the host half of the
+hot path) contains every (species, sign, reaction) entry exactly once."""
+import os
+import re
+from collections import Counter
+
+import numpy as np
+import pytest
+
+import paper_1409_5826_b200 as K
+from gen import make_toy
+from gen.configs import network
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "kinnet.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(net_[a-z_]+)\s*\(", header))
+    assert declared == set(K.EXPORTS)
+    for name in declared:
+        assert hasattr(K.lib, name), name
+
+
+def test_default_params():
+    p = K.net_default_params()
+    assert (p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision) == (
+        1.0, 0.05, 1e-10, 2.0, 10_000_000, 64)
+
+
+def test_integrate_without_device_copy_fails_loudly(g16):
+    net = K.Net(g16, host_only=True)
+    z = np.zeros(1)
+    with pytest.raises(K.KinnetError) as e:
+        net.net_integrate(1, z, z, np.zeros(16), 1e-6, stream=0)
+    assert e.value.code == K.NET_ECUDA and "no device copy" in str(e.value)
+
+
+def _broken(net, **kw):
+    import copy
+
+    bad = copy.deepcopy(net)
+    for k, v in kw.items():
+        setattr(bad, k, v)
+    return bad
+
+
+def test_invalid_tables_are_rejected(g16):
+    re_ = g16.react.copy()
+    re_[0, 0] = 99
+    with pytest.raises(K.KinnetError) as e:
+        K.Net(_broken(g16, react=re_), host_only=True)
+    assert e.value.code == K.NET_EINVAL and "reactant index" in str(e.value)
+    nr = g16.n_react.copy()
+    nr[3] = 4
+    with pytest.raises(K.KinnetError):
+        K.Net(_broken(g16, n_react=nr), host_only=True)
+    npd = g16.n_prod.copy()
+    npd[3] = 0
+    with pytest.raises(K.KinnetError):
+        K.Net(_broken(g16, n_prod=npd), host_only=True)
+    A = g16.A.copy()
+    A[5] += 1
+    with pytest.raises(K.KinnetError) as e:
+        K.Net(_broken(g16, A=A), host_only=True)
+    assert "conserve" in str(e.value)
+    co = g16.coef.copy()
+    co[0, 0] = np.nan
+    with pytest.raises(K.KinnetError):
+        K.Net(_broken(g16, coef=co), host_only=True)
+    with pytest.raises(K.KinnetError):
+        K.Net(g16, K.NetParams(precision=16), host_only=True)
+    with pytest.raises(K.KinnetError):
+        K.Net(g16, K.NetParams(kappa=0.0), host_only=True)
+
+
+def expected_entries(net):
+    ent = Counter()
+    for r in range(net.n_reactions):
+        for s in net.react[r, : net.n_react[r]]:
+            ent[(int(s), "-", r)] += 1
+        for s in net.prod[r, : net.n_prod[r]]:
+            ent[(int(s), "+", r)] += 1
+    return ent
+
+
+def schedule_entries(net, kn):
+    info = kn.schedule_info()
+    T = info["threads"]
+    rxn = kn.schedule_table("flux_rxn")
+    owner = kn.schedule_table("owner")
+    sp, sm = kn.schedule_table("small_plus"), kn.schedule_table("small_minus")
+    src = kn.schedule_table("small_src").reshape(-1, T) if info["small_max"] else None
+    ent = Counter()
+    for t in range(T):
+        for e in range(sp[t] + sm[t]):
+            assert owner[t] >= 0
+            r = rxn[src[e, t]]
+            assert r >= 0
+            ent[(int(owner[t]), "+" if e < sp[t] else "-", int(r))] += 1
+    nbs = info["n_big_species"]
+    if nbs:
+        bs = kn.schedule_table("big_species")
+        cnt = kn.schedule_table("big_cnt").reshape(2 * nbs, T)
+        slot = kn.schedule_table("big_slot").reshape(-1, T)
+        for t in range(T):
+            e = 0
+            for b in range(2 * nbs):
+                for _ in range(cnt[b, t]):
+                    r = rxn[slot[e, t] * T + t]  # own column only
+                    assert r >= 0
+                    ent[(int(bs[b // 2]), "+" if b % 2 == 0 else "-", int(r))] += 1
+                    e += 1
+            assert e <= info["readback_max"]
+    return ent, info
+
+
+@pytest.mark.parametrize("name", ["g16", "hub150", "hub365"])
+def test_schedule_round_trip(name):
+    net = network(name)
+    kn = K.Net(net, host_only=True)
+    got, info = schedule_entries(net, kn)
+    want = expected_entries(net)
+    assert got == want
+    assert info["n_entries"] == sum(want.values())
+    T, rs = info["threads"], info["flux_slots"]
+    assert T % 32 == 0 and T >= net.n_species and rs * T >= net.n_reactions
+    # every reaction sits in exactly one flux slot, with its reactants in order
+    rxn = kn.schedule_table("flux_rxn")
+    assert sorted(r for r in rxn if r >= 0) == list(range(net.n_reactions))
+    fr = kn.schedule_table("flux_react").reshape(-1, 3)
+    for idx, r in enumerate(rxn):
+        j = idx // T
+        if r < 0:
+            assert (fr[idx] == net.n_species).all()
+            continue
+        n = net.n_react[r]
+        assert list(fr[idx, :n]) == list(net.react[r, :n]) and (fr[idx, n:] == net.n_species).all()
+        assert n == 1 or j < info["slots_2body"]
+        assert n <= 2 or j < info["slots_3body"]
+    # each species has exactly one owner thread; big species sit at W .. W+nbs-1
+    owner = kn.schedule_table("owner")
+    assert sorted(o for o in owner if o >= 0) == list(range(net.n_species))
+    W = T // 32
+    if info["n_big_species"]:
+        assert list(owner[W: W + info["n_big_species"]]) == list(kn.schedule_table("big_species"))
+
+
+def test_schedule_hub_rows_are_the_big_ones(hub150):
+    """p, n, 4He have hundreds of fluxes, the rest a few tens."""
+    kn = K.Net(hub150, host_only=True)
+    info = kn.schedule_info()
+    assert list(kn.schedule_table("big_species")) == [0, 1, 2]
+    assert info["n_entries_big"] > 0.35 * info["n_entries"]
+    assert info["small_max"] <= 40
+    # readback lists are balanced: within 2x of the mean
+    assert info["readback_max"] <= 2 * info["n_entries_big"] / info["threads"] + 2
+
+
+def test_three_alpha_multiplicity_in_schedule():
+    """3a -> C and back: the alpha rows receive the flux three times (S:Q2)."""
+    net = make_toy([4, 12], [((0, 0, 0), (1,)), ((1,), (0, 0, 0))], [7.0, 0.5])
+    kn = K.Net(net, host_only=True)
+    got, _ = schedule_entries(net, kn)
+    assert got[(0, "-", 0)] == 3 and got[(0, "+", 1)] == 3 and got[(1, "+", 0)] == 1

