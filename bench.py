@@ -1,0 +1,343 @@
+"""bench.py -- zone-networks integrated per second over one hydro step
+(150 species / 1604 reactions, fp64): BASELINE.json's metric on configs[3]
+(16384 zones, one hydro step of 1e-6 s, seeded synthetic network and profile).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one net_integrate call over the whole batch (rates, then every
+sub-step of every zone: the whole hot path).  Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "zone-networks integrated per second over one hydro step (150sp/1604rx, fp64)"
+UNIT = "zone-networks/s"
+ZONES_PER_GPU = 16384
+T_HYDRO = 1e-6
+PROFILE_SEED = 4
+
+# Algorithmic work per zone per sub-step: one multiply per
+# reactant of every reaction, one add per F+/F- entry, ~10 flops per species for
+# k, the branch, the update and the dt candidate; 8-byte shared-memory traffic:
+# Y gathers, flux writes, flux gathers, ~5 words per species.
+def algorithmic_work(net, n_entries):
+    n_react_total = int(net.n_react.sum())
+    flops = n_react_total + n_entries + 10 * net.n_species
+    smem_bytes = 8 * (n_react_total + net.n_reactions + n_entries + 5 * net.n_species)
+    return flops, smem_bytes
+
+
+# FP64 / shared-memory peaks: measured on this pool's B200 with
+# `python -m paper_1409_5826_b200.peaks` (profiles/r01_peaks.md); fallback =
+# unit counts x clocks.max.sm from the guides (64 FP64 lanes and 128 B of shared
+# memory per clock per SM, 148 SMs, 1965 MHz).
+NOMINAL_FP64_TINSTR = 148 * 64 * 1.965e9 / 1e12
+NOMINAL_SMEM_TBS = 148 * 128 * 1.965e9 / 1e12
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "profiles", "peaks.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            p = json.load(fh)
+        return p["fp64_add_tinstr_s"], p["smem_lds64_tb_s"], "measured (profiles/peaks.json)"
+    return NOMINAL_FP64_TINSTR, NOMINAL_SMEM_TBS, "nominal (148 SM x 64 lanes | 128 B x 1965 MHz)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU):
+    """Weak scaling: the global batch is world x 16384 zones of one seeded profile;
+    rank r integrates the contiguous shard r (no data-path collective)."""
+    from gen import perturbed_co_start, zone_profile
+    from gen.configs import network
+    from paper_1409_5826_b200.shard import zone_shard
+
+    net = network("hub150")
+    total = zones_per_gpu * world
+    lo, hi = zone_shard(total, rank, world)
+    T9, rho = zone_profile(total, PROFILE_SEED)
+    Y0 = perturbed_co_start(net, total, seed=1000 + PROFILE_SEED)
+    return net, T9[lo:hi].copy(), rho[lo:hi].copy(), Y0[lo:hi].copy()
+
+
+def cpu_baseline(net, T9, rho, Y0, zones_per_core=96, reps=1):
+    """The oracle as it stands on the host cores, on a bounded prefix sample."""
+    from oracle import Oracle, max_threads
+
+    cores = max_threads()
+    n = int(min(len(T9), zones_per_core * cores))
+    o = Oracle(net)
+    best, steps = None, 0
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        out = o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+        steps = int(out["n_steps"].sum())
+    return {"value": n / best, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n} of {len(T9)} zones of the same workload, {steps} sub-steps, "
+                      f"{best:.2f} s, gcc -O2 -ffp-contract=off, OpenMP dynamic over zones",
+            "zone_substeps_per_s": steps / best}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    net, T9, rho, Y0 = workload(0, 1)
+    from oracle import Oracle, max_threads
+
+    cores = max_threads()
+    n = int(min(len(T9), 48 * cores))
+    o = Oracle(net)
+    for _ in range(args.warmup):
+        o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        out = o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
+    el = time.perf_counter() - t0
+    value = n * args.steps / el
+    sample = (f"each step = first {n} of {ZONES_PER_GPU} zones, {int(out['n_steps'].sum())} sub-steps; "
+              "gcc -O2 -ffp-contract=off, OpenMP dynamic over zones")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "configs[3]: hub150 (150sp/1604rx), one hydro step 1e-6 s; CPU oracle on a bounded sample",
+                   "zones_per_step": n},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import torch
+
+    import paper_1409_5826_b200 as K
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world}"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    net, T9h, rhoh, Y0h = workload(rank, world, args.zones)
+    z, N = Y0h.shape
+    kn = K.Net(net)
+    info = kn.schedule_info()
+    T9, rho = torch.from_numpy(T9h).to(dev), torch.from_numpy(rhoh).to(dev)
+    Y0 = torch.from_numpy(Y0h).to(dev)
+    Y = torch.empty_like(Y0)
+    dt = torch.zeros(z, dtype=torch.float64, device=dev)
+    n_steps = torch.zeros(z, dtype=torch.int32, device=dev)
+    status = torch.zeros(z, dtype=torch.int32, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step(timed_events=None):
+        Y.copy_(Y0)       # restore the start state outside the timed launch
+        dt.zero_()
+        flush.zero_()     # L2 flush between timed iterations
+        if timed_events is not None:
+            timed_events[0].record(stream)
+        kn.net_integrate(z, T9, rho, Y, T_HYDRO, dt, n_steps, status, stream)
+        if timed_events is not None:
+            timed_events[1].record(stream)
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+              for _ in range(args.steps)]
+    barrier()
+    t0 = time.perf_counter()
+    for ev in events:
+        one_step(ev)
+    barrier()
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop() if rank == 0 else None
+    kernel_ms = [a.elapsed_time(b) for a, b in events]
+    total_ms = float(sum(kernel_ms))
+    substeps = int(n_steps.sum().item())
+    assert int(status.max().item()) == 0, "a zone reported a status bit"
+
+    # ---- e2e: same call through the host-buffer entry point, copies inside --
+    Yp = torch.from_numpy(Y0h.copy()).pin_memory()
+    Ysrc = torch.from_numpy(Y0h.copy())
+    T9p, rhop = torch.from_numpy(T9h.copy()).pin_memory(), torch.from_numpy(rhoh.copy()).pin_memory()
+    dtp = torch.zeros(z, dtype=torch.float64).pin_memory()
+    stp = torch.zeros(z, dtype=torch.int32).pin_memory()
+    sts = torch.zeros(z, dtype=torch.int32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_s = 0.0
+    for it in range(1 + e2e_steps):
+        Yp.copy_(Ysrc)
+        dtp.zero_()
+        barrier()
+        t1 = time.perf_counter()
+        kn.net_integrate_host(z, T9p.numpy(), rhop.numpy(), Yp.numpy(), T_HYDRO, dtp.numpy(),
+                              stp.numpy(), sts.numpy())
+        if it > 0:
+            e2e_s += time.perf_counter() - t1
+    h2d = z * (N * 8 + 8 + 8 + 8)
+    d2h = z * (N * 8 + 8 + 4 + 4)
+
+    # ---- max over ranks ---------------------------------------------------
+    tm = torch.tensor([total_ms, e2e_s, float(substeps)], dtype=torch.float64, device=dev)
+    if world > 1:
+        mx = tm.clone()
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = tm.clone()
+        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        total_ms, e2e_s, substeps_all = float(mx[0]), float(mx[1]), float(sm[2])
+    else:
+        substeps_all = float(substeps)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = total_ms / args.steps
+    value = z * world / (ms_per_step * 1e-3)
+    e2e_value = z * world / (e2e_s / e2e_steps)
+    flops, smem_b = algorithmic_work(net, info["n_entries"])
+    fp64_peak, smem_peak, peak_src = load_peaks()
+    per_launch_substeps = substeps  # rank 0's launch
+    k_ms = float(np.mean(kernel_ms))
+    fp64_ach = flops * per_launch_substeps / (k_ms * 1e-3) / 1e12
+    smem_ach = smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12
+    traffic_path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    traffic = None
+    if os.path.exists(traffic_path):
+        with open(traffic_path) as fh:
+            traffic = json.load(fh).get("dram_bytes_per_launch")
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {
+            "workload": "configs[3]: synthetic 150sp/1604rx hub network (seed 1409), 16384 zones per GPU, "
+                        "T9~U[1,10], log10 rho~U[7,9.5] (seed 4), lognormal-perturbed C/O start, "
+                        "one hydro step of 1e-6 s, adaptive dt",
+            "zones_per_gpu": z, "sub_steps_per_step": substeps_all,
+            "mean_sub_steps_per_zone": substeps_all / (z * world),
+            "l2": "256 MB buffer written between timed iterations (L2 flush)",
+            "parallelism": f"zones sharded contiguously over {world} GPU(s), no collective",
+            "threads_per_zone": info["threads"], "zones_per_sm": info["zones_per_sm"],
+        },
+        "zone_substeps_per_s": substeps_all / (ms_per_step * 1e-3),
+        "wall_s_timed_region": wall,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "api": "net_integrate_host (pinned host buffers)"},
+        "gpu_launches": args.steps,
+        "roofline": {
+            "bound": "alu", "kernel": "zone_kernel<double, adaptive>", "achieved": fp64_ach,
+            "peak": fp64_peak, "unit": "TFLOP/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
+            "what": f"{flops} algorithmic FP64 ops per zone-substep x {per_launch_substeps} zone-substeps "
+                    f"per launch / {k_ms:.2f} ms; peak = FP64 non-FMA issue rate, {peak_src}",
+        },
+        "roofline_smem": {
+            "bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "TB/s",
+            "frac": smem_ach / smem_peak,
+            "what": f"{smem_b} algorithmic shared-memory bytes per zone-substep; peak {peak_src}",
+        },
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(net, T9h, rhoh, Y0h)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--zones", type=int, default=ZONES_PER_GPU,
+                    help="zones per GPU (profiling only; the metric is quoted at the default)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -63,7 +63,8 @@ typedef struct {
     double growth;       /* dt control: dt may grow by at most this factor per step (2)   */
     long long max_steps; /* per call and zone (1e7)                                       */
     int precision;       /* 64 (default) or 32                                            */
-    int reserved;
+    int kernel;          /* 0 = automatic: register-resident kernel when the network fits its
+                            capacities; 1 = always the table-driven kernel (A/B and fallback) */
 } net_params_t;
 
 /* Fill *p with the defaults listed above. */

@@ -31,7 +31,7 @@ class net_params_t(C.Structure):
     _fields_ = [
         ("kappa", C.c_double), ("eps_y", C.c_double), ("y_floor", C.c_double),
         ("growth", C.c_double), ("max_steps", C.c_longlong), ("precision", C.c_int),
-        ("reserved", C.c_int),
+        ("kernel", C.c_int),
     ]
 
 
@@ -93,16 +93,17 @@ class NetParams:
     growth: float = 2.0
     max_steps: int = 10_000_000
     precision: int = 64
+    kernel: int = 0  # 0 = automatic, 1 = table-driven kernel only
 
     def to_c(self) -> net_params_t:
         return net_params_t(self.kappa, self.eps_y, self.y_floor, self.growth, self.max_steps,
-                            self.precision, 0)
+                            self.precision, self.kernel)
 
 
 def net_default_params() -> NetParams:
     p = net_params_t()
     _check(lib.net_default_params(C.byref(p)))
-    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision)
+    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel)
 
 
 def _ptr(t):

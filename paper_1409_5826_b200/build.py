@@ -25,6 +25,20 @@ def nvcc() -> str:
     return exe
 
 
+PEAKS_SRC = os.path.join(CSRC, "peaks.cu")
+PEAKS_BIN = os.path.join(HERE, "kinnet_peaks")
+
+
+def build_peaks(force: bool = False) -> str:
+    """Micro-benchmark binary for the FP64 / shared-memory roofline denominators."""
+    if force or not os.path.exists(PEAKS_BIN) or os.path.getmtime(PEAKS_BIN) < os.path.getmtime(PEAKS_SRC):
+        tmp = PEAKS_BIN + f".tmp{os.getpid()}"
+        subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo",
+                               "-std=c++17", "-cudart", "static", PEAKS_SRC, "-o", tmp])
+        os.replace(tmp, PEAKS_BIN)
+    return PEAKS_BIN
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     deps = SOURCES + HEADERS + [__file__]
     newest = max(os.path.getmtime(p) for p in deps)
@@ -40,3 +54,4 @@ if __name__ == "__main__":
     import sys
 
     print(build(force=True, verbose="-v" in sys.argv))
+    print(build_peaks(force=True))

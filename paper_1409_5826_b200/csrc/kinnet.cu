@@ -63,6 +63,14 @@ struct KParams {
     const uint16_t* small_src;
     const uint8_t* big_cnt;
     const uint8_t* big_slot;
+    // packed tables of the register-resident kernel
+    const uint32_t* fx_pack;
+    const uint32_t* fxc_pack;
+    const uint32_t* plus_pack;
+    const uint32_t* minus_pack;
+    const uint32_t* rb_pack;
+    const uint32_t* cnt_pack;
+    const uint32_t* rbcnt_pack;
     // zones
     const double* T9;
     const double* rho;
@@ -309,6 +317,352 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
     }
 }
 
+// ---------------------------------------------------------------------------
+// Register-resident variant (the one bench.py times when the network fits the
+// kFast* capacities): same schedule, same three barriers, but
+//   * rates and every index table of a thread live in registers for the whole
+//     hydro step (topology is static, sub-steps number 1e2..1e4), loops are
+//     fully unrolled, so the sub-step issues no global loads and no address math;
+//   * the six big-row partial sums are combined by ONE transposed butterfly
+//     (9 shuffle rounds instead of 30);
+//   * one reciprocal per dt candidate and one per asymptotic update (MUFU seed
+//     + Newton) replace three IEEE divisions.
+// ---------------------------------------------------------------------------
+constexpr int kRS = kinnet::kFastSlots;
+constexpr int kPC = kinnet::kFastPlus;
+constexpr int kMC = kinnet::kFastMinus;
+
+__device__ __forceinline__ double rcp_pos(double b) {  // b normal, positive
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+    double e = fma(-b, r, 1.0);
+    e = fma(e, e, e);
+    r = fma(r, e, r);
+    e = fma(-b, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+__device__ __forceinline__ float rcp_pos(float b) { return __frcp_rn(b); }
+
+template <typename real> struct Tiny;
+template <> struct Tiny<double> { static __device__ __forceinline__ double v() { return 1e-290; } };
+template <> struct Tiny<float> { static __device__ __forceinline__ float v() { return 1e-30f; } };
+
+// Sum rows 0..7 of acc over the warp; on return lane l holds, in the returned
+// value, the warp total of row (l >> 2) & 7.  Fixed order: deterministic.
+template <typename real>
+__device__ __forceinline__ real warp_sum_rows8(const real (&acc)[8], int lane) {
+    real a[4], b[2], c;
+    const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const real send = up16 ? acc[i] : acc[i + 4];
+        const real keep = up16 ? acc[i + 4] : acc[i];
+        a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const real send = up8 ? a[i] : a[i + 2];
+        const real keep = up8 ? a[i + 2] : a[i];
+        b[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    {
+        const real send = up4 ? b[0] : b[1];
+        const real keep = up4 ? b[1] : b[0];
+        c = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    c += __shfl_xor_sync(0xffffffffu, c, 2);
+    c += __shfl_xor_sync(0xffffffffu, c, 1);
+    return c;
+}
+
+template <typename real>
+size_t smem_bytes_reg(const Schedule& S) {
+    return 64 * sizeof(double) +
+           sizeof(real) * (static_cast<size_t>(real_words_before_flux(S.N)) +
+                           static_cast<size_t>(S.rs + 1) * S.T +
+                           static_cast<size_t>(S.W) * kRedStride);
+}
+
+// Field extraction from the packed tables.  volatile: the tables are loop
+// invariant, and without it the compiler hoists every unpacked field out of the
+// sub-step loop into its own register (and then spills).
+__device__ __forceinline__ uint32_t lo16(uint32_t x) {
+    uint32_t r;
+    asm volatile("and.b32 %0, %1, 0xffff;" : "=r"(r) : "r"(x));
+    return r;
+}
+__device__ __forceinline__ uint32_t hi16(uint32_t x) {
+    uint32_t r;
+    asm volatile("shr.u32 %0, %1, 16;" : "=r"(r) : "r"(x));
+    return r;
+}
+__device__ __forceinline__ uint32_t nib(uint32_t x, int q) {
+    uint32_t r;
+    asm volatile("bfe.u32 %0, %1, %2, 4;" : "=r"(r) : "r"(x), "r"(4 * q));
+    return r;
+}
+
+template <typename real>
+__device__ __forceinline__ real lds_at(const unsigned char* base, uint32_t byte_off) {
+    return *reinterpret_cast<const real*>(base + byte_off);
+}
+
+template <typename real, int MODE, int TB, int MINB>
+__global__ void __launch_bounds__(TB, MINB) zone_kernel_reg(const KParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int T = p.T, N = p.N, W = p.W, rs = p.rs, nbs = p.nbs;
+    const int j2 = p.j2, j3 = p.j3;
+    const int z = blockIdx.x;
+
+    double* redmin = reinterpret_cast<double*>(smem_raw);
+    double* ybig = redmin + 32;
+    real* Ybuf = reinterpret_cast<real*>(redmin + 64);
+    real* fbuf = Ybuf + real_words_before_flux(N);  // [rs + 1][T]; row rs stays zero
+    real* red = fbuf + (rs + 1) * T;
+    real* fcol = fbuf + tid;  // this thread's bank-aligned flux column
+    const unsigned char* Yb = reinterpret_cast<const unsigned char*>(Ybuf);
+    const unsigned char* fb = reinterpret_cast<const unsigned char*>(fbuf);
+    const uint32_t col_stride = static_cast<uint32_t>(T) * sizeof(real);
+
+    // ---- tables -> registers -------------------------------------------------
+    uint32_t fx[kRS], fxc[kinnet::kFastSlots3], pl[kPC / 2], mi[kMC / 2], rb[2 * kMaxBig];
+#pragma unroll
+    for (int j = 0; j < kRS; ++j) fx[j] = (j < rs) ? p.fx_pack[j * T + tid] : 0u;
+#pragma unroll
+    for (int j = 0; j < kinnet::kFastSlots3; ++j) fxc[j] = (j < rs) ? p.fxc_pack[j * T + tid] : 0u;
+#pragma unroll
+    for (int e = 0; e < kPC / 2; ++e) pl[e] = p.plus_pack[e * T + tid];
+#pragma unroll
+    for (int e = 0; e < kMC / 2; ++e) mi[e] = p.minus_pack[e * T + tid];
+#pragma unroll
+    for (int b = 0; b < 2 * kMaxBig; ++b) rb[b] = p.rb_pack[b * T + tid];
+    // warp-wide trip counts (threads of a warp own rows of similar length)
+    int wnp, wnm;
+    uint32_t wrb = 0;
+    {
+        const uint32_t cnt = p.cnt_pack[tid], rbcnt = p.rbcnt_pack[tid];
+        wnp = __reduce_max_sync(0xffffffffu, cnt & 255u);
+        wnm = __reduce_max_sync(0xffffffffu, (cnt >> 8) & 255u);
+#pragma unroll
+        for (int b = 0; b < 2 * kMaxBig; ++b)
+            wrb |= __reduce_max_sync(0xffffffffu, (rbcnt >> (4 * b)) & 15u) << (4 * b);
+    }
+
+    // ---- S1: rates, once per zone per call, kept in registers ------------------
+    real R[kRS];
+    {
+        const int slots = rs * T;
+        const double T9 = p.T9[z], rho = p.rho[z];
+        const double t13 = cbrt(T9);
+        const double t53 = T9 * t13 * t13;
+        const double lnT = log(T9), lnrho = log(rho);
+#pragma unroll
+        for (int j = 0; j < kRS; ++j) {
+            R[j] = 0;
+            if (j < rs) {
+                const double* c = p.coef + (j * T + tid);
+                const double lnR = c[0] + c[1 * (size_t)slots] / T9 + c[2 * (size_t)slots] / t13 +
+                                   c[3 * (size_t)slots] * t13 + c[4 * (size_t)slots] * T9 +
+                                   c[5 * (size_t)slots] * t53 + c[6 * (size_t)slots] * lnT;
+                R[j] = static_cast<real>(exp(c[7 * (size_t)slots] * lnrho + lnR));
+            }
+        }
+    }
+
+    // ---- S6: zone state in ------------------------------------------------------
+    real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
+    for (int i = tid; i < N; i += T) Ybuf[i] = Yg[i];
+    if (tid == 0) Ybuf[N] = static_cast<real>(1);
+    fcol[rs * T] = static_cast<real>(0);
+    const int own = p.owner[tid];
+    const bool is_big = (tid >= W && tid < W + nbs);
+    __syncthreads();
+    real y = (own >= 0) ? Ybuf[own] : static_cast<real>(0);
+
+    const real kappa = static_cast<real>(p.kappa);
+    const real eps_y = static_cast<real>(p.eps_y);
+    const real y_floor = static_cast<real>(p.y_floor);
+    const double growth = p.growth, t_hydro = p.t_hydro;
+
+    double t = 0.0, dt_prev = 0.0;
+    int steps = 0;
+    int status = 0;
+    bool run = true;
+    if (MODE == kAdaptive) {
+        const double dt_in = p.dt ? p.dt[z] : 0.0;
+        dt_prev = (dt_in > 0.0) ? dt_in : t_hydro;
+        run = t_hydro > 0.0;
+        if (!run) dt_prev = dt_in;
+    } else if (MODE == kFixed) {
+        run = p.n_fixed > 0;
+    }
+    const int max_steps = static_cast<int>(MODE == kFixed ? p.n_fixed : p.max_steps);
+
+    while (run) {
+        // ---- S2: fluxes -------------------------------------------------------
+#pragma unroll
+        for (int j = 0; j < kRS; ++j) {
+            if (j < rs) {
+                real v = R[j] * lds_at<real>(Yb, lo16(fx[j]));
+                if (j < j2) v = v * lds_at<real>(Yb, hi16(fx[j]));
+                if (j < kinnet::kFastSlots3 && j < j3) v = v * lds_at<real>(Yb, fxc[j]);
+                fcol[j * T] = v;
+            }
+        }
+        __syncthreads();
+
+        // ---- S3: sums (zero-padded lists: no per-lane predicates) ------------------
+        real Fp = 0, Fm = 0;
+        {
+            real Fp1 = 0, Fm1 = 0;
+#pragma unroll
+            for (int g = 0; g < kPC / 4; ++g) {
+                if (4 * g < wnp) {
+                    const uint32_t w0 = pl[2 * g], w1 = pl[2 * g + 1];
+                    Fp += lds_at<real>(fb, lo16(w0));
+                    Fp1 += lds_at<real>(fb, hi16(w0));
+                    Fp += lds_at<real>(fb, lo16(w1));
+                    Fp1 += lds_at<real>(fb, hi16(w1));
+                }
+            }
+#pragma unroll
+            for (int g = 0; g < kMC / 4; ++g) {
+                if (4 * g < wnm) {
+                    const uint32_t w0 = mi[2 * g], w1 = mi[2 * g + 1];
+                    Fm += lds_at<real>(fb, lo16(w0));
+                    Fm1 += lds_at<real>(fb, hi16(w0));
+                    Fm += lds_at<real>(fb, lo16(w1));
+                    Fm1 += lds_at<real>(fb, hi16(w1));
+                }
+            }
+            Fp += Fp1;
+            Fm += Fm1;
+        }
+        if (nbs > 0) {
+            real acc[8];
+            const unsigned char* fc = reinterpret_cast<const unsigned char*>(fcol);
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                acc[b] = 0;
+                if (b < 2 * kMaxBig) {
+                    const int wmax = (wrb >> (4 * b)) & 15u;
+#pragma unroll
+                    for (int q = 0; q < kinnet::kFastRowCap; q += 2) {
+                        if (q < wmax) {
+                            const uint32_t s0 = nib(rb[b], q);
+                            const uint32_t s1 = nib(rb[b], q + 1);
+                            acc[b] += lds_at<real>(fc, s0 * col_stride);
+                            acc[b] += lds_at<real>(fc, s1 * col_stride);
+                        }
+                    }
+                }
+            }
+            const real tot = warp_sum_rows8(acc, lane);
+            if ((lane & 3) == 0) red[warp * kRedStride + (lane >> 2)] = tot;
+        }
+        // ---- S5: dt candidates of the small species ---------------------------------
+        if (MODE == kAdaptive) {
+            double c = INFINITY;
+            if (own >= 0 && !is_big) {
+                real a = Fp - Fm;
+                a = a < 0 ? -a : a;
+                if (a > Tiny<real>::v())
+                    c = static_cast<double>(eps_y * (y > y_floor ? y : y_floor) * rcp_pos(a));
+            }
+            c = warp_min_pos(c);
+            if (lane == 0) redmin[warp] = c;
+            if (is_big) ybig[tid - W] = static_cast<double>(y);
+        }
+        __syncthreads();
+
+        // ---- finalize: big species sums, zone-wide dt ---------------------------------
+        real bFp = 0, bFm = 0;
+        double cand = INFINITY;
+        if (lane >= W && lane < W + nbs) {
+            const int s = lane - W;
+            for (int w = 0; w < W; ++w) {
+                bFp += red[w * kRedStride + 2 * s];
+                bFm += red[w * kRedStride + 2 * s + 1];
+            }
+            if (MODE == kAdaptive) {
+                const real yb = static_cast<real>(ybig[s]);
+                real a = bFp - bFm;
+                a = a < 0 ? -a : a;
+                if (a > Tiny<real>::v())
+                    cand = static_cast<double>(eps_y * (yb > y_floor ? yb : y_floor) * rcp_pos(a));
+            }
+        } else if (MODE == kAdaptive && lane < W) {
+            cand = redmin[lane];
+        }
+        if (is_big) {
+            Fp = bFp;
+            Fm = bFm;
+        }
+        if (MODE == kRhs) {
+            if (own >= 0) {
+                reinterpret_cast<real*>(p.Fplus)[(size_t)z * N + own] = Fp;
+                reinterpret_cast<real*>(p.Fminus)[(size_t)z * N + own] = Fm;
+            }
+            return;
+        }
+
+        double dts;
+        bool last;
+        if (MODE == kAdaptive) {
+            const double cmin = warp_min_pos(cand);
+            double dt_ctrl = growth * dt_prev;
+            if (cmin < dt_ctrl) dt_ctrl = cmin;
+            const double rem = t_hydro - t;
+            if (dt_ctrl >= rem * (1.0 - 1e-12)) {
+                dts = rem;
+                last = true;
+            } else {
+                dts = dt_ctrl;
+                last = false;
+            }
+            dt_prev = dt_ctrl;
+        } else {
+            dts = p.dt_fixed;
+            last = (steps + 1 >= max_steps);
+        }
+
+        // ---- S4: update -------------------------------------------------------------------
+        if (own >= 0) {
+            const real h = static_cast<real>(dts);
+            const real hFm = h * Fm;
+            if (y > 0 && hFm >= kappa * y) {  // k dt >= kappa with k = F-/Y
+                const real den = y + hFm;      // Eq. (3) as Y (Y + dt F+) / (Y + dt F-)
+                if (den > Tiny<real>::v() && y > Tiny<real>::v())
+                    y = (y + h * Fp) * (y * rcp_pos(den));
+                else
+                    y = (y + h * Fp) / (static_cast<real>(1) + (Fm / y) * h);
+            } else {
+                y = y + h * (Fp - Fm);
+            }
+            Ybuf[own] = y;
+        }
+        t = last ? t_hydro : t + dts;
+        ++steps;
+        if (last) run = false;
+        else if (MODE == kAdaptive && steps >= max_steps) {
+            status |= NET_STATUS_MAX_STEPS;
+            run = false;
+        }
+        __syncthreads();
+    }
+
+    const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
+    if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    for (int i = tid; i < N; i += T) Yg[i] = Ybuf[i];
+    if (tid == 0) {
+        if (MODE == kAdaptive && p.dt) p.dt[z] = dt_prev;
+        if (p.n_steps) p.n_steps[z] = steps;
+        if (p.status) p.status[z] = status;
+    }
+}
+
 struct DeviceTables {
     int32_t* flux_rxn = nullptr;
     ushort4* flux_react = nullptr;
@@ -319,6 +673,13 @@ struct DeviceTables {
     uint16_t* small_src = nullptr;
     uint8_t* big_cnt = nullptr;
     uint8_t* big_slot = nullptr;
+    uint32_t* fx_pack = nullptr;
+    uint32_t* fxc_pack = nullptr;
+    uint32_t* plus_pack = nullptr;
+    uint32_t* minus_pack = nullptr;
+    uint32_t* rb_pack = nullptr;
+    uint32_t* cnt_pack = nullptr;
+    uint32_t* rbcnt_pack = nullptr;
 };
 
 }  // namespace
@@ -327,6 +688,7 @@ struct net {
     Schedule S;
     net_params_t P;
     bool has_device = false;
+    bool force_generic = false;  // params.kernel == 1: keep the table-driven kernel (A/B tests)
     int device = -1;
     int zones_per_sm = 0;
     DeviceTables D;
@@ -356,13 +718,35 @@ kernel_fn pick_block(int T) {
     return zone_kernel<real, MODE, 1024>;
 }
 
+// register-resident kernel: block-size classes with the residency the register
+// file allows (65536 / (TB * MINB) registers per thread)
+template <typename real, int MODE>
+kernel_fn pick_block_reg(int T) {
+    if (T <= 64) return zone_kernel_reg<real, MODE, 64, 8>;
+    if (T <= 160) return zone_kernel_reg<real, MODE, 160, 3>;
+    if (T <= 256) return zone_kernel_reg<real, MODE, 256, 2>;
+    if (T <= 512) return zone_kernel_reg<real, MODE, 512, 1>;
+    return nullptr;
+}
+
+bool use_reg_kernel(const net* n);
+
 template <int MODE>
 kernel_fn pick_kernel(const net* n) {
-    if (MODE == kRates) return pick_block<double, MODE>(n->S.T);
+    if constexpr (MODE == kRates) return pick_block<double, MODE>(n->S.T);
+    else if (use_reg_kernel(n)) {
+        kernel_fn f = n->P.precision == 32 ? pick_block_reg<float, MODE>(n->S.T)
+                                           : pick_block_reg<double, MODE>(n->S.T);
+        if (f) return f;
+    }
     return n->P.precision == 32 ? pick_block<float, MODE>(n->S.T) : pick_block<double, MODE>(n->S.T);
 }
 
+bool use_reg_kernel(const net* n) { return n->S.fast_ok && !n->force_generic; }
+
 size_t net_smem(const net* n) {
+    if (use_reg_kernel(n))
+        return n->P.precision == 32 ? smem_bytes_reg<float>(n->S) : smem_bytes_reg<double>(n->S);
     return n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
 }
 
@@ -398,6 +782,13 @@ void fill_params(const net* n, KParams& k) {
     k.small_src = n->D.small_src;
     k.big_cnt = n->D.big_cnt;
     k.big_slot = n->D.big_slot;
+    k.fx_pack = n->D.fx_pack;
+    k.fxc_pack = n->D.fxc_pack;
+    k.plus_pack = n->D.plus_pack;
+    k.minus_pack = n->D.minus_pack;
+    k.rb_pack = n->D.rb_pack;
+    k.cnt_pack = n->D.cnt_pack;
+    k.rbcnt_pack = n->D.rbcnt_pack;
     k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
     k.growth = n->P.growth; k.max_steps = n->P.max_steps;
 }
@@ -425,6 +816,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
     if (!n) return fail(NET_ENOMEM, "out of host memory");
     if (params) n->P = *params; else net_default_params(&n->P);
     if (n->P.precision == 0) n->P.precision = 64;
+    n->force_generic = (n->P.kernel == 1);
     if (n->P.precision != 64 && n->P.precision != 32) {
         delete n;
         return fail(NET_EINVAL, "precision must be 64 or 32");
@@ -446,6 +838,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         delete n;
         return fail(rc, err);
     }
+    if (n->S.fast_ok) kinnet::pack_fast_tables(n->S, n->P.precision == 32 ? 4 : 8);
     if (net_smem(n) > 227 * 1024) {
         delete n;
         return fail(NET_EINVAL, "network too large for one CTA's shared memory");
@@ -464,6 +857,15 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         if (rc == NET_OK) rc = upload(&n->D.small_src, S.small_src.data(), S.small_src.size());
         if (rc == NET_OK) rc = upload(&n->D.big_cnt, S.big_cnt.data(), S.big_cnt.size());
         if (rc == NET_OK) rc = upload(&n->D.big_slot, S.big_slot.data(), S.big_slot.size());
+        if (rc == NET_OK && S.fast_ok) {
+            rc = upload(&n->D.fx_pack, S.fx_pack.data(), S.fx_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.fxc_pack, S.fxc_pack.data(), S.fxc_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.plus_pack, S.plus_pack.data(), S.plus_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.minus_pack, S.minus_pack.data(), S.minus_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.rb_pack, S.rb_pack.data(), S.rb_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.cnt_pack, S.cnt_pack.data(), S.cnt_pack.size());
+            if (rc == NET_OK) rc = upload(&n->D.rbcnt_pack, S.rbcnt_pack.data(), S.rbcnt_pack.size());
+        }
         if (rc == NET_OK) {
             n->has_device = true;
             rc = prepare_kernels(n);
@@ -491,7 +893,7 @@ int net_default_params(net_params_t* p) {
     p->growth = 2.0;
     p->max_steps = 10000000LL;
     p->precision = 64;
-    p->reserved = 0;
+    p->kernel = 0;
     return NET_OK;
 }
 
@@ -515,6 +917,8 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.flux_rxn); cudaFree(n->D.flux_react); cudaFree(n->D.coef);
         cudaFree(n->D.owner); cudaFree(n->D.small_plus); cudaFree(n->D.small_minus);
         cudaFree(n->D.small_src); cudaFree(n->D.big_cnt); cudaFree(n->D.big_slot);
+        cudaFree(n->D.fx_pack); cudaFree(n->D.fxc_pack); cudaFree(n->D.plus_pack); cudaFree(n->D.minus_pack);
+        cudaFree(n->D.rb_pack); cudaFree(n->D.cnt_pack); cudaFree(n->D.rbcnt_pack);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
         cudaFree(n->ssteps); cudaFree(n->sstatus);
         if (n->host_stream) cudaStreamDestroy(n->host_stream);
@@ -538,7 +942,7 @@ int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho
                         double dt_fixed, long long n_steps, void* stream) {
     if (!n) return fail(NET_EINVAL, "null net");
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
-    if (n_steps < 0) return fail(NET_EINVAL, "n_steps < 0");
+    if (n_steps < 0 || n_steps > 2000000000LL) return fail(NET_EINVAL, "n_steps out of range [0, 2e9]");
     KParams k;
     fill_params(n, k);
     k.T9 = T9; k.rho = rho; k.Y = Y;

@@ -266,7 +266,63 @@ int build_schedule(int N, const int* A, int M, const int* n_react, const int* re
         for (int b = 0; b < 2 * S.nbs; ++b)
             for (uint8_t v : rb[t][b]) S.big_slot[static_cast<size_t>(e++) * T + t] = v;
     }
+
+    // ---- packed tables for the register-resident kernel ---------------------
+    S.plus_max = *std::max_element(S.small_plus.begin(), S.small_plus.end());
+    S.minus_max = *std::max_element(S.small_minus.begin(), S.small_minus.end());
+    S.bigrow_max = 0;
+    for (uint8_t c : S.big_cnt) S.bigrow_max = std::max<int>(S.bigrow_max, c);
+    S.fast_ok = N <= 1023 && S.rs <= kFastSlots && S.rs <= 15 && S.j3 <= kFastSlots3 &&
+                S.plus_max <= kFastPlus && S.minus_max <= kFastMinus &&
+                S.bigrow_max <= kFastRowCap && (S.rs + 1) * T * 8 <= 65535;
     return NET_OK;
+}
+
+// Packed tables of the register-resident kernel.  Offsets are BYTE offsets for
+// elements of `elem` bytes (8: double, 4: float).  Gather lists are padded to
+// their capacity with the offset of the thread's own word in the all-zero flux
+// row `rs`, readback lists with the slot id `rs`, so the kernel needs no
+// per-lane predicates.
+void pack_fast_tables(Schedule& S, int elem) {
+    const int T = S.T, slots = S.rs * T;
+    const uint32_t e32 = static_cast<uint32_t>(elem);
+    S.fx_pack.assign(static_cast<size_t>(S.rs) * T, 0);
+    S.fxc_pack.assign(static_cast<size_t>(kFastSlots3) * T, 0);
+    for (int idx = 0; idx < slots; ++idx) {
+        const uint16_t* re = &S.flux_react[static_cast<size_t>(idx) * 4];
+        S.fx_pack[idx] = re[0] * e32 | (re[1] * e32) << 16;
+        if (idx / T < kFastSlots3) S.fxc_pack[idx] = re[2] * e32;
+    }
+    S.plus_pack.assign(static_cast<size_t>(kFastPlus / 2) * T, 0);
+    S.minus_pack.assign(static_cast<size_t>(kFastMinus / 2) * T, 0);
+    S.rb_pack.assign(static_cast<size_t>(2 * kMaxBigSpecies) * T, 0);
+    S.cnt_pack.assign(T, 0);
+    S.rbcnt_pack.assign(T, 0);
+    for (int t = 0; t < T; ++t) {
+        const uint32_t zero_off = static_cast<uint32_t>(S.rs * T + t) * e32;
+        const int np = S.small_plus[t], nm = S.small_minus[t];
+        for (int e = 0; e < kFastPlus; ++e) {
+            const uint32_t off = e < np ? S.small_src[static_cast<size_t>(e) * T + t] * e32 : zero_off;
+            S.plus_pack[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
+        }
+        for (int e = 0; e < kFastMinus; ++e) {
+            const uint32_t off =
+                e < nm ? S.small_src[static_cast<size_t>(np + e) * T + t] * e32 : zero_off;
+            S.minus_pack[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
+        }
+        S.cnt_pack[t] = static_cast<uint32_t>(np) | static_cast<uint32_t>(nm) << 8;
+        int e = 0;
+        for (int b = 0; b < 2 * kMaxBigSpecies; ++b) {
+            const int c = b < 2 * S.nbs ? S.big_cnt[static_cast<size_t>(b) * T + t] : 0;
+            for (int q = 0; q < kFastRowCap; ++q) {
+                const uint32_t sid = q < c ? S.big_slot[static_cast<size_t>(e + q) * T + t]
+                                           : static_cast<uint32_t>(S.rs);
+                S.rb_pack[static_cast<size_t>(b) * T + t] |= sid << (4 * q);
+            }
+            e += c;
+            S.rbcnt_pack[t] |= static_cast<uint32_t>(c) << (4 * b);
+        }
+    }
 }
 
 }  // namespace kinnet

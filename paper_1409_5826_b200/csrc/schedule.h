@@ -52,7 +52,27 @@ struct Schedule {
     std::vector<uint8_t> big_cnt;      // [2*nbs][T] readback entries for row 2*s (+) / 2*s+1 (-)
     int readback_max = 0;
     std::vector<uint8_t> big_slot;     // [readback_max*T] own flux slot of readback entry e
+
+    // ---- packed copies for the register-resident kernel -------------------
+    // fast_ok when the network fits its compile-time capacities (kFast*).
+    bool fast_ok = false;
+    int plus_max = 0, minus_max = 0, bigrow_max = 0;
+    std::vector<uint32_t> fx_pack;     // [rs][T]   byte offsets of Y[a] | Y[b] << 16
+    std::vector<uint32_t> fxc_pack;    // [kFastSlots3][T] byte offset of Y[c] for slot rows < j3
+    std::vector<uint32_t> plus_pack;   // [kFastPlus/2][T]  two 16-bit flux byte offsets per word
+    std::vector<uint32_t> minus_pack;  // [kFastMinus/2][T]
+    std::vector<uint32_t> rb_pack;     // [2*kMaxBigSpecies][T] eight 4-bit own-slot ids per row
+    std::vector<uint32_t> cnt_pack;    // [T] plus | minus << 8
+    std::vector<uint32_t> rbcnt_pack;  // [T] eight 4-bit readback counts, one per big row
 };
+
+constexpr int kFastSlots = 12;   // flux slots per thread held in registers
+constexpr int kFastPlus = 24;    // F+ small-row entries per thread
+constexpr int kFastMinus = 24;   // F- small-row entries per thread
+constexpr int kFastRowCap = 8;   // readback entries per thread and big row
+constexpr int kFastSlots3 = 2;   // slot rows that may hold three-body reactions
+
+void pack_fast_tables(Schedule& S, int elem_bytes);
 
 // Returns 0 or a NET_E* code with a message in err.
 int build_schedule(int N, const int* A, int M, const int* n_react, const int* react,
