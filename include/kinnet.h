@@ -63,8 +63,9 @@ typedef struct {
     double growth;       /* dt control: dt may grow by at most this factor per step (2)   */
     long long max_steps; /* per call and zone (1e7)                                       */
     int precision;       /* 64 (default) or 32                                            */
-    int kernel;          /* 0 = automatic: register-resident kernel when the network fits its
-                            capacities; 1 = always the table-driven kernel (A/B and fallback) */
+    int kernel;          /* 0 = automatic: pull kernel when the network qualifies (every reaction
+                            has at most one non-hub reactant); 1 = always the
+                            generic flux-array kernel (A/B tests and fallback) */
 } net_params_t;
 
 /* Fill *p with the defaults listed above. */
@@ -149,6 +150,16 @@ typedef struct {
     int readback_max;    /* longest per-thread readback list                         */
     int smem_bytes;      /* dynamic shared memory per zone at this precision         */
     int zones_per_sm;    /* co-resident CTAs per SM (0 without a device)             */
+    /* the fields above except threads/smem_bytes/zones_per_sm describe the generic
+       flux-array schedule; the ones below the pull schedule */
+    int kernel;          /* kernel net_integrate* will launch: 1 = pull, 0 = generic  */
+    int pull_ok;         /* the network qualifies for the pull kernel                 */
+    int pull_hubs;       /* hub species tracked in registers by every thread (0..3)   */
+    int pull_slots;      /* longest per-thread list of incoming reactions (P-slots)   */
+    int pull_slots2;     /* ... of which with a second factor                         */
+    int pull_agg_max;    /* longest per-thread rate-sum list                          */
+    int pull_wavefronts;       /* predicted shared-memory wavefronts of the fp64 P-slot gathers */
+    int pull_wavefronts_ideal; /* ... without bank conflicts                          */
 } net_schedule_info_t;
 
 int net_schedule_info(const net_t *net, net_schedule_info_t *info);
@@ -165,6 +176,17 @@ int net_schedule_info(const net_t *net, net_schedule_info_t *info);
  *   "big_species" [n_big_species]
  *   "big_cnt"     [2*n_big_species*threads] readback entries of thread t for row 2*s+{0:+,1:-}
  *   "big_slot"    [readback_max*threads]   own flux slot of readback entry e of thread t
+ * Pull schedule (only when pull_ok; T = threads, word = index into the published
+ * table YP[4][T] followed by the constant one at 4*T):
+ *   "pull_hub"      [pull_hubs]            hub species; hub h is owned by thread h
+ *   "pull_owner"    [T]                    species owned by thread t, -1 = none
+ *   "pull_n_slots"  [T]   "pull_n_slots2" [T]
+ *   "pull_slot_rxn" [max(1,pull_slots)*T]  slot e of thread t: reaction | nu << 24, -1 = empty
+ *   "pull_slot_f1"  [max(1,pull_slots)*T]  word class*T + thread of its first factor
+ *   "pull_slot_f2"  [max(1,pull_slots2)*T] word of its second factor (4*T = one)
+ *   "pull_agg_ptr"  [20*T]                 rate-sum coefficient s of thread t sums entries
+ *                                          [ptr[s][t], ptr[s+1][t]) of its list
+ *   "pull_agg_ent"  [max(1,pull_agg_max)*T] reaction | nu << 24
  */
 int net_schedule_table(const net_t *net, const char *name, int *out, int cap);
 

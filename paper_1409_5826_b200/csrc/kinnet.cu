@@ -21,8 +21,10 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/kinnet.h"
 #include "schedule.h"
@@ -63,14 +65,6 @@ struct KParams {
     const uint16_t* small_src;
     const uint8_t* big_cnt;
     const uint8_t* big_slot;
-    // packed tables of the register-resident kernel
-    const uint32_t* fx_pack;
-    const uint32_t* fxc_pack;
-    const uint32_t* plus_pack;
-    const uint32_t* minus_pack;
-    const uint32_t* rb_pack;
-    const uint32_t* cnt_pack;
-    const uint32_t* rbcnt_pack;
     // zones
     const double* T9;
     const double* rho;
@@ -318,19 +312,49 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
 }
 
 // ---------------------------------------------------------------------------
-// Register-resident variant (the one bench.py times when the network fits the
-// kFast* capacities): same schedule, same three barriers, but
-//   * rates and every index table of a thread live in registers for the whole
-//     hydro step (topology is static, sub-steps number 1e2..1e4), loops are
-//     fully unrolled, so the sub-step issues no global loads and no address math;
-//   * the six big-row partial sums are combined by ONE transposed butterfly
-//     (9 shuffle rounds instead of 30);
-//   * one reciprocal per dt candidate and one per asymptotic update (MUFU seed
-//     + Newton) replace three IEEE divisions.
+// Pull kernel (the one bench.py times when the network qualifies, see
+// schedule.h "Pull schedule"): no flux array, two barriers per sub-step.
+//
+//   publish   YP[c][t] = y * {1, Y_hub0, Y_hub1, Y_hub2}[c]            4 STS
+//   rate sums k = F-/y and the six hub-row partials from the per-thread
+//             coefficients K, G0, Gx (sums of rates formed once per call)
+//   ------------------------------------------------------------------- barrier
+//   P-slots   F+ = sum_e R[e] * YP[f1[e]] (* YP[f2[e]])   fluxes at the consumer
+//   dt        candidate eps*max(y,floor)/|F+ - k y|, warp min -> redmin[warp]
+//   hub rows  transposed warp butterfly of the six partials -> red[warp][row]
+//   ------------------------------------------------------------------- barrier
+//   finalize  every warp redundantly: lanes 0..2 sum the hub rows over warps,
+//             zone-wide dt, hub update, shuffle-broadcast of the new hub Y
+//   update    k dt >= kappa ? (y + dt F+)/(1 + k dt) : y + dt (F+ - k y)
+// Rates, rate sums and every gather offset of a thread stay in registers for
+// the whole hydro step (topology is static, sub-steps number 1e2..1e4).
 // ---------------------------------------------------------------------------
-constexpr int kRS = kinnet::kFastSlots;
-constexpr int kPC = kinnet::kFastPlus;
-constexpr int kMC = kinnet::kFastMinus;
+constexpr int kJ2C = kinnet::kPullMaxSlots2;
+
+struct KPull {
+    int N, M, T, W, nbs;
+    int hub[kinnet::kPullHubs];
+    int mode;                 // Mode: kAdaptive, kFixed or kRhs
+    const double* coef;       // [8][M] reaction order: a0 + ln p, a1..a6, n_react - 1
+    const int32_t* owner;     // [T]
+    const uint32_t* cnt;      // [T] n_slots | n_slots2 << 8
+    const int32_t* slot_rxn;  // [kPullMaxSlots][T] reaction | nu << 24, -1 = empty
+    const uint32_t* f1_pack;  // [kPullMaxSlots / 2][T] two 16-bit YP byte offsets per word
+    const uint32_t* f2_pack;  // [kPullMaxSlots2 / 2][T]
+    const uint16_t* agg_ptr;  // [kPullCoefs + 1][T]
+    const int32_t* agg_ent;   // [agg_max][T]
+    const double* T9;
+    const double* rho;
+    void* Y;
+    double* dt;
+    int* n_steps;
+    int* status;
+    void* Fplus;
+    void* Fminus;
+    double t_hydro, dt_fixed;
+    double kappa, eps_y, y_floor, growth;
+    int n_fixed, max_steps;
+};
 
 __device__ __forceinline__ double rcp_pos(double b) {  // b normal, positive
     double r;
@@ -348,8 +372,8 @@ template <typename real> struct Tiny;
 template <> struct Tiny<double> { static __device__ __forceinline__ double v() { return 1e-290; } };
 template <> struct Tiny<float> { static __device__ __forceinline__ float v() { return 1e-30f; } };
 
-// Sum rows 0..7 of acc over the warp; on return lane l holds, in the returned
-// value, the warp total of row (l >> 2) & 7.  Fixed order: deterministic.
+// Sum rows 0..7 of acc over the warp; on return lane l holds the warp total of
+// row (l >> 2) & 7.  Fixed order: deterministic.
 template <typename real>
 __device__ __forceinline__ real warp_sum_rows8(const real (&acc)[8], int lane) {
     real a[4], b[2], c;
@@ -376,15 +400,7 @@ __device__ __forceinline__ real warp_sum_rows8(const real (&acc)[8], int lane) {
     return c;
 }
 
-template <typename real>
-size_t smem_bytes_reg(const Schedule& S) {
-    return 64 * sizeof(double) +
-           sizeof(real) * (static_cast<size_t>(real_words_before_flux(S.N)) +
-                           static_cast<size_t>(S.rs + 1) * S.T +
-                           static_cast<size_t>(S.W) * kRedStride);
-}
-
-// Field extraction from the packed tables.  volatile: the tables are loop
+// Field extraction from the packed offset words.  volatile: the words are loop
 // invariant, and without it the compiler hoists every unpacked field out of the
 // sub-step loop into its own register (and then spills).
 __device__ __forceinline__ uint32_t lo16(uint32_t x) {
@@ -397,89 +413,104 @@ __device__ __forceinline__ uint32_t hi16(uint32_t x) {
     asm volatile("shr.u32 %0, %1, 16;" : "=r"(r) : "r"(x));
     return r;
 }
-__device__ __forceinline__ uint32_t nib(uint32_t x, int q) {
-    uint32_t r;
-    asm volatile("bfe.u32 %0, %1, %2, 4;" : "=r"(r) : "r"(x), "r"(4 * q));
-    return r;
-}
-
 template <typename real>
 __device__ __forceinline__ real lds_at(const unsigned char* base, uint32_t byte_off) {
     return *reinterpret_cast<const real*>(base + byte_off);
 }
 
-template <typename real, int MODE, int TB, int MINB>
-__global__ void __launch_bounds__(TB, MINB) zone_kernel_reg(const KParams p) {
+template <typename real>
+__host__ __device__ inline size_t pull_smem_bytes(int T, int W, int M) {
+    return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(W) * 8 + 4 * T + 4) +
+           sizeof(double) * static_cast<size_t>(M);
+}
+
+// dt candidate of one species: eps max(y, floor) / |F+ - F-|   (reading Q7)
+template <typename real>
+__device__ __forceinline__ double dt_candidate(real y, real a, real eps_y, real y_floor) {
+    a = a < 0 ? -a : a;
+    if (a > Tiny<real>::v())
+        return static_cast<double>(eps_y * (y > y_floor ? y : y_floor) * rcp_pos(a));
+    return INFINITY;
+}
+
+template <typename real, int TB, int MINB, int CP>
+__global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
+    static_assert(CP % 4 == 0 && CP <= kinnet::kPullMaxSlots, "slot capacity");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int T = p.T, N = p.N, W = p.W, rs = p.rs, nbs = p.nbs;
-    const int j2 = p.j2, j3 = p.j3;
+    const int T = p.T, N = p.N, W = p.W, M = p.M, nbs = p.nbs;
     const int z = blockIdx.x;
+    const int mode = p.mode;
 
-    double* redmin = reinterpret_cast<double*>(smem_raw);
-    double* ybig = redmin + 32;
-    real* Ybuf = reinterpret_cast<real*>(redmin + 64);
-    real* fbuf = Ybuf + real_words_before_flux(N);  // [rs + 1][T]; row rs stays zero
-    real* red = fbuf + (rs + 1) * T;
-    real* fcol = fbuf + tid;  // this thread's bank-aligned flux column
-    const unsigned char* Yb = reinterpret_cast<const unsigned char*>(Ybuf);
-    const unsigned char* fb = reinterpret_cast<const unsigned char*>(fbuf);
-    const uint32_t col_stride = static_cast<uint32_t>(T) * sizeof(real);
+    double* redmin = reinterpret_cast<double*>(smem_raw);        // [32] per-warp dt minima
+    real* red = reinterpret_cast<real*>(redmin + 32);            // [W][8] per-warp hub-row sums
+    real* YP = red + W * 8;                                      // [4][T] published products, then 1
+    double* Rbuf = reinterpret_cast<double*>(YP + 4 * T + 4);    // [M] rates, used during set-up only
+    const unsigned char* YPb = reinterpret_cast<const unsigned char*>(YP);
 
-    // ---- tables -> registers -------------------------------------------------
-    uint32_t fx[kRS], fxc[kinnet::kFastSlots3], pl[kPC / 2], mi[kMC / 2], rb[2 * kMaxBig];
+    // ---- gather offsets -> registers -------------------------------------------
+    uint32_t f1[CP / 2], f2[kJ2C / 2];
 #pragma unroll
-    for (int j = 0; j < kRS; ++j) fx[j] = (j < rs) ? p.fx_pack[j * T + tid] : 0u;
+    for (int e = 0; e < CP / 2; ++e) f1[e] = p.f1_pack[e * T + tid];
 #pragma unroll
-    for (int j = 0; j < kinnet::kFastSlots3; ++j) fxc[j] = (j < rs) ? p.fxc_pack[j * T + tid] : 0u;
-#pragma unroll
-    for (int e = 0; e < kPC / 2; ++e) pl[e] = p.plus_pack[e * T + tid];
-#pragma unroll
-    for (int e = 0; e < kMC / 2; ++e) mi[e] = p.minus_pack[e * T + tid];
-#pragma unroll
-    for (int b = 0; b < 2 * kMaxBig; ++b) rb[b] = p.rb_pack[b * T + tid];
-    // warp-wide trip counts (threads of a warp own rows of similar length)
-    int wnp, wnm;
-    uint32_t wrb = 0;
+    for (int e = 0; e < kJ2C / 2; ++e) f2[e] = p.f2_pack[e * T + tid];
+    int npair, wn2;
     {
-        const uint32_t cnt = p.cnt_pack[tid], rbcnt = p.rbcnt_pack[tid];
-        wnp = __reduce_max_sync(0xffffffffu, cnt & 255u);
-        wnm = __reduce_max_sync(0xffffffffu, (cnt >> 8) & 255u);
-#pragma unroll
-        for (int b = 0; b < 2 * kMaxBig; ++b)
-            wrb |= __reduce_max_sync(0xffffffffu, (rbcnt >> (4 * b)) & 15u) << (4 * b);
+        const uint32_t cnt = p.cnt[tid];
+        npair = (__reduce_max_sync(0xffffffffu, cnt & 255u) + 1) >> 1;  // warp-wide trip count
+        wn2 = __reduce_max_sync(0xffffffffu, (cnt >> 8) & 255u);
     }
 
-    // ---- S1: rates, once per zone per call, kept in registers ------------------
-    real R[kRS];
+    // ---- S1: rates, once per zone per call -----------
     {
-        const int slots = rs * T;
         const double T9 = p.T9[z], rho = p.rho[z];
         const double t13 = cbrt(T9);
         const double t53 = T9 * t13 * t13;
         const double lnT = log(T9), lnrho = log(rho);
-#pragma unroll
-        for (int j = 0; j < kRS; ++j) {
-            R[j] = 0;
-            if (j < rs) {
-                const double* c = p.coef + (j * T + tid);
-                const double lnR = c[0] + c[1 * (size_t)slots] / T9 + c[2 * (size_t)slots] / t13 +
-                                   c[3 * (size_t)slots] * t13 + c[4 * (size_t)slots] * T9 +
-                                   c[5 * (size_t)slots] * t53 + c[6 * (size_t)slots] * lnT;
-                R[j] = static_cast<real>(exp(c[7 * (size_t)slots] * lnrho + lnR));
-            }
+        for (int r = tid; r < M; r += T) {
+            const double* c = p.coef + r;
+            const double lnR = c[0] + c[1 * (size_t)M] / T9 + c[2 * (size_t)M] / t13 +
+                               c[3 * (size_t)M] * t13 + c[4 * (size_t)M] * T9 +
+                               c[5 * (size_t)M] * t53 + c[6 * (size_t)M] * lnT;
+            Rbuf[r] = exp(c[7 * (size_t)M] * lnrho + lnR);
         }
     }
-
-    // ---- S6: zone state in ------------------------------------------------------
-    real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
-    for (int i = tid; i < N; i += T) Ybuf[i] = Yg[i];
-    if (tid == 0) Ybuf[N] = static_cast<real>(1);
-    fcol[rs * T] = static_cast<real>(0);
-    const int own = p.owner[tid];
-    const bool is_big = (tid >= W && tid < W + nbs);
+    if (tid < 4) YP[4 * T + tid] = static_cast<real>(1);
     __syncthreads();
-    real y = (own >= 0) ? Ybuf[own] : static_cast<real>(0);
+
+    // rates of the P-slots and the rate sums of this thread, kept in registers
+    real R[CP];
+#pragma unroll
+    for (int e = 0; e < CP; ++e) {
+        const int32_t v = p.slot_rxn[e * T + tid];
+        R[e] = v < 0 ? static_cast<real>(0)
+                     : static_cast<real>(static_cast<double>(v >> 24) * Rbuf[v & 0xffffff]);
+    }
+    real C[kinnet::kPullCoefs];
+    {
+        int q = p.agg_ptr[tid];
+#pragma unroll
+        for (int s = 0; s < kinnet::kPullCoefs; ++s) {
+            const int qe = p.agg_ptr[(s + 1) * T + tid];
+            double acc = 0.0;
+            for (; q < qe; ++q) {  // fixed (reaction) order
+                const int32_t v = p.agg_ent[(size_t)q * T + tid];
+                acc += static_cast<double>(v >> 24) * Rbuf[v & 0xffffff];
+            }
+            C[s] = static_cast<real>(acc);
+        }
+    }
+    const real K0 = C[0], K1 = C[1], K2 = C[2], K3 = C[3], K00 = C[4], K01 = C[5], K02 = C[6],
+               K11 = C[7], K12 = C[8], K22 = C[9];
+
+    // ---- S6: zone state in ---------------------------------------------------------
+    real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
+    const int own = p.owner[tid];
+    const bool hub_owner = tid < nbs;  // hub h is owned by thread h
+    real y = (own >= 0) ? Yg[own] : static_cast<real>(0);
+    real yh0 = nbs > 0 ? Yg[p.hub[0]] : static_cast<real>(0);
+    real yh1 = nbs > 1 ? Yg[p.hub[1]] : static_cast<real>(0);
+    real yh2 = nbs > 2 ? Yg[p.hub[2]] : static_cast<real>(0);
 
     const real kappa = static_cast<real>(p.kappa);
     const real eps_y = static_cast<real>(p.eps_y);
@@ -490,127 +521,149 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_reg(const KParams p) {
     int steps = 0;
     int status = 0;
     bool run = true;
-    if (MODE == kAdaptive) {
+    if (mode == kAdaptive) {
         const double dt_in = p.dt ? p.dt[z] : 0.0;
         dt_prev = (dt_in > 0.0) ? dt_in : t_hydro;
         run = t_hydro > 0.0;
-        if (!run) dt_prev = dt_in;
-    } else if (MODE == kFixed) {
+        if (!run) dt_prev = dt_in;  // nothing to do: the trial dt is returned unchanged
+    } else if (mode == kFixed) {
         run = p.n_fixed > 0;
     }
-    const int max_steps = static_cast<int>(MODE == kFixed ? p.n_fixed : p.max_steps);
+    const int max_steps = (mode == kFixed) ? p.n_fixed : p.max_steps;
 
     while (run) {
-        // ---- S2: fluxes -------------------------------------------------------
-#pragma unroll
-        for (int j = 0; j < kRS; ++j) {
-            if (j < rs) {
-                real v = R[j] * lds_at<real>(Yb, lo16(fx[j]));
-                if (j < j2) v = v * lds_at<real>(Yb, hi16(fx[j]));
-                if (j < kinnet::kFastSlots3 && j < j3) v = v * lds_at<real>(Yb, fxc[j]);
-                fcol[j * T] = v;
+        // ---- publish y x {1, hubs} ------------------------------------------------
+        YP[tid] = y;
+        YP[T + tid] = y * yh0;
+        YP[2 * T + tid] = y * yh1;
+        YP[3 * T + tid] = y * yh2;
+
+        // ---- rate sums: k = F-/y (Eq. (1)) and this thread's share of the hub rows ---
+        real k, acc[8];
+        {
+            real e0 = fma(K00, yh0, K1);
+            e0 = fma(K01, yh1, e0);
+            e0 = fma(K02, yh2, e0);
+            real e1 = fma(K11, yh1, K2);
+            e1 = fma(K12, yh2, e1);
+            const real e2 = fma(K22, yh2, K3);
+            k = fma(yh0, e0, K0);
+            k = fma(yh1, e1, k);
+            k = fma(yh2, e2, k);
+            // F-_hub share / y: Y_h dk/dY_h (each hub co-reactant occurrence counts once)
+            real m0 = fma(K00, yh0, e0);
+            real m1 = fma(K01, yh0, e1);
+            m1 = fma(K11, yh1, m1);
+            real m2 = fma(K02, yh0, e2);
+            m2 = fma(K12, yh1, m2);
+            m2 = fma(K22, yh2, m2);
+            m0 *= yh0;
+            m1 *= yh1;
+            m2 *= yh2;
+            if (hub_owner) {  // the owner's own consumption of a hub-only reaction
+                if (tid == 0) m0 += k;
+                if (tid == 1) m1 += k;
+                if (tid == 2) m2 += k;
             }
+            // F+_hub share / y
+            real g0 = fma(C[13], yh1, C[10]);
+            g0 = fma(C[14], yh2, g0);
+            real g1 = fma(C[15], yh0, C[11]);
+            g1 = fma(C[16], yh2, g1);
+            real g2 = fma(C[17], yh0, C[12]);
+            g2 = fma(C[18], yh1, g2);
+            acc[0] = y * g0;
+            acc[1] = y * g1;
+            acc[2] = y * g2;
+            acc[3] = y * m0;
+            acc[4] = y * m1;
+            acc[5] = y * m2;
+            acc[6] = 0;
+            acc[7] = 0;
         }
         __syncthreads();
 
-        // ---- S3: sums (zero-padded lists: no per-lane predicates) ------------------
-        real Fp = 0, Fm = 0;
+        // ---- S2+S3: F+ = sum of the incoming fluxes, each evaluated here ---------------
+        real Fp;
         {
-            real Fp1 = 0, Fm1 = 0;
-#pragma unroll
-            for (int g = 0; g < kPC / 4; ++g) {
-                if (4 * g < wnp) {
-                    const uint32_t w0 = pl[2 * g], w1 = pl[2 * g + 1];
-                    Fp += lds_at<real>(fb, lo16(w0));
-                    Fp1 += lds_at<real>(fb, hi16(w0));
-                    Fp += lds_at<real>(fb, lo16(w1));
-                    Fp1 += lds_at<real>(fb, hi16(w1));
-                }
+            real s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+#define PULL_PAIR(I, SA, SB)                                        \
+    if constexpr (2 * (I) < CP) {                                   \
+        const uint32_t w_ = f1[I];                                  \
+        real a_ = lds_at<real>(YPb, lo16(w_));                      \
+        real b_ = lds_at<real>(YPb, hi16(w_));                      \
+        if constexpr (2 * (I) < kJ2C) {                             \
+            if (2 * (I) < wn2) {                                    \
+                const uint32_t v_ = f2[I];                          \
+                a_ *= lds_at<real>(YPb, lo16(v_));                  \
+                b_ *= lds_at<real>(YPb, hi16(v_));                  \
+            }                                                       \
+        }                                                           \
+        SA = fma(R[2 * (I)], a_, SA);                               \
+        SB = fma(R[2 * (I) + 1], b_, SB);                           \
+    }
+            switch (npair) {
+                case 12: PULL_PAIR(11, s2, s3) [[fallthrough]];
+                case 11: PULL_PAIR(10, s0, s1) [[fallthrough]];
+                case 10: PULL_PAIR(9, s2, s3) [[fallthrough]];
+                case 9: PULL_PAIR(8, s0, s1) [[fallthrough]];
+                case 8: PULL_PAIR(7, s2, s3) [[fallthrough]];
+                case 7: PULL_PAIR(6, s0, s1) [[fallthrough]];
+                case 6: PULL_PAIR(5, s2, s3) [[fallthrough]];
+                case 5: PULL_PAIR(4, s0, s1) [[fallthrough]];
+                case 4: PULL_PAIR(3, s2, s3) [[fallthrough]];
+                case 3: PULL_PAIR(2, s0, s1) [[fallthrough]];
+                case 2: PULL_PAIR(1, s2, s3) [[fallthrough]];
+                case 1: PULL_PAIR(0, s0, s1) [[fallthrough]];
+                default: break;
             }
-#pragma unroll
-            for (int g = 0; g < kMC / 4; ++g) {
-                if (4 * g < wnm) {
-                    const uint32_t w0 = mi[2 * g], w1 = mi[2 * g + 1];
-                    Fm += lds_at<real>(fb, lo16(w0));
-                    Fm1 += lds_at<real>(fb, hi16(w0));
-                    Fm += lds_at<real>(fb, lo16(w1));
-                    Fm1 += lds_at<real>(fb, hi16(w1));
-                }
-            }
-            Fp += Fp1;
-            Fm += Fm1;
+#undef PULL_PAIR
+            Fp = (s0 + s1) + (s2 + s3);
         }
-        if (nbs > 0) {
-            real acc[8];
-            const unsigned char* fc = reinterpret_cast<const unsigned char*>(fcol);
-#pragma unroll
-            for (int b = 0; b < 8; ++b) {
-                acc[b] = 0;
-                if (b < 2 * kMaxBig) {
-                    const int wmax = (wrb >> (4 * b)) & 15u;
-#pragma unroll
-                    for (int q = 0; q < kinnet::kFastRowCap; q += 2) {
-                        if (q < wmax) {
-                            const uint32_t s0 = nib(rb[b], q);
-                            const uint32_t s1 = nib(rb[b], q + 1);
-                            acc[b] += lds_at<real>(fc, s0 * col_stride);
-                            acc[b] += lds_at<real>(fc, s1 * col_stride);
-                        }
-                    }
-                }
-            }
-            const real tot = warp_sum_rows8(acc, lane);
-            if ((lane & 3) == 0) red[warp * kRedStride + (lane >> 2)] = tot;
-        }
-        // ---- S5: dt candidates of the small species ---------------------------------
-        if (MODE == kAdaptive) {
+
+        // ---- S5: dt candidates of the non-hub species ------------------------------------
+        if (mode == kAdaptive) {
             double c = INFINITY;
-            if (own >= 0 && !is_big) {
-                real a = Fp - Fm;
-                a = a < 0 ? -a : a;
-                if (a > Tiny<real>::v())
-                    c = static_cast<double>(eps_y * (y > y_floor ? y : y_floor) * rcp_pos(a));
-            }
+            if (own >= 0 && !hub_owner) c = dt_candidate(y, Fp - k * y, eps_y, y_floor);
             c = warp_min_pos(c);
             if (lane == 0) redmin[warp] = c;
-            if (is_big) ybig[tid - W] = static_cast<double>(y);
+        }
+        // ---- hub rows: warp totals of the six partial sums ---------------------------------
+        if (nbs > 0) {
+            const real tot = warp_sum_rows8(acc, lane);
+            if ((lane & 3) == 0) red[warp * 8 + (lane >> 2)] = tot;
         }
         __syncthreads();
 
-        // ---- finalize: big species sums, zone-wide dt ---------------------------------
-        real bFp = 0, bFm = 0;
+        // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
+        real hFp = 0, hFm = 0;
+        const real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
         double cand = INFINITY;
-        if (lane >= W && lane < W + nbs) {
-            const int s = lane - W;
-            for (int w = 0; w < W; ++w) {
-                bFp += red[w * kRedStride + 2 * s];
-                bFm += red[w * kRedStride + 2 * s + 1];
+        if (lane < nbs) {
+            for (int w = 0; w < W; ++w) {  // fixed order over warps
+                hFp += red[w * 8 + lane];
+                hFm += red[w * 8 + 3 + lane];
             }
-            if (MODE == kAdaptive) {
-                const real yb = static_cast<real>(ybig[s]);
-                real a = bFp - bFm;
-                a = a < 0 ? -a : a;
-                if (a > Tiny<real>::v())
-                    cand = static_cast<double>(eps_y * (yb > y_floor ? yb : y_floor) * rcp_pos(a));
-            }
-        } else if (MODE == kAdaptive && lane < W) {
-            cand = redmin[lane];
+            if (mode == kAdaptive) cand = dt_candidate(yme, hFp - hFm, eps_y, y_floor);
+        } else if (mode == kAdaptive && lane >= 8 && lane < 8 + W) {
+            cand = redmin[lane - 8];
         }
-        if (is_big) {
-            Fp = bFp;
-            Fm = bFm;
-        }
-        if (MODE == kRhs) {
-            if (own >= 0) {
-                reinterpret_cast<real*>(p.Fplus)[(size_t)z * N + own] = Fp;
-                reinterpret_cast<real*>(p.Fminus)[(size_t)z * N + own] = Fm;
+        if (mode == kRhs) {
+            real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
+            real* Fmo = reinterpret_cast<real*>(p.Fminus) + (size_t)z * N;
+            if (hub_owner) {
+                Fpo[own] = hFp;
+                Fmo[own] = hFm;
+            } else if (own >= 0) {
+                Fpo[own] = Fp;
+                Fmo[own] = k * y;
             }
             return;
         }
 
         double dts;
         bool last;
-        if (MODE == kAdaptive) {
+        if (mode == kAdaptive) {
             const double cmin = warp_min_pos(cand);
             double dt_ctrl = growth * dt_prev;
             if (cmin < dt_ctrl) dt_ctrl = cmin;
@@ -627,37 +680,49 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_reg(const KParams p) {
             dts = p.dt_fixed;
             last = (steps + 1 >= max_steps);
         }
+        const real h = static_cast<real>(dts);
 
-        // ---- S4: update -------------------------------------------------------------------
-        if (own >= 0) {
-            const real h = static_cast<real>(dts);
-            const real hFm = h * Fm;
-            if (y > 0 && hFm >= kappa * y) {  // k dt >= kappa with k = F-/Y
-                const real den = y + hFm;      // Eq. (3) as Y (Y + dt F+) / (Y + dt F-)
-                if (den > Tiny<real>::v() && y > Tiny<real>::v())
-                    y = (y + h * Fp) * (y * rcp_pos(den));
+        // ---- S4: update (Eq. (3)) -------------------------------------------
+        if (nbs > 0) {  // hub species, on lanes 0..nbs-1 of every warp, from F+ and F-
+            real yn = yme;
+            const real hFmh = h * hFm;
+            if (yme > 0 && hFmh >= kappa * yme) {  // k dt >= kappa with k = F-/Y
+                const real den = yme + hFmh;        // Eq. (3) as Y (Y + dt F+) / (Y + dt F-)
+                if (den > Tiny<real>::v() && yme > Tiny<real>::v())
+                    yn = (yme + h * hFp) * (yme * rcp_pos(den));
                 else
-                    y = (y + h * Fp) / (static_cast<real>(1) + (Fm / y) * h);
+                    yn = (yme + h * hFp) / (static_cast<real>(1) + (hFm / yme) * h);
             } else {
-                y = y + h * (Fp - Fm);
+                yn = yme + h * (hFp - hFm);
             }
-            Ybuf[own] = y;
+            yh0 = __shfl_sync(0xffffffffu, yn, 0);
+            if (nbs > 1) yh1 = __shfl_sync(0xffffffffu, yn, 1);
+            if (nbs > 2) yh2 = __shfl_sync(0xffffffffu, yn, 2);
+        }
+        if (hub_owner) {
+            y = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
+        } else {  // own species from F+ and k
+            const real kh = k * h;
+            if (y > 0 && kh >= kappa)
+                y = (y + h * Fp) * rcp_pos(static_cast<real>(1) + kh);
+            else
+                y = y + h * (Fp - k * y);
         }
         t = last ? t_hydro : t + dts;
         ++steps;
         if (last) run = false;
-        else if (MODE == kAdaptive && steps >= max_steps) {
+        else if (mode == kAdaptive && steps >= max_steps) {
             status |= NET_STATUS_MAX_STEPS;
             run = false;
         }
-        __syncthreads();
     }
 
+    // ---- S6: zone state out ------------------------------------------------------------------
     const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
-    for (int i = tid; i < N; i += T) Yg[i] = Ybuf[i];
+    if (own >= 0) Yg[own] = y;
     if (tid == 0) {
-        if (MODE == kAdaptive && p.dt) p.dt[z] = dt_prev;
+        if (mode == kAdaptive && p.dt) p.dt[z] = dt_prev;
         if (p.n_steps) p.n_steps[z] = steps;
         if (p.status) p.status[z] = status;
     }
@@ -673,19 +738,22 @@ struct DeviceTables {
     uint16_t* small_src = nullptr;
     uint8_t* big_cnt = nullptr;
     uint8_t* big_slot = nullptr;
-    uint32_t* fx_pack = nullptr;
-    uint32_t* fxc_pack = nullptr;
-    uint32_t* plus_pack = nullptr;
-    uint32_t* minus_pack = nullptr;
-    uint32_t* rb_pack = nullptr;
-    uint32_t* cnt_pack = nullptr;
-    uint32_t* rbcnt_pack = nullptr;
+    // pull kernel
+    double* coef_rxn = nullptr;
+    int32_t* p_owner = nullptr;
+    uint32_t* p_cnt = nullptr;
+    int32_t* p_slot_rxn = nullptr;
+    uint32_t* p_f1 = nullptr;
+    uint32_t* p_f2 = nullptr;
+    uint16_t* p_agg_ptr = nullptr;
+    int32_t* p_agg_ent = nullptr;
 };
 
 }  // namespace
 
 struct net {
     Schedule S;
+    kinnet::PullSchedule PS;
     net_params_t P;
     bool has_device = false;
     bool force_generic = false;  // params.kernel == 1: keep the table-driven kernel (A/B tests)
@@ -718,40 +786,54 @@ kernel_fn pick_block(int T) {
     return zone_kernel<real, MODE, 1024>;
 }
 
-// register-resident kernel: block-size classes with the residency the register
-// file allows (65536 / (TB * MINB) registers per thread)
-template <typename real, int MODE>
-kernel_fn pick_block_reg(int T) {
-    if (T <= 64) return zone_kernel_reg<real, MODE, 64, 8>;
-    if (T <= 160) return zone_kernel_reg<real, MODE, 160, 3>;
-    if (T <= 256) return zone_kernel_reg<real, MODE, 256, 2>;
-    if (T <= 512) return zone_kernel_reg<real, MODE, 512, 1>;
-    return nullptr;
+// pull kernel: block-size classes with the residency the register file allows
+// (65536 / (TB * MINB) registers per thread) x P-slot capacity classes
+typedef void (*pull_fn)(const KPull);
+
+template <typename real, int CP>
+pull_fn pick_pull_block(int T) {
+    if (T <= 64) return zone_kernel_pull<real, 64, 8, CP>;
+    if (T <= 160) {
+        const char* e = std::getenv("KINNET_PULL_MINB");  // tuning knob while measuring residency
+        if (e && e[0] == '2') return zone_kernel_pull<real, 160, 2, CP>;
+        return zone_kernel_pull<real, 160, 3, CP>;
+    }
+    if (T <= 256) return zone_kernel_pull<real, 256, 2, CP>;
+    if (T <= 384) return zone_kernel_pull<real, 384, 1, CP>;
+    return zone_kernel_pull<real, 512, 1, CP>;
 }
 
-bool use_reg_kernel(const net* n);
+template <typename real>
+pull_fn pick_pull_real(const kinnet::PullSchedule& P) {
+    if (P.slots <= 12) return pick_pull_block<real, 12>(P.T);
+    if (P.slots <= 20) return pick_pull_block<real, 20>(P.T);
+    return pick_pull_block<real, 24>(P.T);
+}
+
+bool use_pull_kernel(const net* n) { return n->PS.ok && !n->force_generic; }
+
+pull_fn pick_pull(const net* n) {
+    return n->P.precision == 32 ? pick_pull_real<float>(n->PS) : pick_pull_real<double>(n->PS);
+}
+
+size_t pull_smem(const net* n) {
+    return n->P.precision == 32 ? pull_smem_bytes<float>(n->PS.T, n->PS.W, n->S.M)
+                                : pull_smem_bytes<double>(n->PS.T, n->PS.W, n->S.M);
+}
 
 template <int MODE>
 kernel_fn pick_kernel(const net* n) {
     if constexpr (MODE == kRates) return pick_block<double, MODE>(n->S.T);
-    else if (use_reg_kernel(n)) {
-        kernel_fn f = n->P.precision == 32 ? pick_block_reg<float, MODE>(n->S.T)
-                                           : pick_block_reg<double, MODE>(n->S.T);
-        if (f) return f;
-    }
     return n->P.precision == 32 ? pick_block<float, MODE>(n->S.T) : pick_block<double, MODE>(n->S.T);
 }
 
-bool use_reg_kernel(const net* n) { return n->S.fast_ok && !n->force_generic; }
-
 size_t net_smem(const net* n) {
-    if (use_reg_kernel(n))
-        return n->P.precision == 32 ? smem_bytes_reg<float>(n->S) : smem_bytes_reg<double>(n->S);
+    if (use_pull_kernel(n)) return pull_smem(n);
     return n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
 }
 
 int prepare_kernels(net* n) {
-    const size_t smem = net_smem(n);
+    const size_t smem = n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
     kernel_fn fns[4] = {pick_kernel<kAdaptive>(n), pick_kernel<kFixed>(n), pick_kernel<kRhs>(n),
                         pick_kernel<kRates>(n)};
     for (kernel_fn f : fns) {
@@ -761,10 +843,88 @@ int prepare_kernels(net* n) {
                                       static_cast<int>(need)));
     }
     int nb = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-        &nb, reinterpret_cast<const void*>(fns[0]), n->S.T, smem));
+    if (use_pull_kernel(n)) {
+        const void* f = reinterpret_cast<const void*>(pick_pull(n));
+        CUDA_TRY(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      static_cast<int>(pull_smem(n))));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, n->PS.T, pull_smem(n)));
+    } else {
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+            &nb, reinterpret_cast<const void*>(fns[0]), n->S.T, smem));
+    }
     n->zones_per_sm = nb;
     return NET_OK;
+}
+
+void fill_pull(const net* n, KPull& k) {
+    const kinnet::PullSchedule& P = n->PS;
+    std::memset(&k, 0, sizeof(k));
+    k.N = n->S.N; k.M = n->S.M; k.T = P.T; k.W = P.W; k.nbs = P.nbs;
+    for (int h = 0; h < kinnet::kPullHubs; ++h) k.hub[h] = P.hub[h];
+    k.coef = n->D.coef_rxn;
+    k.owner = n->D.p_owner;
+    k.cnt = n->D.p_cnt;
+    k.slot_rxn = n->D.p_slot_rxn;
+    k.f1_pack = n->D.p_f1;
+    k.f2_pack = n->D.p_f2;
+    k.agg_ptr = n->D.p_agg_ptr;
+    k.agg_ent = n->D.p_agg_ent;
+    k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
+    k.growth = n->P.growth; k.max_steps = static_cast<int>(n->P.max_steps);
+}
+
+int launch_pull(net* n, int zones, KPull& k, void* stream) {
+    pull_fn f = pick_pull(n);
+    f<<<zones, n->PS.T, pull_smem(n), static_cast<cudaStream_t>(stream)>>>(k);
+    CUDA_TRY(cudaGetLastError());
+    return NET_OK;
+}
+
+// Device copies of the pull schedule.  Offsets are BYTE offsets into the YP
+// table for elements of `elem` bytes; rows are padded to the largest kernel
+// instantiation so every instantiation may read its full capacity.
+int upload_pull(net* n) {
+    const kinnet::PullSchedule& P = n->PS;
+    const Schedule& S = n->S;
+    const int T = P.T, M = S.M;
+    const uint32_t elem = n->P.precision == 32 ? 4u : 8u;
+    const int slots = S.rs * S.T;
+    std::vector<double> coef(static_cast<size_t>(kinnet::kCoefRows) * M);
+    for (int idx = 0; idx < slots; ++idx) {
+        const int r = S.flux_rxn[idx];
+        if (r < 0) continue;
+        for (int c = 0; c < kinnet::kCoefRows; ++c)
+            coef[static_cast<size_t>(c) * M + r] = S.coef[static_cast<size_t>(c) * slots + idx];
+    }
+    const uint32_t one_off = static_cast<uint32_t>(4 * T) * elem;
+    std::vector<uint32_t> cnt(T), f1(static_cast<size_t>(kinnet::kPullMaxSlots / 2) * T),
+        f2(static_cast<size_t>(kinnet::kPullMaxSlots2 / 2) * T);
+    std::vector<int32_t> rxn(static_cast<size_t>(kinnet::kPullMaxSlots) * T, -1);
+    for (int t = 0; t < T; ++t) {
+        cnt[t] = P.n_slots[t] | static_cast<uint32_t>(P.n_slots2[t]) << 8;
+        for (int e = 0; e < kinnet::kPullMaxSlots; ++e) {
+            uint32_t off = one_off;
+            if (e < P.slots) {
+                off = P.slot_f1[static_cast<size_t>(e) * T + t] * elem;
+                rxn[static_cast<size_t>(e) * T + t] = P.slot_rxn[static_cast<size_t>(e) * T + t];
+            }
+            f1[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
+        }
+        for (int e = 0; e < kinnet::kPullMaxSlots2; ++e) {
+            const uint32_t off =
+                e < P.slots2 ? P.slot_f2[static_cast<size_t>(e) * T + t] * elem : one_off;
+            f2[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
+        }
+    }
+    int rc = upload(&n->D.coef_rxn, coef.data(), coef.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_owner, P.owner.data(), P.owner.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_cnt, cnt.data(), cnt.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_slot_rxn, rxn.data(), rxn.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_f1, f1.data(), f1.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_f2, f2.data(), f2.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_agg_ptr, P.agg_ptr.data(), P.agg_ptr.size());
+    if (rc == NET_OK) rc = upload(&n->D.p_agg_ent, P.agg_ent.data(), P.agg_ent.size());
+    return rc;
 }
 
 void fill_params(const net* n, KParams& k) {
@@ -782,13 +942,6 @@ void fill_params(const net* n, KParams& k) {
     k.small_src = n->D.small_src;
     k.big_cnt = n->D.big_cnt;
     k.big_slot = n->D.big_slot;
-    k.fx_pack = n->D.fx_pack;
-    k.fxc_pack = n->D.fxc_pack;
-    k.plus_pack = n->D.plus_pack;
-    k.minus_pack = n->D.minus_pack;
-    k.rb_pack = n->D.rb_pack;
-    k.cnt_pack = n->D.cnt_pack;
-    k.rbcnt_pack = n->D.rbcnt_pack;
     k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
     k.growth = n->P.growth; k.max_steps = n->P.max_steps;
 }
@@ -838,7 +991,12 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         delete n;
         return fail(rc, err);
     }
-    if (n->S.fast_ok) kinnet::pack_fast_tables(n->S, n->P.precision == 32 ? 4 : 8);
+    try {
+        kinnet::build_pull_schedule(N, M, n_react, react, n_prod, prod, n->PS);
+    } catch (const std::bad_alloc&) {
+        delete n;
+        return fail(NET_ENOMEM, "out of host memory");
+    }
     if (net_smem(n) > 227 * 1024) {
         delete n;
         return fail(NET_EINVAL, "network too large for one CTA's shared memory");
@@ -857,15 +1015,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         if (rc == NET_OK) rc = upload(&n->D.small_src, S.small_src.data(), S.small_src.size());
         if (rc == NET_OK) rc = upload(&n->D.big_cnt, S.big_cnt.data(), S.big_cnt.size());
         if (rc == NET_OK) rc = upload(&n->D.big_slot, S.big_slot.data(), S.big_slot.size());
-        if (rc == NET_OK && S.fast_ok) {
-            rc = upload(&n->D.fx_pack, S.fx_pack.data(), S.fx_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.fxc_pack, S.fxc_pack.data(), S.fxc_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.plus_pack, S.plus_pack.data(), S.plus_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.minus_pack, S.minus_pack.data(), S.minus_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.rb_pack, S.rb_pack.data(), S.rb_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.cnt_pack, S.cnt_pack.data(), S.cnt_pack.size());
-            if (rc == NET_OK) rc = upload(&n->D.rbcnt_pack, S.rbcnt_pack.data(), S.rbcnt_pack.size());
-        }
+        if (rc == NET_OK && n->PS.ok) rc = upload_pull(n);
         if (rc == NET_OK) {
             n->has_device = true;
             rc = prepare_kernels(n);
@@ -917,8 +1067,9 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.flux_rxn); cudaFree(n->D.flux_react); cudaFree(n->D.coef);
         cudaFree(n->D.owner); cudaFree(n->D.small_plus); cudaFree(n->D.small_minus);
         cudaFree(n->D.small_src); cudaFree(n->D.big_cnt); cudaFree(n->D.big_slot);
-        cudaFree(n->D.fx_pack); cudaFree(n->D.fxc_pack); cudaFree(n->D.plus_pack); cudaFree(n->D.minus_pack);
-        cudaFree(n->D.rb_pack); cudaFree(n->D.cnt_pack); cudaFree(n->D.rbcnt_pack);
+        cudaFree(n->D.coef_rxn); cudaFree(n->D.p_owner); cudaFree(n->D.p_cnt);
+        cudaFree(n->D.p_slot_rxn); cudaFree(n->D.p_f1); cudaFree(n->D.p_f2);
+        cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
         cudaFree(n->ssteps); cudaFree(n->sstatus);
         if (n->host_stream) cudaStreamDestroy(n->host_stream);
@@ -931,6 +1082,17 @@ int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void
     if (!n) return fail(NET_EINVAL, "null net");
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
     if (!(t_hydro == t_hydro)) return fail(NET_EINVAL, "t_hydro is NaN");
+    if (n->has_device && use_pull_kernel(n)) {
+        if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+        if (zones == 0) return NET_OK;
+        if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
+        KPull q;
+        fill_pull(n, q);
+        q.mode = kAdaptive;
+        q.T9 = T9; q.rho = rho; q.Y = Y; q.dt = dt; q.n_steps = n_steps; q.status = status;
+        q.t_hydro = t_hydro;
+        return launch_pull(n, zones, q, stream);
+    }
     KParams k;
     fill_params(n, k);
     k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
@@ -943,6 +1105,17 @@ int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho
     if (!n) return fail(NET_EINVAL, "null net");
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
     if (n_steps < 0 || n_steps > 2000000000LL) return fail(NET_EINVAL, "n_steps out of range [0, 2e9]");
+    if (n->has_device && use_pull_kernel(n)) {
+        if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+        if (zones == 0) return NET_OK;
+        if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
+        KPull q;
+        fill_pull(n, q);
+        q.mode = kFixed;
+        q.T9 = T9; q.rho = rho; q.Y = Y;
+        q.dt_fixed = dt_fixed; q.n_fixed = static_cast<int>(n_steps);
+        return launch_pull(n, zones, q, stream);
+    }
     KParams k;
     fill_params(n, k);
     k.T9 = T9; k.rho = rho; k.Y = Y;
@@ -963,6 +1136,16 @@ int net_rhs(net_t* n, int zones, const double* T9, const double* rho, const void
             void* Fminus, void* stream) {
     if (!n) return fail(NET_EINVAL, "null net");
     if (zones > 0 && (!Y || !Fplus || !Fminus)) return fail(NET_EINVAL, "null Y/Fplus/Fminus");
+    if (n->has_device && use_pull_kernel(n)) {
+        if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+        if (zones == 0) return NET_OK;
+        if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
+        KPull q;
+        fill_pull(n, q);
+        q.mode = kRhs;
+        q.T9 = T9; q.rho = rho; q.Y = const_cast<void*>(Y); q.Fplus = Fplus; q.Fminus = Fminus;
+        return launch_pull(n, zones, q, stream);
+    }
     KParams k;
     fill_params(n, k);
     k.T9 = T9; k.rho = rho; k.Y = const_cast<void*>(Y); k.Fplus = Fplus; k.Fminus = Fminus;
@@ -1015,7 +1198,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     const Schedule& S = n->S;
     info->n_species = S.N;
     info->n_reactions = S.M;
-    info->threads = S.T;
+    info->threads = use_pull_kernel(n) ? n->PS.T : S.T;
     info->flux_slots = S.rs;
     info->slots_2body = S.j2;
     info->slots_3body = S.j3;
@@ -1026,6 +1209,14 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     info->readback_max = S.readback_max;
     info->smem_bytes = static_cast<int>(net_smem(n));
     info->zones_per_sm = n->zones_per_sm;
+    info->kernel = use_pull_kernel(n) ? 1 : 0;
+    info->pull_ok = n->PS.ok ? 1 : 0;
+    info->pull_hubs = n->PS.nbs;
+    info->pull_slots = n->PS.slots;
+    info->pull_slots2 = n->PS.slots2;
+    info->pull_agg_max = n->PS.agg_max;
+    info->pull_wavefronts = static_cast<int>(n->PS.conflict_wavefronts);
+    info->pull_wavefronts_ideal = static_cast<int>(n->PS.ideal_wavefronts);
     return NET_OK;
 }
 
@@ -1054,6 +1245,21 @@ int net_schedule_table(const net_t* n, const char* name, int* out, int cap) {
         if (S.nbs == 0) count = 0; else emit(S.big_cnt, 1, 1);
     } else if (key == "big_slot") {
         if (S.readback_max == 0) count = 0; else emit(S.big_slot, 1, 1);
+    } else if (key.rfind("pull_", 0) == 0) {
+        const kinnet::PullSchedule& P = n->PS;
+        if (!P.ok) return fail(NET_EINVAL, "no pull schedule for this network: " + P.why);
+        if (key == "pull_hub") {
+            const std::vector<int32_t> hubs(P.hub, P.hub + P.nbs);
+            emit(hubs, 1, 1);
+        } else if (key == "pull_owner") emit(P.owner, 1, 1);
+        else if (key == "pull_n_slots") emit(P.n_slots, 1, 1);
+        else if (key == "pull_n_slots2") emit(P.n_slots2, 1, 1);
+        else if (key == "pull_slot_rxn") emit(P.slot_rxn, 1, 1);
+        else if (key == "pull_slot_f1") emit(P.slot_f1, 1, 1);
+        else if (key == "pull_slot_f2") emit(P.slot_f2, 1, 1);
+        else if (key == "pull_agg_ptr") emit(P.agg_ptr, 1, 1);
+        else if (key == "pull_agg_ent") emit(P.agg_ent, 1, 1);
+        else return fail(NET_EINVAL, "unknown schedule table '" + key + "'");
     } else return fail(NET_EINVAL, "unknown schedule table '" + key + "'");
     if (out && cap < count) return fail(NET_EINVAL, "output buffer too small");
     return count;

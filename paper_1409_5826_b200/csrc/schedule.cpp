@@ -267,62 +267,225 @@ int build_schedule(int N, const int* A, int M, const int* n_react, const int* re
             for (uint8_t v : rb[t][b]) S.big_slot[static_cast<size_t>(e++) * T + t] = v;
     }
 
-    // ---- packed tables for the register-resident kernel ---------------------
-    S.plus_max = *std::max_element(S.small_plus.begin(), S.small_plus.end());
-    S.minus_max = *std::max_element(S.small_minus.begin(), S.small_minus.end());
-    S.bigrow_max = 0;
-    for (uint8_t c : S.big_cnt) S.bigrow_max = std::max<int>(S.bigrow_max, c);
-    S.fast_ok = N <= 1023 && S.rs <= kFastSlots && S.rs <= 15 && S.j3 <= kFastSlots3 &&
-                S.plus_max <= kFastPlus && S.minus_max <= kFastMinus &&
-                S.bigrow_max <= kFastRowCap && (S.rs + 1) * T * 8 <= 65535;
     return NET_OK;
 }
 
-// Packed tables of the register-resident kernel.  Offsets are BYTE offsets for
-// elements of `elem` bytes (8: double, 4: float).  Gather lists are padded to
-// their capacity with the offset of the thread's own word in the all-zero flux
-// row `rs`, readback lists with the slot id `rs`, so the kernel needs no
-// per-lane predicates.
-void pack_fast_tables(Schedule& S, int elem) {
-    const int T = S.T, slots = S.rs * T;
-    const uint32_t e32 = static_cast<uint32_t>(elem);
-    S.fx_pack.assign(static_cast<size_t>(S.rs) * T, 0);
-    S.fxc_pack.assign(static_cast<size_t>(kFastSlots3) * T, 0);
-    for (int idx = 0; idx < slots; ++idx) {
-        const uint16_t* re = &S.flux_react[static_cast<size_t>(idx) * 4];
-        S.fx_pack[idx] = re[0] * e32 | (re[1] * e32) << 16;
-        if (idx / T < kFastSlots3) S.fxc_pack[idx] = re[2] * e32;
-    }
-    S.plus_pack.assign(static_cast<size_t>(kFastPlus / 2) * T, 0);
-    S.minus_pack.assign(static_cast<size_t>(kFastMinus / 2) * T, 0);
-    S.rb_pack.assign(static_cast<size_t>(2 * kMaxBigSpecies) * T, 0);
-    S.cnt_pack.assign(T, 0);
-    S.rbcnt_pack.assign(T, 0);
-    for (int t = 0; t < T; ++t) {
-        const uint32_t zero_off = static_cast<uint32_t>(S.rs * T + t) * e32;
-        const int np = S.small_plus[t], nm = S.small_minus[t];
-        for (int e = 0; e < kFastPlus; ++e) {
-            const uint32_t off = e < np ? S.small_src[static_cast<size_t>(e) * T + t] * e32 : zero_off;
-            S.plus_pack[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
-        }
-        for (int e = 0; e < kFastMinus; ++e) {
-            const uint32_t off =
-                e < nm ? S.small_src[static_cast<size_t>(np + e) * T + t] * e32 : zero_off;
-            S.minus_pack[static_cast<size_t>(e / 2) * T + t] |= off << (16 * (e & 1));
-        }
-        S.cnt_pack[t] = static_cast<uint32_t>(np) | static_cast<uint32_t>(nm) << 8;
-        int e = 0;
-        for (int b = 0; b < 2 * kMaxBigSpecies; ++b) {
-            const int c = b < 2 * S.nbs ? S.big_cnt[static_cast<size_t>(b) * T + t] : 0;
-            for (int q = 0; q < kFastRowCap; ++q) {
-                const uint32_t sid = q < c ? S.big_slot[static_cast<size_t>(e + q) * T + t]
-                                           : static_cast<uint32_t>(S.rs);
-                S.rb_pack[static_cast<size_t>(b) * T + t] |= sid << (4 * q);
+namespace {
+
+// Shared-memory wavefronts of the P-slot gathers for 8-byte words: a warp's LDS.64
+// is served as two half-warps; within one, lanes that read different words of the
+// same bank pair (word index mod 16) are serialised, equal words are broadcast.
+void pull_wavefronts(const PullSchedule& P, long& actual, long& ideal) {
+    actual = ideal = 0;
+    const int T = P.T;
+    for (int w = 0; w < P.W; ++w) {
+        int wmax = 0;
+        for (int l = 0; l < 32; ++l) wmax = std::max<int>(wmax, P.n_slots[w * 32 + l]);
+        for (int e = 0; e < wmax; ++e)
+            for (int half = 0; half < 2; ++half) {
+                int worst = 0;
+                for (int b = 0; b < 16; ++b) {
+                    std::vector<int> words;
+                    for (int l = 0; l < 16; ++l) {
+                        const int word = P.slot_f1[static_cast<size_t>(e) * T + w * 32 + half * 16 + l];
+                        if (word % 16 == b && std::find(words.begin(), words.end(), word) == words.end())
+                            words.push_back(word);
+                    }
+                    worst = std::max<int>(worst, words.size());
+                }
+                actual += worst;
+                ideal += 1;
             }
-            e += c;
-            S.rbcnt_pack[t] |= static_cast<uint32_t>(c) << (4 * b);
+    }
+}
+
+}  // namespace
+
+void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
+                         const int* prod, PullSchedule& P) {
+    P = PullSchedule();
+    auto reject = [&](const std::string& why) {
+        P.ok = false;
+        P.why = why;
+    };
+    const int T = std::max(32, (N + 31) / 32 * 32);
+    P.T = T;
+    P.W = T / 32;
+    if (T > 512) return reject("more than 512 species");
+    if (M > 65535) return reject("more than 65535 reactions");
+
+    // ---- hubs: the rows with hundreds of terms ------------------
+    std::vector<int> cnt_plus(N, 0), cnt_minus(N, 0);
+    for (int r = 0; r < M; ++r) {
+        for (int q = 0; q < n_react[r]; ++q) ++cnt_minus[react[r * kMaxReact + q]];
+        for (int q = 0; q < n_prod[r]; ++q) ++cnt_plus[prod[r * kMaxProd + q]];
+    }
+    {
+        const int threshold = std::max(48, T / 2);
+        std::vector<int> cand;
+        for (int i = 0; i < N; ++i)
+            if (std::max(cnt_plus[i], cnt_minus[i]) >= threshold) cand.push_back(i);
+        std::stable_sort(cand.begin(), cand.end(), [&](int a, int b) {
+            return cnt_plus[a] + cnt_minus[a] > cnt_plus[b] + cnt_minus[b];
+        });
+        if (static_cast<int>(cand.size()) > kPullHubs) cand.resize(kPullHubs);
+        std::sort(cand.begin(), cand.end());
+        P.nbs = static_cast<int>(cand.size());
+        for (int h = 0; h < P.nbs; ++h) P.hub[h] = cand[h];
+    }
+    std::vector<int> hub_index(N, -1);
+    for (int h = 0; h < P.nbs; ++h) hub_index[P.hub[h]] = h;
+    auto pair_class = [](int a, int b) {  // a <= b, hubs 0..2 -> 4..9
+        static const int tab[3][3] = {{4, 5, 6}, {-1, 7, 8}, {-1, -1, 9}};
+        return tab[a][b];
+    };
+
+    // ---- per reaction: owner, co-reactant class, factors ---------------------------
+    struct Rx {
+        int owner, cls, co[2], nco;
+    };
+    std::vector<Rx> rx(M);
+    for (int r = 0; r < M; ++r) {
+        int heavy = -1, nheavy = 0;
+        for (int q = 0; q < n_react[r]; ++q) {
+            const int s = react[r * kMaxReact + q];
+            if (hub_index[s] < 0) {
+                heavy = s;
+                ++nheavy;
+            }
+        }
+        if (nheavy > 1)
+            return reject("reaction " + std::to_string(r) + " has more than one non-hub reactant");
+        Rx& x = rx[r];
+        x.owner = nheavy == 1 ? heavy : react[r * kMaxReact];
+        x.nco = 0;
+        bool skipped = false;
+        for (int q = 0; q < n_react[r]; ++q) {
+            const int s = react[r * kMaxReact + q];
+            if (s == x.owner && !skipped) {
+                skipped = true;
+                continue;
+            }
+            x.co[x.nco++] = hub_index[s];
+        }
+        if (x.nco == 2 && x.co[0] > x.co[1]) std::swap(x.co[0], x.co[1]);
+        x.cls = x.nco == 0 ? 0 : x.nco == 1 ? 1 + x.co[0] : pair_class(x.co[0], x.co[1]);
+    }
+
+    // ---- species -> thread: hub h on thread h, the rest by falling in-degree ---------
+    std::vector<int> indeg(N, 0);  // P-slots = distinct (reaction, non-hub product) pairs
+    for (int r = 0; r < M; ++r)
+        for (int q = 0; q < n_prod[r]; ++q) {
+            const int s = prod[r * kMaxProd + q];
+            bool first = true;
+            for (int u = 0; u < q; ++u) first = first && prod[r * kMaxProd + u] != s;
+            if (first && hub_index[s] < 0) ++indeg[s];
+        }
+    P.owner.assign(T, -1);
+    P.thread_of.assign(N, -1);
+    for (int h = 0; h < P.nbs; ++h) {
+        P.owner[h] = P.hub[h];
+        P.thread_of[P.hub[h]] = h;
+    }
+    {
+        std::vector<int> rest;
+        for (int i = 0; i < N; ++i)
+            if (hub_index[i] < 0) rest.push_back(i);
+        std::stable_sort(rest.begin(), rest.end(), [&](int a, int b) { return indeg[a] > indeg[b]; });
+        int t = P.nbs;
+        for (int i : rest) {
+            P.owner[t] = i;
+            P.thread_of[i] = t++;
         }
     }
+
+    // ---- P-slots and rate-sum lists ---------------------------------------------------
+    struct Slot {
+        int32_t rxn;
+        uint16_t f1, f2;
+        bool two;
+    };
+    std::vector<std::vector<Slot>> slots(T);
+    std::vector<std::vector<std::vector<int32_t>>> agg(T, std::vector<std::vector<int32_t>>(kPullCoefs));
+    const uint16_t one_word = static_cast<uint16_t>(4 * T);
+    for (int r = 0; r < M; ++r) {  // reaction order = fixed, documented summation order
+        const Rx& x = rx[r];
+        const int t_own = P.thread_of[x.owner];
+        agg[t_own][x.cls].push_back(r | (1 << 24));
+        for (int q = 0; q < n_prod[r]; ++q) {
+            const int s = prod[r * kMaxProd + q];
+            bool first = true;
+            int nu = 0;
+            for (int u = 0; u < q; ++u) first = first && prod[r * kMaxProd + u] != s;
+            if (!first) continue;
+            for (int u = 0; u < n_prod[r]; ++u) nu += prod[r * kMaxProd + u] == s;
+            const int h = hub_index[s];
+            if (h >= 0) {
+                int slot;
+                if (x.nco == 0) slot = 10 + h;
+                else if (x.nco == 1 && x.co[0] != h) {
+                    const int j = x.co[0] - (x.co[0] > h ? 1 : 0);  // index among the other two hubs
+                    slot = 13 + 2 * h + j;
+                } else
+                    return reject("reaction " + std::to_string(r) +
+                                  " makes a hub next to two hub co-reactants or to itself");
+                agg[t_own][slot].push_back(r | (nu << 24));
+            } else {
+                Slot sl;
+                sl.rxn = r | (nu << 24);
+                const int c1 = x.nco == 0 ? 0 : 1 + x.co[0];
+                sl.f1 = static_cast<uint16_t>(c1 * T + t_own);
+                sl.two = x.nco == 2;
+                sl.f2 = sl.two ? static_cast<uint16_t>(P.thread_of[P.hub[x.co[1]]]) : one_word;
+                slots[P.thread_of[s]].push_back(sl);
+            }
+        }
+    }
+    P.n_slots.assign(T, 0);
+    P.n_slots2.assign(T, 0);
+    P.agg_max = 0;
+    for (int t = 0; t < T; ++t) {
+        std::stable_sort(slots[t].begin(), slots[t].end(),
+                         [](const Slot& a, const Slot& b) { return a.two > b.two; });
+        int n2 = 0;
+        for (const Slot& sl : slots[t]) n2 += sl.two;
+        P.slots = std::max<int>(P.slots, slots[t].size());
+        P.slots2 = std::max(P.slots2, n2);
+        if (slots[t].size() > 255) return reject("too many incoming reactions for one species");
+        P.n_slots[t] = static_cast<uint8_t>(slots[t].size());
+        P.n_slots2[t] = static_cast<uint8_t>(n2);
+        int tot = 0;
+        for (const auto& v : agg[t]) tot += static_cast<int>(v.size());
+        P.agg_max = std::max(P.agg_max, tot);
+    }
+    if (P.slots > kPullMaxSlots)
+        return reject("a non-hub species has more than " + std::to_string(kPullMaxSlots) +
+                      " incoming reactions");
+    if (P.slots2 > kPullMaxSlots2)
+        return reject("a non-hub species has more than " + std::to_string(kPullMaxSlots2) +
+                      " incoming three-body reactions");
+    if (P.agg_max > 65535) return reject("rate-sum list too long");
+    const int ns = std::max(1, P.slots), ns2 = std::max(1, P.slots2);
+    P.slot_rxn.assign(static_cast<size_t>(ns) * T, -1);
+    P.slot_f1.assign(static_cast<size_t>(ns) * T, one_word);
+    P.slot_f2.assign(static_cast<size_t>(ns2) * T, one_word);
+    P.agg_ptr.assign(static_cast<size_t>(kPullCoefs + 1) * T, 0);
+    P.agg_ent.assign(static_cast<size_t>(std::max(1, P.agg_max)) * T, 0);
+    for (int t = 0; t < T; ++t) {
+        for (size_t e = 0; e < slots[t].size(); ++e) {
+            P.slot_rxn[e * T + t] = slots[t][e].rxn;
+            P.slot_f1[e * T + t] = slots[t][e].f1;
+            if (slots[t][e].two) P.slot_f2[e * T + t] = slots[t][e].f2;
+        }
+        int pos = 0;
+        for (int c = 0; c < kPullCoefs; ++c) {
+            P.agg_ptr[static_cast<size_t>(c) * T + t] = static_cast<uint16_t>(pos);
+            for (int32_t v : agg[t][c]) P.agg_ent[static_cast<size_t>(pos++) * T + t] = v;
+        }
+        P.agg_ptr[static_cast<size_t>(kPullCoefs) * T + t] = static_cast<uint16_t>(pos);
+    }
+    pull_wavefronts(P, P.conflict_wavefronts, P.ideal_wavefronts);
+    P.ok = true;
 }
 
 }  // namespace kinnet

@@ -53,30 +53,66 @@ struct Schedule {
     int readback_max = 0;
     std::vector<uint8_t> big_slot;     // [readback_max*T] own flux slot of readback entry e
 
-    // ---- packed copies for the register-resident kernel -------------------
-    // fast_ok when the network fits its compile-time capacities (kFast*).
-    bool fast_ok = false;
-    int plus_max = 0, minus_max = 0, bigrow_max = 0;
-    std::vector<uint32_t> fx_pack;     // [rs][T]   byte offsets of Y[a] | Y[b] << 16
-    std::vector<uint32_t> fxc_pack;    // [kFastSlots3][T] byte offset of Y[c] for slot rows < j3
-    std::vector<uint32_t> plus_pack;   // [kFastPlus/2][T]  two 16-bit flux byte offsets per word
-    std::vector<uint32_t> minus_pack;  // [kFastMinus/2][T]
-    std::vector<uint32_t> rb_pack;     // [2*kMaxBigSpecies][T] eight 4-bit own-slot ids per row
-    std::vector<uint32_t> cnt_pack;    // [T] plus | minus << 8
-    std::vector<uint32_t> rbcnt_pack;  // [T] eight 4-bit readback counts, one per big row
 };
-
-constexpr int kFastSlots = 12;   // flux slots per thread held in registers
-constexpr int kFastPlus = 24;    // F+ small-row entries per thread
-constexpr int kFastMinus = 24;   // F- small-row entries per thread
-constexpr int kFastRowCap = 8;   // readback entries per thread and big row
-constexpr int kFastSlots3 = 2;   // slot rows that may hold three-body reactions
-
-void pack_fast_tables(Schedule& S, int elem_bytes);
 
 // Returns 0 or a NET_E* code with a message in err.
 int build_schedule(int N, const int* A, int M, const int* n_react, const int* react,
                    const int* n_prod, const int* prod, const double* coef, Schedule& out,
                    std::string& err);
+
+// ---------------------------------------------------------------------------
+// Pull schedule: the layout of the fast kernel (zone_kernel_pull).
+//
+// No flux array.  Thread t owns species owner[t] and keeps its abundance y in a
+// register.  Up to three hub species (the n-, p-, alpha-like rows with hundreds
+// of terms) are tracked in registers by every thread.  Each
+// sub-step every thread publishes  YP[c][t] = y * {1, Y_hub0, Y_hub1, Y_hub2}[c]
+// to shared memory; then
+//   * F+ of a non-hub species is a gather over its incoming reactions, each flux
+//     evaluated at the consumer:  f_r = R_r * YP[c1][t1] (* YP[c2][t2])   ("P-slot");
+//   * k = F-/y of a non-hub species and the per-thread partial sums of the six
+//     hub rows are polynomials in the hub abundances whose coefficients are sums of
+//     rates over the reactions that share their abundance factors, formed once per
+//     zone per call (T9 and rho are frozen over the hydro step, PAPER.md L47,
+//     L197, L202);
+//   * the hub rows are reduced over the CTA in a fixed order (no atomics).
+// A network qualifies (ok) when every reaction has at most one non-hub reactant,
+// reactions with a hub product have at most one hub co-reactant different from
+// that product, and the capacities below hold; anything else runs on the generic
+// flux-array kernel.
+constexpr int kPullHubs = 3;
+constexpr int kPullClasses = 10;  // co-reactant classes: {}, {h}, {h,h'} (h <= h')
+constexpr int kPullCoefs = 19;    // K[10], G0[3], Gx[3][2]
+constexpr int kPullMaxSlots = 24; // P-slots per thread (largest kernel instantiation)
+constexpr int kPullMaxSlots2 = 8; // P-slots per thread with a second factor
+
+struct PullSchedule {
+    bool ok = false;
+    std::string why;                   // why not, when !ok
+    int T = 0, W = 0, nbs = 0;
+    int hub[kPullHubs] = {-1, -1, -1}; // hub species; hub h is owned by thread h
+    std::vector<int32_t> owner;        // [T] species of thread t or -1
+    std::vector<int32_t> thread_of;    // [N]
+    int slots = 0;                     // max P-slots of any thread
+    int slots2 = 0;                    // max P-slots with a second factor of any thread
+    std::vector<uint8_t> n_slots;      // [T]
+    std::vector<uint8_t> n_slots2;     // [T]  slots [0, n_slots2) have the second factor
+    std::vector<int32_t> slot_rxn;     // [slots][T] reaction | nu << 24, -1 = empty
+    std::vector<uint16_t> slot_f1;     // [slots][T] YP word index c*T + t of the first factor
+    std::vector<uint16_t> slot_f2;     // [slots2][T] YP word index of the second factor (4T = one)
+    // rate sums: coefficient s of thread t = sum of nu * R over agg_ent[agg_ptr[s][t] .. agg_ptr[s+1][t])
+    int agg_max = 0;
+    std::vector<uint16_t> agg_ptr;     // [kPullCoefs + 1][T]
+    std::vector<int32_t> agg_ent;      // [agg_max][T] reaction | nu << 24
+    long conflict_wavefronts = 0;      // predicted shared-memory wavefronts of the P-slot gathers (fp64)
+    long ideal_wavefronts = 0;
+};
+
+// coefficient slots of PullSchedule::agg_ptr
+//   0..9   K_c   c = 0: {}, 1..3: {hub c-1}, 4..9: {0,0},{0,1},{0,2},{1,1},{1,2},{2,2}
+//   10..12 G0_h  reactions of this thread with hub h as a product and no hub co-reactant
+//   13..18 Gx_h,j  hub h as a product, one hub co-reactant: the j-th of the other two hubs
+void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
+                         const int* prod, PullSchedule& out);
 
 }  // namespace kinnet

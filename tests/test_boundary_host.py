@@ -165,3 +165,92 @@ def test_three_alpha_multiplicity_in_schedule():
     kn = K.Net(net, host_only=True)
     got, _ = schedule_entries(net, kn)
     assert got[(0, "-", 0)] == 3 and got[(0, "+", 1)] == 3 and got[(1, "+", 0)] == 1
+
+
+# ------------------------------------------------------------------ pull schedule
+PAIRS = {4: (0, 0), 5: (0, 1), 6: (0, 2), 7: (1, 1), 8: (1, 2), 9: (2, 2)}
+
+
+def pull_entries(net, kn):
+    """Every (species, sign, reaction) term the pull kernel accounts for, rebuilt
+    from its tables alone: P-slots give F+ of non-hub species; rate-sum
+    coefficient K_c gives the owner's F- and the F- of the hubs in class c;
+    G0/Gx give F+ of the hubs."""
+    info = kn.schedule_info()
+    assert info["pull_ok"] == 1
+    T = info["threads"]
+    hub = list(kn.schedule_table("pull_hub"))
+    owner = kn.schedule_table("pull_owner")
+    ns, ns2 = kn.schedule_table("pull_n_slots"), kn.schedule_table("pull_n_slots2")
+    rxn = kn.schedule_table("pull_slot_rxn").reshape(-1, T)
+    f1 = kn.schedule_table("pull_slot_f1").reshape(-1, T)
+    f2 = kn.schedule_table("pull_slot_f2").reshape(-1, T)
+    ptr = kn.schedule_table("pull_agg_ptr").reshape(20, T)
+    agg = kn.schedule_table("pull_agg_ent").reshape(-1, T)
+    assert sorted(o for o in owner if o >= 0) == list(range(net.n_species))
+    assert list(owner[: len(hub)]) == hub  # hub h on thread h
+    ent = Counter()
+    for t in range(T):
+        assert ns2[t] <= ns[t] <= info["pull_slots"]
+        for e in range(rxn.shape[0]):
+            if e >= ns[t]:
+                assert rxn[e, t] == -1
+                continue
+            assert owner[t] >= 0 and owner[t] not in hub
+            r, nu = int(rxn[e, t]) & 0xFFFFFF, int(rxn[e, t]) >> 24
+            ent[(int(owner[t]), "+", r)] += nu
+            # the factors of the slot reproduce the reactant multiset of the reaction
+            c1, t1 = divmod(int(f1[e, t]), T)
+            react = [int(owner[t1])] + ([hub[c1 - 1]] if c1 else [])
+            if e < ns2[t]:
+                assert f2[e, t] < T
+                react.append(int(owner[f2[e, t]]))
+            elif e < f2.shape[0]:
+                assert f2[e, t] == 4 * T
+            assert sorted(react) == sorted(int(s) for s in net.react[r, : net.n_react[r]])
+        for s in range(19):
+            for q in range(ptr[s, t], ptr[s + 1, t]):
+                r, nu = int(agg[q, t]) & 0xFFFFFF, int(agg[q, t]) >> 24
+                if s < 10:
+                    assert nu == 1
+                    ent[(int(owner[t]), "-", r)] += 1
+                    co = [] if s == 0 else [s - 1] if s < 4 else list(PAIRS[s])
+                    for h in co:
+                        ent[(hub[h], "-", r)] += 1
+                    assert sorted([int(owner[t])] + [hub[h] for h in co]) == sorted(
+                        int(x) for x in net.react[r, : net.n_react[r]])
+                elif s < 13:
+                    ent[(hub[s - 10], "+", r)] += nu
+                    assert net.n_react[r] == 1
+                else:
+                    h, j = divmod(s - 13, 2)
+                    other = [x for x in range(3) if x != h][j]
+                    ent[(hub[h], "+", r)] += nu
+                    assert sorted(int(x) for x in net.react[r, :2]) == sorted([int(owner[t]), hub[other]])
+    return ent, info
+
+
+@pytest.mark.parametrize("name", ["hub150", "hub365", "hub150+perm"])
+def test_pull_schedule_round_trip(name):
+    net = network("hub150").permuted(7)[0] if name.endswith("+perm") else network(name)
+    kn = K.Net(net, host_only=True)
+    got, info = pull_entries(net, kn)
+    assert got == expected_entries(net)
+    assert info["kernel"] == 1 and info["pull_hubs"] == 3
+    assert info["pull_wavefronts"] >= info["pull_wavefronts_ideal"] > 0
+
+
+def test_pull_schedule_small_and_unsupported_networks(g16):
+    # no hubs, one non-hub reactant per reaction: qualifies with zero hubs
+    net = make_toy([1, 1, 1], [((0,), (1,)), ((1,), (0,)), ((1,), (2,))], [2.0, 3.0, 0.5])
+    kn = K.Net(net, host_only=True)
+    got, info = pull_entries(net, kn)
+    assert got == expected_entries(net) and info["pull_hubs"] == 0 and info["kernel"] == 1
+    # two non-hub reactants: generic flux-array kernel
+    info = K.Net(g16, host_only=True).schedule_info()
+    assert info["pull_ok"] == 0 and info["kernel"] == 0
+    with pytest.raises(K.KinnetError):
+        K.Net(g16, host_only=True).schedule_table("pull_owner")
+    # kernel = 1 forces the generic kernel even when the network qualifies
+    info = K.Net(network("hub150"), K.NetParams(kernel=1), host_only=True).schedule_info()
+    assert info["pull_ok"] == 1 and info["kernel"] == 0

@@ -241,6 +241,19 @@ def test_config5_large_network_sampled():
     print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, net.A, "config5"))
 
 
+def test_generic_kernel_on_a_pull_network(hub150):
+    """params.kernel = 1 keeps the flux-array kernel (the fallback of networks
+    that do not qualify for the pull kernel) on a network the pull kernel
+    normally takes: both must meet the same parity."""
+    c = build_config(3, zones=24)
+    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    for kernel in (0, 1):
+        kn = K.Net(hub150, K.NetParams(kernel=kernel))
+        assert kn.schedule_info()["kernel"] == 1 - kernel
+        g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+        print(kernel, check_adaptive(g, ref, delta, dsteps, hub150.A, f"kernel={kernel}", min_well=0.5))
+
+
 # -------------------------------------------------------------- edge cases
 def test_gpu_single_decay_closed_forms():
     """The paper-fixed closed forms directly on the GPU path (pins P2)."""
