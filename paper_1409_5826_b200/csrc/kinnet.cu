@@ -332,7 +332,7 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
 constexpr int kJ2C = kinnet::kPullMaxSlots2;
 
 struct KPull {
-    int N, M, T, W, nbs;
+    int N, M, nbs;
     int hub[kinnet::kPullHubs];
     int mode;                 // Mode: kAdaptive, kFixed or kRhs
     const double* coef;       // [8][M] reaction order: a0 + ln p, a1..a6, n_react - 1
@@ -372,34 +372,6 @@ template <typename real> struct Tiny;
 template <> struct Tiny<double> { static __device__ __forceinline__ double v() { return 1e-290; } };
 template <> struct Tiny<float> { static __device__ __forceinline__ float v() { return 1e-30f; } };
 
-// Sum rows 0..7 of acc over the warp; on return lane l holds the warp total of
-// row (l >> 2) & 7.  Fixed order: deterministic.
-template <typename real>
-__device__ __forceinline__ real warp_sum_rows8(const real (&acc)[8], int lane) {
-    real a[4], b[2], c;
-    const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const real send = up16 ? acc[i] : acc[i + 4];
-        const real keep = up16 ? acc[i + 4] : acc[i];
-        a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const real send = up8 ? a[i] : a[i + 2];
-        const real keep = up8 ? a[i + 2] : a[i];
-        b[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-    }
-    {
-        const real send = up4 ? b[0] : b[1];
-        const real keep = up4 ? b[1] : b[0];
-        c = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    }
-    c += __shfl_xor_sync(0xffffffffu, c, 2);
-    c += __shfl_xor_sync(0xffffffffu, c, 1);
-    return c;
-}
-
 // Field extraction from the packed offset words.  volatile: the words are loop
 // invariant, and without it the compiler hoists every unpacked field out of the
 // sub-step loop into its own register (and then spills).
@@ -424,27 +396,81 @@ __host__ __device__ inline size_t pull_smem_bytes(int T, int W, int M) {
            sizeof(double) * static_cast<size_t>(M);
 }
 
-// dt candidate of one species: eps max(y, floor) / |F+ - F-|   (reading Q7)
+// dt candidate of one species: eps max(y, floor) / |F+ - F-|   (reading Q7).
+// Branch-free: the reciprocal is always formed, of 1 when the change is (near) zero.
 template <typename real>
 __device__ __forceinline__ double dt_candidate(real y, real a, real eps_y, real y_floor) {
     a = a < 0 ? -a : a;
-    if (a > Tiny<real>::v())
-        return static_cast<double>(eps_y * (y > y_floor ? y : y_floor) * rcp_pos(a));
-    return INFINITY;
+    const bool moves = a > Tiny<real>::v();
+    const real c = eps_y * (y > y_floor ? y : y_floor) * rcp_pos(moves ? a : static_cast<real>(1));
+    return moves ? static_cast<double>(c) : static_cast<double>(INFINITY);
 }
 
-template <typename real, int TB, int MINB, int CP>
+// Sum rows 0..5 of v over the warp (rows 0..2 = F+ shares of the hubs, 3..5 = F-
+// shares).  On return the lanes 0, 8, 4, 16, 24, 20 hold the totals of rows
+// 0, 1, 2, 3, 4, 5.  Fixed order: deterministic.  14 shuffles of 4-byte halves
+// per 8-byte value instead of 60 for six plain butterflies.
+template <typename real>
+__device__ __forceinline__ real warp_sum_rows6(const real (&v)[6], int lane) {
+    const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
+    real a[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const real send = up16 ? v[i] : v[i + 3];
+        const real keep = up16 ? v[i + 3] : v[i];
+        a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+    real b0, b1;
+    {
+        const real send = up8 ? a[0] : a[1];
+        const real keep = up8 ? a[1] : a[0];
+        b0 = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        b1 = a[2] + __shfl_xor_sync(0xffffffffu, a[2], 8);
+    }
+    real c;
+    {
+        const real send = up4 ? b0 : b1;
+        const real keep = up4 ? b1 : b0;
+        c = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    c += __shfl_xor_sync(0xffffffffu, c, 2);
+    c += __shfl_xor_sync(0xffffffffu, c, 1);
+    return c;
+}
+
+// Explicit asymptotic / forward Euler update of one species from F+ and k = F-/y
+// (Eq. (3); y = 0 takes the Euler branch, reading Q8).
+// Branch-free: both candidates are formed, 1 + k dt >= 1 is always a safe divisor.
+template <typename real>
+__device__ __forceinline__ real update_k(real y, real Fp, real k, real h, real kappa) {
+    const real kh = k * h;
+    const real ya = fma(h, Fp, y) * rcp_pos(static_cast<real>(1) + kh);
+    const real ye = fma(h, Fp - k * y, y);
+    return (y > 0 && kh >= kappa) ? ya : ye;
+}
+
+// Same update from F+ and F- (hub species): Eq. (3) as Y (Y + dt F+) / (Y + dt F-).
+template <typename real>
+__device__ __forceinline__ real update_fm(real y, real Fp, real Fm, real h, real kappa) {
+    const real hFm = h * Fm;
+    const bool pos = y > Tiny<real>::v();
+    const real ya = fma(h, Fp, y) * (y * rcp_pos(pos ? y + hFm : static_cast<real>(1)));
+    const real ye = fma(h, Fp - Fm, y);
+    return (pos && hFm >= kappa * y) ? ya : ye;
+}
+
+template <typename real, int TB, int MINB, int CP, bool ADAPT>
 __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     static_assert(CP % 4 == 0 && CP <= kinnet::kPullMaxSlots, "slot capacity");
+    constexpr int T = TB, NW = TB / 32;  // the schedule is built for exactly TB threads
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int T = p.T, N = p.N, W = p.W, M = p.M, nbs = p.nbs;
+    const int N = p.N, M = p.M, nbs = p.nbs;
     const int z = blockIdx.x;
-    const int mode = p.mode;
 
     double* redmin = reinterpret_cast<double*>(smem_raw);        // [32] per-warp dt minima
-    real* red = reinterpret_cast<real*>(redmin + 32);            // [W][8] per-warp hub-row sums
-    real* YP = red + W * 8;                                      // [4][T] published products, then 1
+    real* red = reinterpret_cast<real*>(redmin + 32);            // [NW][8] per-warp hub-row sums
+    real* YP = red + NW * 8;                                     // [4][T] published products, then 1
     double* Rbuf = reinterpret_cast<double*>(YP + 4 * T + 4);    // [M] rates, used during set-up only
     const unsigned char* YPb = reinterpret_cast<const unsigned char*>(YP);
 
@@ -454,10 +480,10 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     for (int e = 0; e < CP / 2; ++e) f1[e] = p.f1_pack[e * T + tid];
 #pragma unroll
     for (int e = 0; e < kJ2C / 2; ++e) f2[e] = p.f2_pack[e * T + tid];
-    int npair, wn2;
+    int wn, wn2;
     {
         const uint32_t cnt = p.cnt[tid];
-        npair = (__reduce_max_sync(0xffffffffu, cnt & 255u) + 1) >> 1;  // warp-wide trip count
+        wn = __reduce_max_sync(0xffffffffu, cnt & 255u);  // warp-wide trip counts
         wn2 = __reduce_max_sync(0xffffffffu, (cnt >> 8) & 255u);
     }
 
@@ -507,6 +533,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
     const int own = p.owner[tid];
     const bool hub_owner = tid < nbs;  // hub h is owned by thread h
+    const bool plain_owner = own >= 0 && !hub_owner;
     real y = (own >= 0) ? Yg[own] : static_cast<real>(0);
     real yh0 = nbs > 0 ? Yg[p.hub[0]] : static_cast<real>(0);
     real yh1 = nbs > 1 ? Yg[p.hub[1]] : static_cast<real>(0);
@@ -516,20 +543,21 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     const real eps_y = static_cast<real>(p.eps_y);
     const real y_floor = static_cast<real>(p.y_floor);
     const double growth = p.growth, t_hydro = p.t_hydro;
+    const bool rhs_only = p.mode == kRhs;
 
     double t = 0.0, dt_prev = 0.0;
     int steps = 0;
     int status = 0;
     bool run = true;
-    if (mode == kAdaptive) {
+    if (ADAPT) {
         const double dt_in = p.dt ? p.dt[z] : 0.0;
         dt_prev = (dt_in > 0.0) ? dt_in : t_hydro;
         run = t_hydro > 0.0;
         if (!run) dt_prev = dt_in;  // nothing to do: the trial dt is returned unchanged
-    } else if (mode == kFixed) {
+    } else if (!rhs_only) {
         run = p.n_fixed > 0;
     }
-    const int max_steps = (mode == kFixed) ? p.n_fixed : p.max_steps;
+    const int max_steps = ADAPT ? p.max_steps : p.n_fixed;
 
     while (run) {
         // ---- publish y x {1, hubs} ------------------------------------------------
@@ -539,7 +567,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         YP[3 * T + tid] = y * yh2;
 
         // ---- rate sums: k = F-/y (Eq. (1)) and this thread's share of the hub rows ---
-        real k, acc[8];
+        real k, share[6];
         {
             real e0 = fma(K00, yh0, K1);
             e0 = fma(K01, yh1, e0);
@@ -560,11 +588,9 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             m0 *= yh0;
             m1 *= yh1;
             m2 *= yh2;
-            if (hub_owner) {  // the owner's own consumption of a hub-only reaction
-                if (tid == 0) m0 += k;
-                if (tid == 1) m1 += k;
-                if (tid == 2) m2 += k;
-            }
+            if (tid == 0) m0 += k;  // the owner's own consumption in a hub-only reaction
+            if (tid == 1) m1 += k;
+            if (tid == 2) m2 += k;
             // F+_hub share / y
             real g0 = fma(C[13], yh1, C[10]);
             g0 = fma(C[14], yh2, g0);
@@ -572,83 +598,80 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             g1 = fma(C[16], yh2, g1);
             real g2 = fma(C[17], yh0, C[12]);
             g2 = fma(C[18], yh1, g2);
-            acc[0] = y * g0;
-            acc[1] = y * g1;
-            acc[2] = y * g2;
-            acc[3] = y * m0;
-            acc[4] = y * m1;
-            acc[5] = y * m2;
-            acc[6] = 0;
-            acc[7] = 0;
+            share[0] = y * g0;
+            share[1] = y * g1;
+            share[2] = y * g2;
+            share[3] = y * m0;
+            share[4] = y * m1;
+            share[5] = y * m2;
         }
         __syncthreads();
 
-        // ---- S2+S3: F+ = sum of the incoming fluxes, each evaluated here ---------------
+        // ---- hub rows: warp totals of the six shares ---------------------------------------
+        if (nbs > 0) {
+            const real tot = warp_sum_rows6(share, lane);
+            const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
+            if ((lane & 3) == 0 && (lane & 12) != 12) red[warp * 8 + row] = tot;
+        }
+
+        // ---- S2+S3: F+ = sum of the incoming fluxes, each evaluated here -----------------
         real Fp;
         {
             real s0 = 0, s1 = 0, s2 = 0, s3 = 0;
-#define PULL_PAIR(I, SA, SB)                                        \
-    if constexpr (2 * (I) < CP) {                                   \
-        const uint32_t w_ = f1[I];                                  \
-        real a_ = lds_at<real>(YPb, lo16(w_));                      \
-        real b_ = lds_at<real>(YPb, hi16(w_));                      \
-        if constexpr (2 * (I) < kJ2C) {                             \
-            if (2 * (I) < wn2) {                                    \
-                const uint32_t v_ = f2[I];                          \
-                a_ *= lds_at<real>(YPb, lo16(v_));                  \
-                b_ *= lds_at<real>(YPb, hi16(v_));                  \
-            }                                                       \
-        }                                                           \
-        SA = fma(R[2 * (I)], a_, SA);                               \
-        SB = fma(R[2 * (I) + 1], b_, SB);                           \
-    }
-            switch (npair) {
-                case 12: PULL_PAIR(11, s2, s3) [[fallthrough]];
-                case 11: PULL_PAIR(10, s0, s1) [[fallthrough]];
-                case 10: PULL_PAIR(9, s2, s3) [[fallthrough]];
-                case 9: PULL_PAIR(8, s0, s1) [[fallthrough]];
-                case 8: PULL_PAIR(7, s2, s3) [[fallthrough]];
-                case 7: PULL_PAIR(6, s0, s1) [[fallthrough]];
-                case 6: PULL_PAIR(5, s2, s3) [[fallthrough]];
-                case 5: PULL_PAIR(4, s0, s1) [[fallthrough]];
-                case 4: PULL_PAIR(3, s2, s3) [[fallthrough]];
-                case 3: PULL_PAIR(2, s0, s1) [[fallthrough]];
-                case 2: PULL_PAIR(1, s2, s3) [[fallthrough]];
-                case 1: PULL_PAIR(0, s0, s1) [[fallthrough]];
-                default: break;
+#pragma unroll
+            for (int g = 0; g < CP / 4; ++g) {
+                if (4 * g < wn) {  // warp-uniform
+                    const uint32_t w0 = f1[2 * g], w1 = f1[2 * g + 1];
+                    real a0 = lds_at<real>(YPb, lo16(w0));
+                    real a1 = lds_at<real>(YPb, hi16(w0));
+                    real a2 = lds_at<real>(YPb, lo16(w1));
+                    real a3 = lds_at<real>(YPb, hi16(w1));
+                    if (4 * g < kJ2C) {
+                        if (4 * g < wn2) {  // second factors (three-body reactions)
+                            const uint32_t v0 = f2[(2 * g) % (kJ2C / 2)],
+                                           v1 = f2[(2 * g + 1) % (kJ2C / 2)];
+                            a0 *= lds_at<real>(YPb, lo16(v0));
+                            a1 *= lds_at<real>(YPb, hi16(v0));
+                            a2 *= lds_at<real>(YPb, lo16(v1));
+                            a3 *= lds_at<real>(YPb, hi16(v1));
+                        }
+                    }
+                    s0 = fma(R[4 * g], a0, s0);
+                    s1 = fma(R[4 * g + 1], a1, s1);
+                    s2 = fma(R[4 * g + 2], a2, s2);
+                    s3 = fma(R[4 * g + 3], a3, s3);
+                }
             }
-#undef PULL_PAIR
             Fp = (s0 + s1) + (s2 + s3);
         }
 
         // ---- S5: dt candidates of the non-hub species ------------------------------------
-        if (mode == kAdaptive) {
-            double c = INFINITY;
-            if (own >= 0 && !hub_owner) c = dt_candidate(y, Fp - k * y, eps_y, y_floor);
+        if (ADAPT) {
+            double c = dt_candidate(y, Fp - k * y, eps_y, y_floor);
+            if (!plain_owner) c = INFINITY;
             c = warp_min_pos(c);
             if (lane == 0) redmin[warp] = c;
-        }
-        // ---- hub rows: warp totals of the six partial sums ---------------------------------
-        if (nbs > 0) {
-            const real tot = warp_sum_rows8(acc, lane);
-            if ((lane & 3) == 0) red[warp * 8 + (lane >> 2)] = tot;
         }
         __syncthreads();
 
         // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
         real hFp = 0, hFm = 0;
         const real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
-        double cand = INFINITY;
-        if (lane < nbs) {
-            for (int w = 0; w < W; ++w) {  // fixed order over warps
-                hFp += red[w * 8 + lane];
-                hFm += red[w * 8 + 3 + lane];
+        if (nbs > 0) {
+            const int l3 = lane < 3 ? lane : 0;
+            real vp[NW], vm[NW];
+#pragma unroll
+            for (int w = 0; w < NW; ++w) {
+                vp[w] = red[w * 8 + l3];
+                vm[w] = red[w * 8 + 3 + l3];
             }
-            if (mode == kAdaptive) cand = dt_candidate(yme, hFp - hFm, eps_y, y_floor);
-        } else if (mode == kAdaptive && lane >= 8 && lane < 8 + W) {
-            cand = redmin[lane - 8];
+#pragma unroll
+            for (int w = 0; w < NW; ++w) {  // fixed order over warps
+                hFp += vp[w];
+                hFm += vm[w];
+            }
         }
-        if (mode == kRhs) {
+        if (!ADAPT && rhs_only) {
             real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
             real* Fmo = reinterpret_cast<real*>(p.Fminus) + (size_t)z * N;
             if (hub_owner) {
@@ -663,18 +686,17 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
 
         double dts;
         bool last;
-        if (mode == kAdaptive) {
+        if (ADAPT) {
+            double cand = INFINITY;
+            if (lane >= 8 && lane < 8 + NW) cand = redmin[lane - 8];
+            const double hc = dt_candidate(yme, hFp - hFm, eps_y, y_floor);
+            if (lane < nbs) cand = hc;
             const double cmin = warp_min_pos(cand);
             double dt_ctrl = growth * dt_prev;
             if (cmin < dt_ctrl) dt_ctrl = cmin;
             const double rem = t_hydro - t;
-            if (dt_ctrl >= rem * (1.0 - 1e-12)) {
-                dts = rem;
-                last = true;
-            } else {
-                dts = dt_ctrl;
-                last = false;
-            }
+            last = dt_ctrl >= rem * (1.0 - 1e-12);
+            dts = last ? rem : dt_ctrl;
             dt_prev = dt_ctrl;
         } else {
             dts = p.dt_fixed;
@@ -683,35 +705,18 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         const real h = static_cast<real>(dts);
 
         // ---- S4: update (Eq. (3)) -------------------------------------------
+        const real yn = update_k(y, Fp, k, h, kappa);
         if (nbs > 0) {  // hub species, on lanes 0..nbs-1 of every warp, from F+ and F-
-            real yn = yme;
-            const real hFmh = h * hFm;
-            if (yme > 0 && hFmh >= kappa * yme) {  // k dt >= kappa with k = F-/Y
-                const real den = yme + hFmh;        // Eq. (3) as Y (Y + dt F+) / (Y + dt F-)
-                if (den > Tiny<real>::v() && yme > Tiny<real>::v())
-                    yn = (yme + h * hFp) * (yme * rcp_pos(den));
-                else
-                    yn = (yme + h * hFp) / (static_cast<real>(1) + (hFm / yme) * h);
-            } else {
-                yn = yme + h * (hFp - hFm);
-            }
-            yh0 = __shfl_sync(0xffffffffu, yn, 0);
-            if (nbs > 1) yh1 = __shfl_sync(0xffffffffu, yn, 1);
-            if (nbs > 2) yh2 = __shfl_sync(0xffffffffu, yn, 2);
+            const real hn = update_fm(yme, hFp, hFm, h, kappa);
+            yh0 = __shfl_sync(0xffffffffu, hn, 0);
+            if (nbs > 1) yh1 = __shfl_sync(0xffffffffu, hn, 1);
+            if (nbs > 2) yh2 = __shfl_sync(0xffffffffu, hn, 2);
         }
-        if (hub_owner) {
-            y = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
-        } else {  // own species from F+ and k
-            const real kh = k * h;
-            if (y > 0 && kh >= kappa)
-                y = (y + h * Fp) * rcp_pos(static_cast<real>(1) + kh);
-            else
-                y = y + h * (Fp - k * y);
-        }
+        y = hub_owner ? (tid == 0 ? yh0 : (tid == 1 ? yh1 : yh2)) : yn;
         t = last ? t_hydro : t + dts;
         ++steps;
         if (last) run = false;
-        else if (mode == kAdaptive && steps >= max_steps) {
+        else if (ADAPT && steps >= max_steps) {
             status |= NET_STATUS_MAX_STEPS;
             run = false;
         }
@@ -722,7 +727,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
     if (own >= 0) Yg[own] = y;
     if (tid == 0) {
-        if (mode == kAdaptive && p.dt) p.dt[z] = dt_prev;
+        if (ADAPT && p.dt) p.dt[z] = dt_prev;
         if (p.n_steps) p.n_steps[z] = steps;
         if (p.status) p.status[z] = status;
     }
@@ -790,30 +795,37 @@ kernel_fn pick_block(int T) {
 // (65536 / (TB * MINB) registers per thread) x P-slot capacity classes
 typedef void (*pull_fn)(const KPull);
 
-template <typename real, int CP>
+template <typename real, int CP, bool ADAPT>
 pull_fn pick_pull_block(int T) {
-    if (T <= 64) return zone_kernel_pull<real, 64, 8, CP>;
-    if (T <= 160) {
-        const char* e = std::getenv("KINNET_PULL_MINB");  // tuning knob while measuring residency
-        if (e && e[0] == '2') return zone_kernel_pull<real, 160, 2, CP>;
-        return zone_kernel_pull<real, 160, 3, CP>;
+    switch (T) {
+        case 32: return zone_kernel_pull<real, 32, 12, CP, ADAPT>;
+        case 64: return zone_kernel_pull<real, 64, 6, CP, ADAPT>;
+        case 160: {
+            const char* e = std::getenv("KINNET_PULL_MINB");  // tuning knob while measuring residency
+            if (e && e[0] == '2') return zone_kernel_pull<real, 160, 2, CP, ADAPT>;
+            return zone_kernel_pull<real, 160, 3, CP, ADAPT>;
+        }
+        case 256: return zone_kernel_pull<real, 256, 2, CP, ADAPT>;
+        case 384: return zone_kernel_pull<real, 384, 1, CP, ADAPT>;
+        default: return zone_kernel_pull<real, 512, 1, CP, ADAPT>;
     }
-    if (T <= 256) return zone_kernel_pull<real, 256, 2, CP>;
-    if (T <= 384) return zone_kernel_pull<real, 384, 1, CP>;
-    return zone_kernel_pull<real, 512, 1, CP>;
 }
 
-template <typename real>
+template <typename real, bool ADAPT>
 pull_fn pick_pull_real(const kinnet::PullSchedule& P) {
-    if (P.slots <= 12) return pick_pull_block<real, 12>(P.T);
-    if (P.slots <= 20) return pick_pull_block<real, 20>(P.T);
-    return pick_pull_block<real, 24>(P.T);
+    if (P.slots <= 12) return pick_pull_block<real, 12, ADAPT>(P.T);
+    if (P.slots <= 20) return pick_pull_block<real, 20, ADAPT>(P.T);
+    return pick_pull_block<real, 24, ADAPT>(P.T);
 }
 
 bool use_pull_kernel(const net* n) { return n->PS.ok && !n->force_generic; }
 
-pull_fn pick_pull(const net* n) {
-    return n->P.precision == 32 ? pick_pull_real<float>(n->PS) : pick_pull_real<double>(n->PS);
+pull_fn pick_pull(const net* n, bool adaptive) {
+    if (adaptive)
+        return n->P.precision == 32 ? pick_pull_real<float, true>(n->PS)
+                                    : pick_pull_real<double, true>(n->PS);
+    return n->P.precision == 32 ? pick_pull_real<float, false>(n->PS)
+                                : pick_pull_real<double, false>(n->PS);
 }
 
 size_t pull_smem(const net* n) {
@@ -844,8 +856,11 @@ int prepare_kernels(net* n) {
     }
     int nb = 0;
     if (use_pull_kernel(n)) {
-        const void* f = reinterpret_cast<const void*>(pick_pull(n));
+        const void* f = reinterpret_cast<const void*>(pick_pull(n, true));
+        const void* f2 = reinterpret_cast<const void*>(pick_pull(n, false));
         CUDA_TRY(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      static_cast<int>(pull_smem(n))));
+        CUDA_TRY(cudaFuncSetAttribute(f2, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       static_cast<int>(pull_smem(n))));
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, n->PS.T, pull_smem(n)));
     } else {
@@ -859,7 +874,7 @@ int prepare_kernels(net* n) {
 void fill_pull(const net* n, KPull& k) {
     const kinnet::PullSchedule& P = n->PS;
     std::memset(&k, 0, sizeof(k));
-    k.N = n->S.N; k.M = n->S.M; k.T = P.T; k.W = P.W; k.nbs = P.nbs;
+    k.N = n->S.N; k.M = n->S.M; k.nbs = P.nbs;
     for (int h = 0; h < kinnet::kPullHubs; ++h) k.hub[h] = P.hub[h];
     k.coef = n->D.coef_rxn;
     k.owner = n->D.p_owner;
@@ -874,7 +889,7 @@ void fill_pull(const net* n, KPull& k) {
 }
 
 int launch_pull(net* n, int zones, KPull& k, void* stream) {
-    pull_fn f = pick_pull(n);
+    pull_fn f = pick_pull(n, k.mode == kAdaptive);
     f<<<zones, n->PS.T, pull_smem(n), static_cast<cudaStream_t>(stream)>>>(k);
     CUDA_TRY(cudaGetLastError());
     return NET_OK;

@@ -308,10 +308,13 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         P.ok = false;
         P.why = why;
     };
-    const int T = std::max(32, (N + 31) / 32 * 32);
+    // the kernel is instantiated for these block sizes and runs exactly T threads
+    int T = 0;
+    for (int cls : {32, 64, 160, 256, 384, 512})
+        if (T == 0 && N <= cls) T = cls;
+    if (T == 0) return reject("more than 512 species");
     P.T = T;
     P.W = T / 32;
-    if (T > 512) return reject("more than 512 species");
     if (M > 65535) return reject("more than 65535 reactions");
 
     // ---- hubs: the rows with hundreds of terms ------------------
