@@ -272,37 +272,135 @@ int build_schedule(int N, const int* A, int M, const int* n_react, const int* re
 
 namespace {
 
-// Shared-memory wavefronts of the P-slot gathers for 8-byte words: a warp's LDS.64
-// is served as two half-warps; within one, lanes that read different words of the
-// same bank pair (word index mod 16) are serialised, equal words are broadcast.
-void pull_wavefronts(const PullSchedule& P, long& actual, long& ideal) {
+// Shared-memory wavefronts of the P-slot gathers.  One wavefront serves 128 bytes:
+// a warp's LDS.64 goes out as two half-warps, an LDS.32 as one piece.  Within a
+// piece, lanes that read different words of the same bank (word index modulo the
+// piece size) are serialised; equal words are broadcast.
+int piece_wavefronts(const uint16_t* words, int lanes) {
+    int worst = 1;
+    for (int b = 0; b < lanes; ++b) {
+        int distinct = 0;
+        uint16_t seen[32];
+        for (int l = 0; l < lanes; ++l) {
+            const uint16_t w = words[l];
+            if (w % lanes != b) continue;
+            bool dup = false;
+            for (int q = 0; q < distinct; ++q) dup = dup || seen[q] == w;
+            if (!dup) seen[distinct++] = w;
+        }
+        worst = std::max(worst, distinct);
+    }
+    return worst;
+}
+
+void pull_wavefronts(const PullSchedule& P, int elem_bytes, long& actual, long& ideal) {
     actual = ideal = 0;
-    const int T = P.T;
+    const int T = P.T, lanes = 128 / elem_bytes;
     for (int w = 0; w < P.W; ++w) {
         int wmax = 0;
         for (int l = 0; l < 32; ++l) wmax = std::max<int>(wmax, P.n_slots[w * 32 + l]);
         for (int e = 0; e < wmax; ++e)
-            for (int half = 0; half < 2; ++half) {
-                int worst = 0;
-                for (int b = 0; b < 16; ++b) {
-                    std::vector<int> words;
-                    for (int l = 0; l < 16; ++l) {
-                        const int word = P.slot_f1[static_cast<size_t>(e) * T + w * 32 + half * 16 + l];
-                        if (word % 16 == b && std::find(words.begin(), words.end(), word) == words.end())
-                            words.push_back(word);
-                    }
-                    worst = std::max<int>(worst, words.size());
-                }
-                actual += worst;
+            for (int piece = 0; piece < 32 / lanes; ++piece) {
+                uint16_t words[32];
+                for (int l = 0; l < lanes; ++l)
+                    words[l] = P.slot_f1[static_cast<size_t>(e) * T + w * 32 + piece * lanes + l];
+                actual += piece_wavefronts(words, lanes);
                 ideal += 1;
             }
+    }
+}
+
+// Order the P-slots of every thread so that the lanes served by one wavefront
+// read different banks at every position ("memory accesses
+// are not yet optimized" is what the paper blames for the cost of the sums).
+// The order of a thread's slots is free -- it only fixes the order of its F+ sum
+// -- so this is an edge colouring of the bipartite multigraph lanes x banks of
+// each piece; a min-conflicts search from a greedy start gets within a few
+// wavefronts of the bound max(slots of a lane, slots on a bank).
+//   pos[t][p]   slot index of thread t at position p, -1 = hole
+//   cap         positions available to the warp (multiple of 4, the kernel's group size)
+//   cap2        positions that may hold a slot with a second factor
+struct Placement {
+    std::vector<std::vector<int>> pos;
+};
+
+template <typename SlotT>
+void place_piece(const std::vector<std::vector<SlotT>>& slots, int t0, int lanes, int cap, int cap2,
+                 std::vector<std::vector<int>>& pos) {
+    // cnt[p][b] = lanes of the piece reading bank b at position p
+    std::vector<std::vector<int>> cnt(cap, std::vector<int>(lanes, 0));
+    auto bank = [&](int t, int s) { return slots[t][s].f1 % lanes; };
+    auto cost_at = [&](int p) {
+        int worst = 1;
+        for (int b = 0; b < lanes; ++b) worst = std::max(worst, cnt[p][b]);
+        return worst;
+    };
+    for (int l = 0; l < lanes; ++l) pos[t0 + l].assign(cap, -1);
+    // greedy start: two-factor slots first (fewer legal positions), busiest banks first
+    std::vector<int> bank_deg(lanes, 0);
+    for (int l = 0; l < lanes; ++l)
+        for (size_t s = 0; s < slots[t0 + l].size(); ++s) ++bank_deg[bank(t0 + l, s)];
+    struct Item { int t, s; };
+    std::vector<Item> items;
+    for (int l = 0; l < lanes; ++l)
+        for (size_t s = 0; s < slots[t0 + l].size(); ++s) items.push_back({t0 + l, static_cast<int>(s)});
+    std::stable_sort(items.begin(), items.end(), [&](const Item& a, const Item& b) {
+        const bool ta = slots[a.t][a.s].two, tb = slots[b.t][b.s].two;
+        if (ta != tb) return ta;
+        return bank_deg[bank(a.t, a.s)] > bank_deg[bank(b.t, b.s)];
+    });
+    for (const Item& it : items) {
+        const int b = bank(it.t, it.s), lim = slots[it.t][it.s].two ? cap2 : cap;
+        int best = -1, best_cnt = 1 << 30;
+        for (int p = 0; p < lim; ++p)
+            if (pos[it.t][p] < 0 && cnt[p][b] < best_cnt) {
+                best = p;
+                best_cnt = cnt[p][b];
+            }
+        pos[it.t][best] = it.s;
+        ++cnt[best][b];
+    }
+    // min-conflicts: swap two positions of one lane whenever that lowers the wavefront count
+    uint32_t rng = 0x9E3779B9u ^ static_cast<uint32_t>(t0 * 2654435761u);
+    auto next = [&]() { rng = rng * 1664525u + 1013904223u; return rng >> 8; };
+    for (int pass = 0; pass < 400; ++pass) {
+        bool any_conflict = false;
+        for (int p = 0; p < cap; ++p) any_conflict = any_conflict || cost_at(p) > 1;
+        if (!any_conflict) break;
+        for (int l = 0; l < lanes; ++l) {
+            const int t = t0 + l;
+            for (int p = 0; p < cap; ++p) {
+                const int s = pos[t][p];
+                if (s < 0 || cnt[p][bank(t, s)] < 2) continue;  // not in conflict
+                const int q0 = static_cast<int>(next() % cap);
+                for (int dq = 0; dq < cap; ++dq) {
+                    const int q = (q0 + dq) % cap;
+                    if (q == p) continue;
+                    const int s2 = pos[t][q];
+                    if (slots[t][s].two && q >= cap2) continue;
+                    if (s2 >= 0 && slots[t][s2].two && p >= cap2) continue;
+                    const int before = cost_at(p) + cost_at(q);
+                    const int b1 = bank(t, s), b2 = s2 >= 0 ? bank(t, s2) : -1;
+                    --cnt[p][b1]; ++cnt[q][b1];
+                    if (s2 >= 0) { --cnt[q][b2]; ++cnt[p][b2]; }
+                    const int after = cost_at(p) + cost_at(q);
+                    // accept improvements, and sideways moves that empty the conflict here
+                    if (after < before || (after == before && cnt[q][b1] == 1 && (next() & 3) == 0)) {
+                        std::swap(pos[t][p], pos[t][q]);
+                        break;
+                    }
+                    ++cnt[p][b1]; --cnt[q][b1];
+                    if (s2 >= 0) { ++cnt[q][b2]; --cnt[p][b2]; }
+                }
+            }
+        }
     }
 }
 
 }  // namespace
 
 void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
-                         const int* prod, PullSchedule& P) {
+                         const int* prod, int elem_bytes, PullSchedule& P) {
     P = PullSchedule();
     auto reject = [&](const std::string& why) {
         P.ok = false;
@@ -402,6 +500,74 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         }
     }
 
+    // ---- balance the banks: swap species between threads of one warp ---------------------
+    // A piece (the lanes one wavefront serves) cannot gather a position in fewer
+    // wavefronts than its busiest bank holds words, so spread every piece's sources
+    // over the banks before the slots are ordered.  Swaps stay inside a warp: its slot
+    // count (the falling in-degree order) is untouched.
+    {
+        const int lanes = 128 / elem_bytes;
+        std::vector<std::vector<int>> srcs(N);  // non-hub species -> owner species of each P-slot
+        for (int r = 0; r < M; ++r)
+            for (int q = 0; q < n_prod[r]; ++q) {
+                const int s = prod[r * kMaxProd + q];
+                bool first = true;
+                for (int u = 0; u < q; ++u) first = first && prod[r * kMaxProd + u] != s;
+                if (first && hub_index[s] < 0) srcs[s].push_back(rx[r].owner);
+            }
+        const int pieces = T / lanes;
+        std::vector<int> cap(pieces, 0);
+        for (int pc = 0; pc < pieces; ++pc) {
+            int most = 0;
+            for (int l = 0; l < 32; ++l) {
+                const int sp = P.owner[(pc * lanes / 32) * 32 + l];
+                if (sp >= 0) most = std::max<int>(most, srcs[sp].size());
+            }
+            cap[pc] = (most + 3) / 4 * 4;
+        }
+        std::vector<int> deg(static_cast<size_t>(pieces) * lanes);
+        auto total_cost = [&]() {
+            std::fill(deg.begin(), deg.end(), 0);
+            for (int t = 0; t < T; ++t) {
+                const int sp = P.owner[t];
+                if (sp < 0) continue;
+                for (int j : srcs[sp]) ++deg[static_cast<size_t>(t / lanes) * lanes + P.thread_of[j] % lanes];
+            }
+            long cost = 0;
+            for (int pc = 0; pc < pieces; ++pc) {
+                int worst = cap[pc];
+                for (int b = 0; b < lanes; ++b) worst = std::max(worst, deg[static_cast<size_t>(pc) * lanes + b]);
+                cost += worst;
+                // second term: sum of squares breaks ties towards flatter banks
+            }
+            return cost;
+        };
+        uint32_t rng = 0x2545F491u;
+        auto next = [&]() { rng = rng * 1664525u + 1013904223u; return rng >> 8; };
+        long cost = total_cost();
+        long floor_cost = 0;
+        for (int pc = 0; pc < pieces; ++pc) floor_cost += cap[pc];
+        for (int it = 0; it < 20000 && cost > floor_cost; ++it) {
+            const int w = static_cast<int>(next() % P.W);
+            const int t1 = w * 32 + static_cast<int>(next() % 32), t2 = w * 32 + static_cast<int>(next() % 32);
+            if (t1 == t2 || t1 < P.nbs || t2 < P.nbs) continue;  // hubs stay on threads 0..2
+            const int s1 = P.owner[t1], s2 = P.owner[t2];
+            if (s1 < 0 && s2 < 0) continue;
+            auto put = [&](int sp, int t) {
+                P.owner[t] = sp;
+                if (sp >= 0) P.thread_of[sp] = t;
+            };
+            put(s1, t2);
+            put(s2, t1);
+            const long c2 = total_cost();
+            if (c2 <= cost) cost = c2;
+            else {
+                put(s1, t1);
+                put(s2, t2);
+            }
+        }
+    }
+
     // ---- P-slots and rate-sum lists ---------------------------------------------------
     struct Slot {
         int32_t rxn;
@@ -410,7 +576,10 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
     };
     std::vector<std::vector<Slot>> slots(T);
     std::vector<std::vector<std::vector<int32_t>>> agg(T, std::vector<std::vector<int32_t>>(kPullCoefs));
+    // the constant one: YP[4T .. 4T+3]; second factors default to the copy in bank 3,
+    // clear of the hub words 0..2 they are gathered next to
     const uint16_t one_word = static_cast<uint16_t>(4 * T);
+    const uint16_t one_word2 = static_cast<uint16_t>(4 * T + 3);
     for (int r = 0; r < M; ++r) {  // reaction order = fixed, documented summation order
         const Rx& x = rx[r];
         const int t_own = P.thread_of[x.owner];
@@ -448,15 +617,10 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
     P.n_slots2.assign(T, 0);
     P.agg_max = 0;
     for (int t = 0; t < T; ++t) {
-        std::stable_sort(slots[t].begin(), slots[t].end(),
-                         [](const Slot& a, const Slot& b) { return a.two > b.two; });
         int n2 = 0;
         for (const Slot& sl : slots[t]) n2 += sl.two;
         P.slots = std::max<int>(P.slots, slots[t].size());
         P.slots2 = std::max(P.slots2, n2);
-        if (slots[t].size() > 255) return reject("too many incoming reactions for one species");
-        P.n_slots[t] = static_cast<uint8_t>(slots[t].size());
-        P.n_slots2[t] = static_cast<uint8_t>(n2);
         int tot = 0;
         for (const auto& v : agg[t]) tot += static_cast<int>(v.size());
         P.agg_max = std::max(P.agg_max, tot);
@@ -468,26 +632,71 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         return reject("a non-hub species has more than " + std::to_string(kPullMaxSlots2) +
                       " incoming three-body reactions");
     if (P.agg_max > 65535) return reject("rate-sum list too long");
+
+    // ---- positions: bank-conflict-aware order of every thread's slots ------------------
+    const int lanes = 128 / elem_bytes;
+    std::vector<std::vector<int>> pos(T);
+    std::vector<int> warp_cap(P.W, 0);
+    for (int w = 0; w < P.W; ++w) {
+        int most = 0, most2 = 0;
+        for (int l = 0; l < 32; ++l) {
+            int n2 = 0;
+            for (const Slot& sl : slots[w * 32 + l]) n2 += sl.two;
+            most = std::max<int>(most, slots[w * 32 + l].size());
+            most2 = std::max(most2, n2);
+        }
+        const int cap = (most + 3) / 4 * 4, cap2 = std::min(cap, (most2 + 3) / 4 * 4);
+        warp_cap[w] = cap;
+        for (int piece = 0; piece < 32 / lanes; ++piece)
+            place_piece(slots, w * 32 + piece * lanes, lanes, cap, cap2, pos);
+    }
+    P.slots = P.slots2 = 0;
+    for (int t = 0; t < T; ++t)
+        for (int p = 0; p < static_cast<int>(pos[t].size()); ++p) {
+            if (pos[t][p] < 0) continue;
+            P.n_slots[t] = static_cast<uint8_t>(p + 1);
+            if (slots[t][pos[t][p]].two) P.n_slots2[t] = static_cast<uint8_t>(p + 1);
+        }
+    for (int t = 0; t < T; ++t) {
+        P.slots = std::max<int>(P.slots, P.n_slots[t]);
+        P.slots2 = std::max<int>(P.slots2, P.n_slots2[t]);
+    }
     const int ns = std::max(1, P.slots), ns2 = std::max(1, P.slots2);
     P.slot_rxn.assign(static_cast<size_t>(ns) * T, -1);
     P.slot_f1.assign(static_cast<size_t>(ns) * T, one_word);
-    P.slot_f2.assign(static_cast<size_t>(ns2) * T, one_word);
+    P.slot_f2.assign(static_cast<size_t>(ns2) * T, one_word2);
     P.agg_ptr.assign(static_cast<size_t>(kPullCoefs + 1) * T, 0);
     P.agg_ent.assign(static_cast<size_t>(std::max(1, P.agg_max)) * T, 0);
     for (int t = 0; t < T; ++t) {
-        for (size_t e = 0; e < slots[t].size(); ++e) {
-            P.slot_rxn[e * T + t] = slots[t][e].rxn;
-            P.slot_f1[e * T + t] = slots[t][e].f1;
-            if (slots[t][e].two) P.slot_f2[e * T + t] = slots[t][e].f2;
+        for (int p = 0; p < static_cast<int>(pos[t].size()) && p < ns; ++p) {
+            const int sidx = pos[t][p];
+            if (sidx < 0) continue;
+            const Slot& sl = slots[t][sidx];
+            P.slot_rxn[static_cast<size_t>(p) * T + t] = sl.rxn;
+            P.slot_f1[static_cast<size_t>(p) * T + t] = sl.f1;
+            if (sl.two) P.slot_f2[static_cast<size_t>(p) * T + t] = sl.f2;
         }
-        int pos = 0;
+        int q = 0;
         for (int c = 0; c < kPullCoefs; ++c) {
-            P.agg_ptr[static_cast<size_t>(c) * T + t] = static_cast<uint16_t>(pos);
-            for (int32_t v : agg[t][c]) P.agg_ent[static_cast<size_t>(pos++) * T + t] = v;
+            P.agg_ptr[static_cast<size_t>(c) * T + t] = static_cast<uint16_t>(q);
+            for (int32_t v : agg[t][c]) P.agg_ent[static_cast<size_t>(q++) * T + t] = v;
         }
-        P.agg_ptr[static_cast<size_t>(kPullCoefs) * T + t] = static_cast<uint16_t>(pos);
+        P.agg_ptr[static_cast<size_t>(kPullCoefs) * T + t] = static_cast<uint16_t>(q);
     }
-    pull_wavefronts(P, P.conflict_wavefronts, P.ideal_wavefronts);
+    // holes (rate 0): read a word some lane of the same piece reads at that position
+    // anyway, so that the hole costs no wavefront of its own
+    for (int t0 = 0; t0 < T; t0 += lanes)
+        for (int p = 0; p < ns; ++p) {
+            int donor = -1;
+            for (int l = 0; l < lanes && donor < 0; ++l)
+                if (P.slot_rxn[static_cast<size_t>(p) * T + t0 + l] >= 0) donor = t0 + l;
+            if (donor < 0) continue;
+            for (int l = 0; l < lanes; ++l)
+                if (P.slot_rxn[static_cast<size_t>(p) * T + t0 + l] < 0)
+                    P.slot_f1[static_cast<size_t>(p) * T + t0 + l] =
+                        P.slot_f1[static_cast<size_t>(p) * T + donor];
+        }
+    pull_wavefronts(P, elem_bytes, P.conflict_wavefronts, P.ideal_wavefronts);
     P.ok = true;
 }
 

@@ -95,11 +95,11 @@ struct PullSchedule {
     std::vector<int32_t> thread_of;    // [N]
     int slots = 0;                     // max P-slots of any thread
     int slots2 = 0;                    // max P-slots with a second factor of any thread
-    std::vector<uint8_t> n_slots;      // [T]
-    std::vector<uint8_t> n_slots2;     // [T]  slots [0, n_slots2) have the second factor
-    std::vector<int32_t> slot_rxn;     // [slots][T] reaction | nu << 24, -1 = empty
+    std::vector<uint8_t> n_slots;      // [T]  1 + last used position (positions may have holes)
+    std::vector<uint8_t> n_slots2;     // [T]  1 + last position whose slot has a second factor
+    std::vector<int32_t> slot_rxn;     // [slots][T] reaction | nu << 24, -1 = hole
     std::vector<uint16_t> slot_f1;     // [slots][T] YP word index c*T + t of the first factor
-    std::vector<uint16_t> slot_f2;     // [slots2][T] YP word index of the second factor (4T = one)
+    std::vector<uint16_t> slot_f2;     // [slots2][T] YP word index of the second factor (4T+3 = one)
     // rate sums: coefficient s of thread t = sum of nu * R over agg_ent[agg_ptr[s][t] .. agg_ptr[s+1][t])
     int agg_max = 0;
     std::vector<uint16_t> agg_ptr;     // [kPullCoefs + 1][T]
@@ -112,7 +112,8 @@ struct PullSchedule {
 //   0..9   K_c   c = 0: {}, 1..3: {hub c-1}, 4..9: {0,0},{0,1},{0,2},{1,1},{1,2},{2,2}
 //   10..12 G0_h  reactions of this thread with hub h as a product and no hub co-reactant
 //   13..18 Gx_h,j  hub h as a product, one hub co-reactant: the j-th of the other two hubs
+// elem_bytes = size of one abundance (8 or 4): it fixes the shared-memory bank of a word.
 void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
-                         const int* prod, PullSchedule& out);
+                         const int* prod, int elem_bytes, PullSchedule& out);
 
 }  // namespace kinnet

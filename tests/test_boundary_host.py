@@ -193,20 +193,19 @@ def pull_entries(net, kn):
     for t in range(T):
         assert ns2[t] <= ns[t] <= info["pull_slots"]
         for e in range(rxn.shape[0]):
-            if e >= ns[t]:
-                assert rxn[e, t] == -1
+            if rxn[e, t] == -1:  # hole: rate 0, any finite word
+                assert f1[e, t] <= 4 * T and (e >= f2.shape[0] or f2[e, t] == 4 * T + 3)
                 continue
+            assert e < ns[t]
             assert owner[t] >= 0 and owner[t] not in hub
             r, nu = int(rxn[e, t]) & 0xFFFFFF, int(rxn[e, t]) >> 24
             ent[(int(owner[t]), "+", r)] += nu
             # the factors of the slot reproduce the reactant multiset of the reaction
             c1, t1 = divmod(int(f1[e, t]), T)
             react = [int(owner[t1])] + ([hub[c1 - 1]] if c1 else [])
-            if e < ns2[t]:
-                assert f2[e, t] < T
+            if e < f2.shape[0] and f2[e, t] != 4 * T + 3:  # second factor: a hub's own word
+                assert e < ns2[t] and f2[e, t] < len(hub)
                 react.append(int(owner[f2[e, t]]))
-            elif e < f2.shape[0]:
-                assert f2[e, t] == 4 * T
             assert sorted(react) == sorted(int(s) for s in net.react[r, : net.n_react[r]])
         for s in range(19):
             for q in range(ptr[s, t], ptr[s + 1, t]):
