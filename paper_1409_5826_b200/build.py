@@ -17,7 +17,8 @@ LIB = os.path.join(HERE, "libkinnet.so")
 HEADERS = [os.path.join(CSRC, h) for h in ("schedule.h", "zone_pull.cuh", "device_util.cuh")] + [
     os.path.join(HERE, "..", "include", "kinnet.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-NVCC_FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2,-Wall"]
+NVCC_FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2,-Wall",
+              *os.environ.get("KINNET_DEFS", "").split()]  # e.g. KINNET_DEFS="-DKINNET_MINB160=4" for A/B builds
 
 # (object name, source, extra defines)
 UNITS = [

@@ -35,6 +35,12 @@ enum Mode { kAdaptive = 0, kFixed = 1, kRhs = 2, kRates = 3 };
 // ---------------------------------------------------------------------------
 constexpr int kJ2C = kinnet::kPullMaxSlots2;
 
+// resident CTAs per SM the 160-thread instantiation is compiled for (register budget
+// 65536 / (160 * MINB)); build.py may override it for A/B runs
+#ifndef KINNET_MINB160
+#define KINNET_MINB160 3
+#endif
+
 struct KPull {
     int N, M, nbs;
     int hub[kinnet::kPullHubs];
@@ -65,8 +71,11 @@ typedef void (*pull_fn)(const KPull);
 
 template <typename real>
 __host__ __device__ inline size_t pull_smem_bytes(int T, int W, int M) {
+#ifndef KINNET_PAD_SMEM
+#define KINNET_PAD_SMEM 0  // occupancy experiments: extra bytes that lower the CTAs per SM
+#endif
     return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(W) * 8 + 4 * T + 4) +
-           sizeof(double) * static_cast<size_t>(M);
+           sizeof(double) * static_cast<size_t>(M) + KINNET_PAD_SMEM;
 }
 
 // Kernel for a compiled pull schedule; one definition per (state type, adaptive/fixed)
@@ -81,10 +90,11 @@ pull_fn pull_kernel_f32_fixed(const PullSchedule& P);
 __device__ __forceinline__ double rcp_pos(double b) {  // b normal, positive
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+    // r0 is good to 2^-23 (PTX rcp.approx.ftz.f64); one third-order step leaves e^3 < 2^-69,
+    // i.e. a result within an ulp or two -- far inside the 1e-9 parity bound, and three
+    // dependent FMAs instead of five on the critical path of every sub-step
     double e = fma(-b, r, 1.0);
     e = fma(e, e, e);
-    r = fma(r, e, r);
-    e = fma(-b, r, 1.0);
     r = fma(r, e, r);
     return r;
 }
@@ -107,9 +117,27 @@ __device__ __forceinline__ uint32_t hi16(uint32_t x) {
     asm volatile("shr.u32 %0, %1, 16;" : "=r"(r) : "r"(x));
     return r;
 }
+// Shared memory through 32-bit shared-window addresses.  With generic pointers the
+// compiler rebuilds the window base (S2UR CgaCtaId, UMOV, ULEA) in front of every
+// group of accesses and adds it to each gather offset; here the base is folded into
+// the packed offsets once and an access is one LDS/STS on a register.
+__device__ __forceinline__ void lds(double& v, uint32_t a) {
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void lds(float& v, uint32_t a) {
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void sts(uint32_t a, double v) {
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory");
+}
+__device__ __forceinline__ void sts(uint32_t a, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
+}
 template <typename real>
-__device__ __forceinline__ real lds_at(const unsigned char* base, uint32_t byte_off) {
-    return *reinterpret_cast<const real*>(base + byte_off);
+__device__ __forceinline__ real lds_at(uint32_t a) {
+    real v;
+    lds(v, a);
+    return v;
 }
 
 
@@ -189,14 +217,18 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     real* red = reinterpret_cast<real*>(redmin + 32);            // [NW][8] per-warp hub-row sums
     real* YP = red + NW * 8;                                     // [4][T] published products, then 1
     double* Rbuf = reinterpret_cast<double*>(YP + 4 * T + 4);    // [M] rates, used during set-up only
-    const unsigned char* YPb = reinterpret_cast<const unsigned char*>(YP);
+    constexpr uint32_t SZ = sizeof(real);
+    const uint32_t s_redmin = static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw));
+    const uint32_t s_red = s_redmin + 32 * 8;
+    const uint32_t s_YP = s_red + NW * 8 * SZ;
+    if (s_YP + (4 * T + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
 
     // ---- gather offsets -> registers -------------------------------------------
     uint32_t f1[CP / 2], f2[kJ2C / 2];
 #pragma unroll
-    for (int e = 0; e < CP / 2; ++e) f1[e] = p.f1_pack[e * T + tid];
+    for (int e = 0; e < CP / 2; ++e) f1[e] = p.f1_pack[e * T + tid] + s_YP * 0x10001u;
 #pragma unroll
-    for (int e = 0; e < kJ2C / 2; ++e) f2[e] = p.f2_pack[e * T + tid];
+    for (int e = 0; e < kJ2C / 2; ++e) f2[e] = p.f2_pack[e * T + tid] + s_YP * 0x10001u;
     int wn, wn2;
     {
         const uint32_t cnt = p.cnt[tid];
@@ -276,12 +308,13 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     }
     const int max_steps = ADAPT ? p.max_steps : p.n_fixed;
 
+    const uint32_t s_pub = s_YP + tid * SZ;
     while (run) {
         // ---- publish y x {1, hubs} ------------------------------------------------
-        YP[tid] = y;
-        YP[T + tid] = y * yh0;
-        YP[2 * T + tid] = y * yh1;
-        YP[3 * T + tid] = y * yh2;
+        sts(s_pub, y);
+        sts(s_pub + T * SZ, y * yh0);
+        sts(s_pub + 2 * T * SZ, y * yh1);
+        sts(s_pub + 3 * T * SZ, y * yh2);
 
         // ---- rate sums: k = F-/y (Eq. (1)) and this thread's share of the hub rows ---
         real k, share[6];
@@ -328,7 +361,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         if (nbs > 0) {
             const real tot = warp_sum_rows6(share, lane);
             const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
-            if ((lane & 3) == 0 && (lane & 12) != 12) red[warp * 8 + row] = tot;
+            if ((lane & 3) == 0 && (lane & 12) != 12) sts(s_red + (warp * 8 + row) * SZ, tot);
         }
 
         // ---- S2+S3: F+ = sum of the incoming fluxes, each evaluated here -----------------
@@ -339,18 +372,18 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             for (int g = 0; g < CP / 4; ++g) {
                 if (4 * g < wn) {  // warp-uniform
                     const uint32_t w0 = f1[2 * g], w1 = f1[2 * g + 1];
-                    real a0 = lds_at<real>(YPb, lo16(w0));
-                    real a1 = lds_at<real>(YPb, hi16(w0));
-                    real a2 = lds_at<real>(YPb, lo16(w1));
-                    real a3 = lds_at<real>(YPb, hi16(w1));
+                    real a0 = lds_at<real>(lo16(w0));
+                    real a1 = lds_at<real>(hi16(w0));
+                    real a2 = lds_at<real>(lo16(w1));
+                    real a3 = lds_at<real>(hi16(w1));
                     if (4 * g < kJ2C) {
                         if (4 * g < wn2) {  // second factors (three-body reactions)
                             const uint32_t v0 = f2[(2 * g) % (kJ2C / 2)],
                                            v1 = f2[(2 * g + 1) % (kJ2C / 2)];
-                            a0 *= lds_at<real>(YPb, lo16(v0));
-                            a1 *= lds_at<real>(YPb, hi16(v0));
-                            a2 *= lds_at<real>(YPb, lo16(v1));
-                            a3 *= lds_at<real>(YPb, hi16(v1));
+                            a0 *= lds_at<real>(lo16(v0));
+                            a1 *= lds_at<real>(hi16(v0));
+                            a2 *= lds_at<real>(lo16(v1));
+                            a3 *= lds_at<real>(hi16(v1));
                         }
                     }
                     s0 = fma(R[4 * g], a0, s0);
@@ -367,7 +400,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             double c = dt_candidate(y, Fp - k * y, eps_y, y_floor);
             if (!plain_owner) c = INFINITY;
             c = warp_min_pos(c);
-            if (lane == 0) redmin[warp] = c;
+            if (lane == 0) sts(s_redmin + warp * 8, c);
         }
         __syncthreads();
 
@@ -378,14 +411,18 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             real vp[NW], vm[NW];
 #pragma unroll
             for (int w = 0; w < NW; ++w) {
-                vp[w] = red[w * 8 + lane];
-                vm[w] = red[w * 8 + 3 + lane];
+                vp[w] = lds_at<real>(s_red + (w * 8 + lane) * SZ);
+                vm[w] = lds_at<real>(s_red + (w * 8 + 3 + lane) * SZ);
             }
 #pragma unroll
-            for (int w = 0; w < NW; ++w) {  // fixed order over warps
-                hFp += vp[w];
-                hFm += vm[w];
-            }
+            for (int s = 1; s < NW; s *= 2)  // fixed pairwise order over warps (log depth)
+#pragma unroll
+                for (int w = 0; w + s < NW; w += 2 * s) {
+                    vp[w] += vp[w + s];
+                    vm[w] += vm[w + s];
+                }
+            hFp = vp[0];
+            hFm = vm[0];
         }
         if (!ADAPT && rhs_only) {
             real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
@@ -404,7 +441,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         bool last;
         if (ADAPT) {
             double cand = INFINITY;
-            if (lane >= 8 && lane < 8 + NW) cand = redmin[lane - 8];
+            if (lane >= 8 && lane < 8 + NW) cand = lds_at<double>(s_redmin + (lane - 8) * 8);
             const double hc = dt_candidate(yme, hFp - hFm, eps_y, y_floor);
             if (lane < nbs) cand = hc;
             const double cmin = warp_min_pos(cand);
@@ -457,7 +494,7 @@ pull_fn pick_pull_block(int T) {
     switch (T) {
         case 32: return zone_kernel_pull<real, 32, 12, CP, ADAPT>;
         case 64: return zone_kernel_pull<real, 64, 6, CP, ADAPT>;
-        case 160: return zone_kernel_pull<real, 160, 3, CP, ADAPT>;
+        case 160: return zone_kernel_pull<real, 160, KINNET_MINB160, CP, ADAPT>;
         case 256: return zone_kernel_pull<real, 256, 2, CP, ADAPT>;
         case 384: return zone_kernel_pull<real, 384, 1, CP, ADAPT>;
         default: return zone_kernel_pull<real, 512, 1, CP, ADAPT>;
