@@ -25,4 +25,14 @@ __device__ __forceinline__ double warp_min_pos(double c) {
     return __hiloint2double(static_cast<int>(mh), static_cast<int>(ml));
 }
 
+// Maximum over the warp of non-negative doubles (a NaN wins; callers treat it as no
+// candidate): the same two REDUX on the bit pattern.
+__device__ __forceinline__ double warp_max_pos(double c) {
+    const unsigned hi = static_cast<unsigned>(__double2hiint(c));
+    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned lo = (hi == mh) ? static_cast<unsigned>(__double2loint(c)) : 0u;
+    const unsigned ml = __reduce_max_sync(0xffffffffu, lo);
+    return __hiloint2double(static_cast<int>(mh), static_cast<int>(ml));
+}
+
 }  // namespace kinnet

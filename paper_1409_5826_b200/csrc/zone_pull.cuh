@@ -34,6 +34,13 @@ enum Mode { kAdaptive = 0, kFixed = 1, kRhs = 2, kRates = 3 };
 // the whole hydro step (topology is static, sub-steps number 1e2..1e4).
 // ---------------------------------------------------------------------------
 constexpr int kJ2C = kinnet::kPullMaxSlots2;
+// P-slot rates beyond the first CP - kPullSpillSlots of a thread live in shared memory:
+// only the warp with the longest rows reaches them (the species are dealt to threads by
+// falling in-degree), and every thread gets the registers back.
+#ifndef KINNET_SPILL_SLOTS
+#define KINNET_SPILL_SLOTS 8
+#endif
+constexpr int kPullSpillSlots = KINNET_SPILL_SLOTS;
 
 // resident CTAs per SM the 160-thread instantiation is compiled for (register budget
 // 65536 / (160 * MINB)); build.py may override it for A/B runs
@@ -74,7 +81,8 @@ __host__ __device__ inline size_t pull_smem_bytes(int T, int W, int M) {
 #ifndef KINNET_PAD_SMEM
 #define KINNET_PAD_SMEM 0  // occupancy experiments: extra bytes that lower the CTAs per SM
 #endif
-    return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(W) * 8 + 4 * T + 4) +
+    return 32 * sizeof(double) +
+           sizeof(real) * (static_cast<size_t>(W) * 8 + 4 * T + 4 + kPullSpillSlots * T) +
            sizeof(double) * static_cast<size_t>(M) + KINNET_PAD_SMEM;
 }
 
@@ -141,72 +149,15 @@ __device__ __forceinline__ real lds_at(uint32_t a) {
 }
 
 
-// dt candidate of one species: eps max(y, floor) / |F+ - F-|   (reading Q7).
-// Branch-free: the reciprocal is always formed, of 1 when the change is (near) zero.
 template <typename real>
-__device__ __forceinline__ double dt_candidate(real y, real a, real eps_y, real y_floor) {
-    a = a < 0 ? -a : a;
-    const bool moves = a > Tiny<real>::v();
-    const real c = eps_y * (y > y_floor ? y : y_floor) * rcp_pos(moves ? a : static_cast<real>(1));
-    return moves ? static_cast<double>(c) : static_cast<double>(INFINITY);
-}
-
-// Sum rows 0..5 of v over the warp (rows 0..2 = F+ shares of the hubs, 3..5 = F-
-// shares).  On return the lanes 0, 8, 4, 16, 24, 20 hold the totals of rows
-// 0, 1, 2, 3, 4, 5.  Fixed order: deterministic.  14 shuffles of 4-byte halves
-// per 8-byte value instead of 60 for six plain butterflies.
-template <typename real>
-__device__ __forceinline__ real warp_sum_rows6(const real (&v)[6], int lane) {
-    const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
-    real a[3];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const real send = up16 ? v[i] : v[i + 3];
-        const real keep = up16 ? v[i + 3] : v[i];
-        a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-    real b0, b1;
-    {
-        const real send = up8 ? a[0] : a[1];
-        const real keep = up8 ? a[1] : a[0];
-        b0 = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        b1 = a[2] + __shfl_xor_sync(0xffffffffu, a[2], 8);
-    }
-    real c;
-    {
-        const real send = up4 ? b0 : b1;
-        const real keep = up4 ? b1 : b0;
-        c = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    }
-    c += __shfl_xor_sync(0xffffffffu, c, 2);
-    c += __shfl_xor_sync(0xffffffffu, c, 1);
-    return c;
-}
-
-// Explicit asymptotic / forward Euler update of one species from F+ and k = F-/y
-// (Eq. (3); y = 0 takes the Euler branch, reading Q8).
-// Branch-free: both candidates are formed, 1 + k dt >= 1 is always a safe divisor.
-template <typename real>
-__device__ __forceinline__ real update_k(real y, real Fp, real k, real h, real kappa) {
-    const real kh = k * h;
-    const real ya = fma(h, Fp, y) * rcp_pos(static_cast<real>(1) + kh);
-    const real ye = fma(h, Fp - k * y, y);
-    return (y > 0 && kh >= kappa) ? ya : ye;
-}
-
-// Same update from F+ and F- (hub species): Eq. (3) as Y (Y + dt F+) / (Y + dt F-).
-template <typename real>
-__device__ __forceinline__ real update_fm(real y, real Fp, real Fm, real h, real kappa) {
-    const real hFm = h * Fm;
-    const bool pos = y > Tiny<real>::v();
-    const real ya = fma(h, Fp, y) * (y * rcp_pos(pos ? y + hFm : static_cast<real>(1)));
-    const real ye = fma(h, Fp - Fm, y);
-    return (pos && hFm >= kappa * y) ? ya : ye;
+__device__ __forceinline__ real abs_of(real a) {
+    return a < 0 ? -a : a;
 }
 
 template <typename real, int TB, int MINB, int CP, bool ADAPT>
 __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     static_assert(CP % 4 == 0 && CP <= kinnet::kPullMaxSlots, "slot capacity");
+    constexpr int CPR = CP > 12 ? CP - kPullSpillSlots : CP;  // slots whose rate stays in a register
     constexpr int T = TB, NW = TB / 32;  // the schedule is built for exactly TB threads
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -216,11 +167,13 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     double* redmin = reinterpret_cast<double*>(smem_raw);        // [32] per-warp dt minima
     real* red = reinterpret_cast<real*>(redmin + 32);            // [NW][8] per-warp hub-row sums
     real* YP = red + NW * 8;                                     // [4][T] published products, then 1
-    double* Rbuf = reinterpret_cast<double*>(YP + 4 * T + 4);    // [M] rates, used during set-up only
+    real* Rx = YP + 4 * T + 4;                                   // [kPullSpillSlots][T] spilled slot rates
+    double* Rbuf = reinterpret_cast<double*>(Rx + kPullSpillSlots * T);  // [M] rates, set-up only
     constexpr uint32_t SZ = sizeof(real);
     const uint32_t s_redmin = static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw));
     const uint32_t s_red = s_redmin + 32 * 8;
     const uint32_t s_YP = s_red + NW * 8 * SZ;
+    const uint32_t s_Rx = s_YP + (4 * T + 4) * SZ + tid * SZ;
     if (s_YP + (4 * T + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
 
     // ---- gather offsets -> registers -------------------------------------------
@@ -254,12 +207,14 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     __syncthreads();
 
     // rates of the P-slots and the rate sums of this thread, kept in registers
-    real R[CP];
+    real R[CPR];
 #pragma unroll
     for (int e = 0; e < CP; ++e) {
         const int32_t v = p.slot_rxn[e * T + tid];
-        R[e] = v < 0 ? static_cast<real>(0)
-                     : static_cast<real>(static_cast<double>(v >> 24) * Rbuf[v & 0xffffff]);
+        const real r = v < 0 ? static_cast<real>(0)
+                             : static_cast<real>(static_cast<double>(v >> 24) * Rbuf[v & 0xffffff]);
+        if (e < CPR) R[e] = r;
+        else Rx[(e - CPR) * T + tid] = r;
     }
     real C[kinnet::kPullCoefs];
     {
@@ -294,27 +249,38 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     const double growth = p.growth, t_hydro = p.t_hydro;
     const bool rhs_only = p.mode == kRhs;
 
-    double t = 0.0, dt_prev = 0.0;
+    // The controller runs on q = 1/dt: the candidates become
+    // |F+ - F-| / (eps max(y, floor)), their reciprocal factor is formed while the
+    // gathers are in flight, the zone-wide reduction is a maximum, and Eq. (3) reads
+    // (y q + F+) / (q + k), so no reciprocal sits between the reduction and the update
+    // chain except the ones that run side by side.
+    double t = 0.0, q_prev = 0.0, dt_out = 0.0;
     int steps = 0;
     int status = 0;
     bool run = true;
     if (ADAPT) {
         const double dt_in = p.dt ? p.dt[z] : 0.0;
-        dt_prev = (dt_in > 0.0) ? dt_in : t_hydro;
         run = t_hydro > 0.0;
-        if (!run) dt_prev = dt_in;  // nothing to do: the trial dt is returned unchanged
+        dt_out = dt_in;  // nothing to do: the trial dt is returned unchanged
+        if (run) q_prev = 1.0 / ((dt_in > 0.0) ? dt_in : t_hydro);
     } else if (!rhs_only) {
         run = p.n_fixed > 0;
     }
     const int max_steps = ADAPT ? p.max_steps : p.n_fixed;
-
+    const double ginv = 1.0 / growth;
+    const double q_fixed = ADAPT ? 0.0 : 1.0 / p.dt_fixed;
+    const real kappa_ = kappa;
     const uint32_t s_pub = s_YP + tid * SZ;
+    const uint32_t s_own = s_redmin + 16 * 8;  // [3] own-consumption terms of the hub owners
+    const real yfl_eps = eps_y * y_floor;
+
     while (run) {
         // ---- publish y x {1, hubs} ------------------------------------------------
+        const real p1 = y * yh0, p2 = y * yh1, p3 = y * yh2;
         sts(s_pub, y);
-        sts(s_pub + T * SZ, y * yh0);
-        sts(s_pub + 2 * T * SZ, y * yh1);
-        sts(s_pub + 3 * T * SZ, y * yh2);
+        sts(s_pub + T * SZ, p1);
+        sts(s_pub + 2 * T * SZ, p2);
+        sts(s_pub + 3 * T * SZ, p3);
 
         // ---- rate sums: k = F-/y (Eq. (1)) and this thread's share of the hub rows ---
         real k, share[6];
@@ -328,19 +294,13 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             k = fma(yh0, e0, K0);
             k = fma(yh1, e1, k);
             k = fma(yh2, e2, k);
-            // F-_hub share / y: Y_h dk/dY_h (each hub co-reactant occurrence counts once)
-            real m0 = fma(K00, yh0, e0);
+            // F-_hub share / (y Y_h): dk/dY_h (each hub co-reactant occurrence counts once)
+            const real m0 = fma(K00, yh0, e0);
             real m1 = fma(K01, yh0, e1);
             m1 = fma(K11, yh1, m1);
             real m2 = fma(K02, yh0, e2);
             m2 = fma(K12, yh1, m2);
             m2 = fma(K22, yh2, m2);
-            m0 *= yh0;
-            m1 *= yh1;
-            m2 *= yh2;
-            if (tid == 0) m0 += k;  // the owner's own consumption in a hub-only reaction
-            if (tid == 1) m1 += k;
-            if (tid == 2) m2 += k;
             // F+_hub share / y
             real g0 = fma(C[13], yh1, C[10]);
             g0 = fma(C[14], yh2, g0);
@@ -351,62 +311,120 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             share[0] = y * g0;
             share[1] = y * g1;
             share[2] = y * g2;
-            share[3] = y * m0;
-            share[4] = y * m1;
-            share[5] = y * m2;
+            share[3] = p1 * m0;
+            share[4] = p2 * m1;
+            share[5] = p3 * m2;
+        }
+        // the owner's own consumption in a hub-only reaction joins its F- row in finalize
+        if (hub_owner) sts(s_own + tid * SZ, k * y);
+
+        // reciprocal factors of the dt candidates, off the critical path
+        real inv = 0;
+        if (ADAPT) {
+            inv = rcp_pos(y > y_floor ? eps_y * y : yfl_eps);
+            if (!plain_owner) inv = 0;  // hub owners are judged on their full rows in finalize
         }
         __syncthreads();
 
-        // ---- hub rows: warp totals of the six shares ---------------------------------------
-        if (nbs > 0) {
-            const real tot = warp_sum_rows6(share, lane);
-            const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
-            if ((lane & 3) == 0 && (lane & 12) != 12) sts(s_red + (warp * 8 + row) * SZ, tot);
-        }
-
-        // ---- S2+S3: F+ = sum of the incoming fluxes, each evaluated here -----------------
+        // ---- S2+S3 interleaved with the hub-row butterfly -------------------------------------
+        // F+ = sum of the incoming fluxes, each evaluated here (groups of four P-slots), and
+        // the six hub-row shares summed over the warp (rows 0..2 = F+, 3..5 = F-; the lanes
+        // 0, 8, 4, 16, 24, 20 end up with the totals of rows 0, 1, 2, 3, 4, 5; 14 shuffles
+        // of 4-byte halves per 8-byte value instead of 60 for six plain butterflies).  The two
+        // are independent latency chains (SHFL and LDS), so one stage of each alternates.
         real Fp;
         {
             real s0 = 0, s1 = 0, s2 = 0, s3 = 0;
-#pragma unroll
-            for (int g = 0; g < CP / 4; ++g) {
-                if (4 * g < wn) {  // warp-uniform
-                    const uint32_t w0 = f1[2 * g], w1 = f1[2 * g + 1];
-                    real a0 = lds_at<real>(lo16(w0));
-                    real a1 = lds_at<real>(hi16(w0));
-                    real a2 = lds_at<real>(lo16(w1));
-                    real a3 = lds_at<real>(hi16(w1));
-                    if (4 * g < kJ2C) {
-                        if (4 * g < wn2) {  // second factors (three-body reactions)
-                            const uint32_t v0 = f2[(2 * g) % (kJ2C / 2)],
-                                           v1 = f2[(2 * g + 1) % (kJ2C / 2)];
-                            a0 *= lds_at<real>(lo16(v0));
-                            a1 *= lds_at<real>(hi16(v0));
-                            a2 *= lds_at<real>(lo16(v1));
-                            a3 *= lds_at<real>(hi16(v1));
-                        }
-                    }
-                    s0 = fma(R[4 * g], a0, s0);
-                    s1 = fma(R[4 * g + 1], a1, s1);
-                    s2 = fma(R[4 * g + 2], a2, s2);
-                    s3 = fma(R[4 * g + 3], a3, s3);
-                }
-            }
+            real a0, a1, a2, a3;
+#define KINNET_LOADS(g)                                                                 \
+    if (4 * (g) < CP && 4 * (g) < wn) {                                                 \
+        const uint32_t w0 = f1[(2 * (g)) % (CP / 2)], w1 = f1[(2 * (g) + 1) % (CP / 2)]; \
+        a0 = lds_at<real>(lo16(w0));                                                    \
+        a1 = lds_at<real>(hi16(w0));                                                    \
+        a2 = lds_at<real>(lo16(w1));                                                    \
+        a3 = lds_at<real>(hi16(w1));                                                    \
+        if (4 * (g) < kJ2C && 4 * (g) < wn2) { /* second factors (three-body reactions) */ \
+            const uint32_t v0 = f2[(2 * (g)) % (kJ2C / 2)], v1 = f2[(2 * (g) + 1) % (kJ2C / 2)]; \
+            a0 *= lds_at<real>(lo16(v0));                                               \
+            a1 *= lds_at<real>(hi16(v0));                                               \
+            a2 *= lds_at<real>(lo16(v1));                                               \
+            a3 *= lds_at<real>(hi16(v1));                                               \
+        }                                                                               \
+    }
+// byte offset of spilled slot e (dead branches of the unrolled groups clamp to 0)
+#define KINNET_XOFF(e) (static_cast<uint32_t>((e) >= CPR ? (e) - CPR : 0) * T * SZ)
+#define KINNET_FMAS(g)                                                          \
+    if (4 * (g) < CPR && 4 * (g) < wn) {                                        \
+        s0 = fma(R[(4 * (g)) % CPR], a0, s0);                                   \
+        s1 = fma(R[(4 * (g) + 1) % CPR], a1, s1);                               \
+        s2 = fma(R[(4 * (g) + 2) % CPR], a2, s2);                               \
+        s3 = fma(R[(4 * (g) + 3) % CPR], a3, s3);                               \
+    } else if (4 * (g) < CP && 4 * (g) < wn) {                                  \
+        s0 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g))), a0, s0);        \
+        s1 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 1)), a1, s1);    \
+        s2 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 2)), a2, s2);    \
+        s3 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 3)), a3, s3);    \
+    }
+            const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
+            // level 16
+            real r0 = __shfl_xor_sync(0xffffffffu, up16 ? share[0] : share[3], 16);
+            real r1 = __shfl_xor_sync(0xffffffffu, up16 ? share[1] : share[4], 16);
+            real r2 = __shfl_xor_sync(0xffffffffu, up16 ? share[2] : share[5], 16);
+            KINNET_LOADS(0)
+            const real b0_ = (up16 ? share[3] : share[0]) + r0;
+            const real b1_ = (up16 ? share[4] : share[1]) + r1;
+            const real b2_ = (up16 ? share[5] : share[2]) + r2;
+            // level 8
+            r0 = __shfl_xor_sync(0xffffffffu, up8 ? b0_ : b1_, 8);
+            r1 = __shfl_xor_sync(0xffffffffu, b2_, 8);
+            KINNET_FMAS(0)
+            KINNET_LOADS(1)
+            const real c0_ = (up8 ? b1_ : b0_) + r0;
+            const real c1_ = b2_ + r1;
+            // level 4
+            r0 = __shfl_xor_sync(0xffffffffu, up4 ? c0_ : c1_, 4);
+            KINNET_FMAS(1)
+            KINNET_LOADS(2)
+            real tot = (up4 ? c1_ : c0_) + r0;
+            r0 = __shfl_xor_sync(0xffffffffu, tot, 2);
+            KINNET_FMAS(2)
+            KINNET_LOADS(3)
+            tot += r0;
+            r0 = __shfl_xor_sync(0xffffffffu, tot, 1);
+            KINNET_FMAS(3)
+            KINNET_LOADS(4)
+            tot += r0;
+            KINNET_FMAS(4)
+            KINNET_LOADS(5)
+            KINNET_FMAS(5)
+#undef KINNET_LOADS
+#undef KINNET_FMAS
+#undef KINNET_XOFF
+            const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
+            if ((lane & 3) == 0 && (lane & 12) != 12) sts(s_red + (warp * 8 + row) * SZ, tot);
             Fp = (s0 + s1) + (s2 + s3);
         }
 
-        // ---- S5: dt candidates of the non-hub species ------------------------------------
+        // ---- S5: q candidates of the non-hub species: |F+ - F-| / (eps max(y, floor)) ------
+        const real change = fma(-k, y, Fp);
         if (ADAPT) {
-            double c = dt_candidate(y, Fp - k * y, eps_y, y_floor);
-            if (!plain_owner) c = INFINITY;
-            c = warp_min_pos(c);
+            const double c = warp_max_pos(static_cast<double>(fabs(change) * inv));
             if (lane == 0) sts(s_redmin + warp * 8, c);
         }
         __syncthreads();
 
         // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
-        real hFp = 0, hFm = 0;
+        // (the reciprocals below depend on nothing the barrier waited for: they run beside
+        // the loads and the sums over warps)
         const real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
+        real invh = 0;
+        double q_rem = 0.0, rem = 0.0;
+        if (ADAPT) {
+            invh = rcp_pos(yme > y_floor ? eps_y * yme : yfl_eps);
+            rem = t_hydro - t;
+            q_rem = rcp_pos(rem);
+        }
+        real hFp = 0, hFm = 0;
         if (lane < nbs) {  // three active lanes: one wavefront per load instead of two
             real vp[NW], vm[NW];
 #pragma unroll
@@ -414,6 +432,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
                 vp[w] = lds_at<real>(s_red + (w * 8 + lane) * SZ);
                 vm[w] = lds_at<real>(s_red + (w * 8 + 3 + lane) * SZ);
             }
+            const real own_term = lds_at<real>(s_own + lane * SZ);
 #pragma unroll
             for (int s = 1; s < NW; s *= 2)  // fixed pairwise order over warps (log depth)
 #pragma unroll
@@ -422,7 +441,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
                     vm[w] += vm[w + s];
                 }
             hFp = vp[0];
-            hFm = vm[0];
+            hFm = vm[0] + own_term;
         }
         if (!ADAPT && rhs_only) {
             real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
@@ -437,36 +456,48 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             return;
         }
 
-        double dts;
+        double q, hd;
         bool last;
         if (ADAPT) {
-            double cand = INFINITY;
+            double cand = 0.0;
             if (lane >= 8 && lane < 8 + NW) cand = lds_at<double>(s_redmin + (lane - 8) * 8);
-            const double hc = dt_candidate(yme, hFp - hFm, eps_y, y_floor);
-            if (lane < nbs) cand = hc;
-            const double cmin = warp_min_pos(cand);
-            double dt_ctrl = growth * dt_prev;
-            if (cmin < dt_ctrl) dt_ctrl = cmin;
-            const double rem = t_hydro - t;
-            last = dt_ctrl >= rem * (1.0 - 1e-12);
-            dts = last ? rem : dt_ctrl;
-            dt_prev = dt_ctrl;
+            const double qh = static_cast<double>(abs_of(hFp - hFm) * invh);
+            if (lane < nbs) cand = qh;
+            const double qmax = warp_max_pos(cand);
+            const double qg = q_prev * ginv;             // growth cap: dt <= g dt_prev
+            const double q_ctrl = (qmax > qg) ? qmax : qg;  // a NaN candidate loses
+            last = q_ctrl <= q_rem * (1.0 / (1.0 - 1e-12));  // dt_ctrl >= rem (1 - 1e-12)
+            q = last ? q_rem : q_ctrl;
+            hd = last ? rem : rcp_pos(q_ctrl);
+            q_prev = q_ctrl;
         } else {
-            dts = p.dt_fixed;
+            q = q_fixed;
+            hd = p.dt_fixed;
             last = (steps + 1 >= max_steps);
         }
-        const real h = static_cast<real>(dts);
+        const real h = static_cast<real>(hd), qr = static_cast<real>(q);
 
         // ---- S4: update (Eq. (3)) -------------------------------------------
-        const real yn = update_k(y, Fp, k, h, kappa);
-        if (nbs > 0) {  // hub species, on lanes 0..nbs-1 of every warp, from F+ and F-
-            const real hn = update_fm(yme, hFp, hFm, h, kappa);
-            yh0 = __shfl_sync(0xffffffffu, hn, 0);
+        // Eq. (3) times q/q: (y + dt F+) / (1 + k dt) = (y q + F+) / (q + k); y = 0 takes the
+        // Euler branch (reading Q8).  Branch-free: both candidates are formed.
+        real yn;
+        {
+            const real ya = fma(y, qr, Fp) * rcp_pos(qr + k);
+            const real ye = fma(h, change, y);
+            yn = (y > 0 && k * h >= kappa_) ? ya : ye;
+        }
+        {  // hub species, on lanes 0..nbs-1 of every warp: Y (Y q + F+) / (Y q + F-)
+            const bool pos = yme > Tiny<real>::v();
+            const real den = fma(yme, qr, hFm);
+            const real ya = fma(yme, qr, hFp) * (yme * rcp_pos(pos ? den : static_cast<real>(1)));
+            const real ye = fma(h, hFp - hFm, yme);
+            const real hn = (pos && h * hFm >= kappa_ * yme) ? ya : ye;
+            if (nbs > 0) yh0 = __shfl_sync(0xffffffffu, hn, 0);
             if (nbs > 1) yh1 = __shfl_sync(0xffffffffu, hn, 1);
             if (nbs > 2) yh2 = __shfl_sync(0xffffffffu, hn, 2);
+            y = hub_owner ? hn : yn;  // hub h lives on thread h: warp 0, lane h
         }
-        y = hub_owner ? (tid == 0 ? yh0 : (tid == 1 ? yh1 : yh2)) : yn;
-        t = last ? t_hydro : t + dts;
+        t = last ? t_hydro : t + hd;
         ++steps;
         if (last) run = false;
         else if (ADAPT && steps >= max_steps) {
@@ -474,13 +505,14 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             run = false;
         }
     }
+    if (ADAPT && steps > 0) dt_out = 1.0 / q_prev;
 
     // ---- S6: zone state out ------------------------------------------------------------------
     const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
     if (own >= 0) Yg[own] = y;
     if (tid == 0) {
-        if (ADAPT && p.dt) p.dt[z] = dt_prev;
+        if (ADAPT && p.dt) p.dt[z] = dt_out;
         if (p.n_steps) p.n_steps[z] = steps;
         if (p.status) p.status[z] = status;
     }
