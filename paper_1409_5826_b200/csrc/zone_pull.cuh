@@ -170,7 +170,12 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     real* Rx = YP + 4 * T + 4;                                   // [kPullSpillSlots][T] spilled slot rates
     double* Rbuf = reinterpret_cast<double*>(Rx + kPullSpillSlots * T);  // [M] rates, set-up only
     constexpr uint32_t SZ = sizeof(real);
-    const uint32_t s_redmin = static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw));
+    // opaque to the compiler: otherwise it rebuilds the window base (S2UR CgaCtaId + ULEA,
+    // ~30 exposed cycles) in front of every group of accesses instead of keeping a register
+    uint32_t s_redmin;
+    asm volatile("mov.u32 %0, %1;"
+                 : "=r"(s_redmin)
+                 : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw))));
     const uint32_t s_red = s_redmin + 32 * 8;
     const uint32_t s_YP = s_red + NW * 8 * SZ;
     const uint32_t s_Rx = s_YP + (4 * T + 4) * SZ + tid * SZ;
@@ -334,10 +339,10 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         // are independent latency chains (SHFL and LDS), so one stage of each alternates.
         real Fp;
         {
-            real s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+            real s0, s1, s2, s3;  // group 0 always runs (wn >= 4: holes carry rate 0)
             real a0, a1, a2, a3;
 #define KINNET_LOADS(g)                                                                 \
-    if (4 * (g) < CP && 4 * (g) < wn) {                                                 \
+    if ((g) == 0 || (4 * (g) < CP && 4 * (g) < wn)) {                                   \
         const uint32_t w0 = f1[(2 * (g)) % (CP / 2)], w1 = f1[(2 * (g) + 1) % (CP / 2)]; \
         a0 = lds_at<real>(lo16(w0));                                                    \
         a1 = lds_at<real>(hi16(w0));                                                    \
@@ -354,7 +359,12 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
 // byte offset of spilled slot e (dead branches of the unrolled groups clamp to 0)
 #define KINNET_XOFF(e) (static_cast<uint32_t>((e) >= CPR ? (e) - CPR : 0) * T * SZ)
 #define KINNET_FMAS(g)                                                          \
-    if (4 * (g) < CPR && 4 * (g) < wn) {                                        \
+    if ((g) == 0) {                                                             \
+        s0 = R[0] * a0;                                                         \
+        s1 = R[1] * a1;                                                         \
+        s2 = R[2] * a2;                                                         \
+        s3 = R[3] * a3;                                                         \
+    } else if (4 * (g) < CPR && 4 * (g) < wn) {                                        \
         s0 = fma(R[(4 * (g)) % CPR], a0, s0);                                   \
         s1 = fma(R[(4 * (g) + 1) % CPR], a1, s1);                               \
         s2 = fma(R[(4 * (g) + 2) % CPR], a2, s2);                               \
@@ -491,10 +501,11 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             const real den = fma(yme, qr, hFm);
             const real ya = fma(yme, qr, hFp) * (yme * rcp_pos(pos ? den : static_cast<real>(1)));
             const real ye = fma(h, hFp - hFm, yme);
-            const real hn = (pos && h * hFm >= kappa_ * yme) ? ya : ye;
-            if (nbs > 0) yh0 = __shfl_sync(0xffffffffu, hn, 0);
-            if (nbs > 1) yh1 = __shfl_sync(0xffffffffu, hn, 1);
-            if (nbs > 2) yh2 = __shfl_sync(0xffffffffu, hn, 2);
+            real hn = (pos && h * hFm >= kappa_ * yme) ? ya : ye;
+            if (lane >= nbs) hn = 0;  // a missing hub reads as abundance 0
+            yh0 = __shfl_sync(0xffffffffu, hn, 0);  // unconditional: the three go out back to back
+            yh1 = __shfl_sync(0xffffffffu, hn, 1);
+            yh2 = __shfl_sync(0xffffffffu, hn, 2);
             y = hub_owner ? hn : yn;  // hub h lives on thread h: warp 0, lane h
         }
         t = last ? t_hydro : t + hd;
