@@ -154,9 +154,10 @@ __device__ __forceinline__ real abs_of(real a) {
     return a < 0 ? -a : a;
 }
 
-template <typename real, int TB, int MINB, int CP, bool ADAPT>
+template <typename real, int TB, int MINB, int CP, int J2, bool ADAPT>
 __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     static_assert(CP % 4 == 0 && CP <= kinnet::kPullMaxSlots, "slot capacity");
+    static_assert(J2 % 4 == 0 && J2 <= kJ2C, "second-factor slot capacity");
     constexpr int CPR = CP > 12 ? CP - kPullSpillSlots : CP;  // slots whose rate stays in a register
     constexpr int T = TB, NW = TB / 32;  // the schedule is built for exactly TB threads
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -182,11 +183,11 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     if (s_YP + (4 * T + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
 
     // ---- gather offsets -> registers -------------------------------------------
-    uint32_t f1[CP / 2], f2[kJ2C / 2];
+    uint32_t f1[CP / 2], f2[J2 / 2];
 #pragma unroll
     for (int e = 0; e < CP / 2; ++e) f1[e] = p.f1_pack[e * T + tid] + s_YP * 0x10001u;
 #pragma unroll
-    for (int e = 0; e < kJ2C / 2; ++e) f2[e] = p.f2_pack[e * T + tid] + s_YP * 0x10001u;
+    for (int e = 0; e < J2 / 2; ++e) f2[e] = p.f2_pack[e * T + tid] + s_YP * 0x10001u;
     int wn, wn2;
     {
         const uint32_t cnt = p.cnt[tid];
@@ -348,8 +349,8 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
         a1 = lds_at<real>(hi16(w0));                                                    \
         a2 = lds_at<real>(lo16(w1));                                                    \
         a3 = lds_at<real>(hi16(w1));                                                    \
-        if (4 * (g) < kJ2C && 4 * (g) < wn2) { /* second factors (three-body reactions) */ \
-            const uint32_t v0 = f2[(2 * (g)) % (kJ2C / 2)], v1 = f2[(2 * (g) + 1) % (kJ2C / 2)]; \
+        if (4 * (g) < J2 && 4 * (g) < wn2) { /* second factors (three-body reactions) */ \
+            const uint32_t v0 = f2[(2 * (g)) % (J2 / 2)], v1 = f2[(2 * (g) + 1) % (J2 / 2)]; \
             a0 *= lds_at<real>(lo16(v0));                                               \
             a1 *= lds_at<real>(hi16(v0));                                               \
             a2 *= lds_at<real>(lo16(v1));                                               \
@@ -532,23 +533,31 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
 // pull kernel: block-size classes with the residency the register file allows
 // (65536 / (TB * MINB) registers per thread) x P-slot capacity classes
 
-template <typename real, int CP, bool ADAPT>
+template <typename real, int CP, int J2, bool ADAPT>
 pull_fn pick_pull_block(int T) {
     switch (T) {
-        case 32: return zone_kernel_pull<real, 32, 12, CP, ADAPT>;
-        case 64: return zone_kernel_pull<real, 64, 6, CP, ADAPT>;
-        case 160: return zone_kernel_pull<real, 160, KINNET_MINB160, CP, ADAPT>;
-        case 256: return zone_kernel_pull<real, 256, 2, CP, ADAPT>;
-        case 384: return zone_kernel_pull<real, 384, 1, CP, ADAPT>;
-        default: return zone_kernel_pull<real, 512, 1, CP, ADAPT>;
+        case 32: return zone_kernel_pull<real, 32, 12, CP, J2, ADAPT>;
+        case 64: return zone_kernel_pull<real, 64, 6, CP, J2, ADAPT>;
+        case 160: return zone_kernel_pull<real, 160, KINNET_MINB160, CP, J2, ADAPT>;
+        case 256: return zone_kernel_pull<real, 256, 2, CP, J2, ADAPT>;
+        case 384: return zone_kernel_pull<real, 384, 1, CP, J2, ADAPT>;
+        default: return zone_kernel_pull<real, 512, 1, CP, J2, ADAPT>;
     }
 }
 
+template <typename real, int J2, bool ADAPT>
+pull_fn pick_pull_slots(const kinnet::PullSchedule& P) {
+    if (P.slots <= 12) return pick_pull_block<real, 12, J2, ADAPT>(P.T);
+    if (P.slots <= 20) return pick_pull_block<real, 20, J2, ADAPT>(P.T);
+    return pick_pull_block<real, 24, J2, ADAPT>(P.T);
+}
+
+// P-slot capacity classes x second-factor capacity classes (the packed offsets of
+// the unused capacity would only hold registers)
 template <typename real, bool ADAPT>
 pull_fn pick_pull_real(const kinnet::PullSchedule& P) {
-    if (P.slots <= 12) return pick_pull_block<real, 12, ADAPT>(P.T);
-    if (P.slots <= 20) return pick_pull_block<real, 20, ADAPT>(P.T);
-    return pick_pull_block<real, 24, ADAPT>(P.T);
+    if (P.slots2 <= 4) return pick_pull_slots<real, 4, ADAPT>(P);
+    return pick_pull_slots<real, 8, ADAPT>(P);
 }
 
 #endif  // KINNET_PULL_INSTANTIATE
