@@ -28,6 +28,7 @@ UNIT = "zone-networks/s"
 ZONES_PER_GPU = 16384
 T_HYDRO = 1e-6
 PROFILE_SEED = 4
+DRAM_BYTES_PER_LAUNCH = 20342784
 
 # Algorithmic work per zone per sub-step: one multiply per
 # reactant of every reaction, one add per F+/F- entry, ~10 flops per species for
@@ -117,20 +118,28 @@ def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU):
     return net, T9[lo:hi].copy(), rho[lo:hi].copy(), Y0[lo:hi].copy()
 
 
-def cpu_baseline(net, T9, rho, Y0, zones_per_core=96, reps=1):
-    """The oracle as it stands on the host cores, on a bounded prefix sample."""
+def cpu_sample_size(o, T9, rho, Y0, cores, target_s):
+    """Prefix of the workload that costs the oracle about target_s seconds on
+    these cores, sized from a short probe (8 zones per core)."""
+    probe = int(min(len(T9), 8 * cores))
+    t0 = time.perf_counter()
+    o.integrate(T9[:probe], rho[:probe], Y0[:probe], T_HYDRO, n_threads=cores)
+    rate = probe / max(time.perf_counter() - t0, 1e-6)
+    return int(max(probe, min(len(T9), rate * target_s)))
+
+
+def cpu_baseline(net, T9, rho, Y0, target_s=15.0):
+    """The oracle as it stands on the host cores, on a bounded prefix sample
+    (about target_s seconds of CPU work)."""
     from oracle import Oracle, max_threads
 
     cores = max_threads()
-    n = int(min(len(T9), zones_per_core * cores))
     o = Oracle(net)
-    best, steps = None, 0
-    for _ in range(reps):
-        t0 = time.perf_counter()
-        out = o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
-        dt = time.perf_counter() - t0
-        best = dt if best is None else min(best, dt)
-        steps = int(out["n_steps"].sum())
+    n = cpu_sample_size(o, T9, rho, Y0, cores, target_s)
+    t0 = time.perf_counter()
+    out = o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
+    best = time.perf_counter() - t0
+    steps = int(out["n_steps"].sum())
     return {"value": n / best, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {n} of {len(T9)} zones of the same workload, {steps} sub-steps, "
                       f"{best:.2f} s, gcc -O2 -ffp-contract=off, OpenMP dynamic over zones",
@@ -145,8 +154,9 @@ def run_reference(args):
     from oracle import Oracle, max_threads
 
     cores = max_threads()
-    n = int(min(len(T9), 48 * cores))
     o = Oracle(net)
+    # each step a bounded sample: the whole --steps/--warmup run ends within ~2 minutes
+    n = cpu_sample_size(o, T9, rho, Y0, cores, 100.0 / max(1, args.steps + args.warmup))
     for _ in range(args.warmup):
         o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
     t0 = time.perf_counter()
@@ -188,8 +198,11 @@ def run_ours(args):
 
     net, T9h, rhoh, Y0h = workload(rank, world, args.zones)
     z, N = Y0h.shape
-    kn = K.Net(net)
+    kn = K.Net(net, K.NetParams(precision=args.precision))
     info = kn.schedule_info()
+    ynp = np.float64 if args.precision == 64 else np.float32
+    ybytes = 8 if args.precision == 64 else 4
+    Y0h = np.ascontiguousarray(Y0h.astype(ynp))
     T9, rho = torch.from_numpy(T9h).to(dev), torch.from_numpy(rhoh).to(dev)
     Y0 = torch.from_numpy(Y0h).to(dev)
     Y = torch.empty_like(Y0)
@@ -252,19 +265,13 @@ def run_ours(args):
                               stp.numpy(), sts.numpy())
         if it > 0:
             e2e_s += time.perf_counter() - t1
-    h2d = z * (N * 8 + 8 + 8 + 8)
-    d2h = z * (N * 8 + 8 + 4 + 4)
+    h2d = z * (N * ybytes + 8 + 8 + 8)
+    d2h = z * (N * ybytes + 8 + 4 + 4)
 
     # ---- max over ranks ---------------------------------------------------
-    tm = torch.tensor([total_ms, e2e_s, float(substeps)], dtype=torch.float64, device=dev)
-    if world > 1:
-        mx = tm.clone()
-        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = tm.clone()
-        dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        total_ms, e2e_s, substeps_all = float(mx[0]), float(mx[1]), float(sm[2])
-    else:
-        substeps_all = float(substeps)
+    from paper_1409_5826_b200.shard import reduce_job
+
+    (total_ms, e2e_s), (substeps_all,) = reduce_job([total_ms, e2e_s], [substeps], device=dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -279,15 +286,14 @@ def run_ours(args):
     k_ms = float(np.mean(kernel_ms))
     fp64_ach = flops * per_launch_substeps / (k_ms * 1e-3) / 1e12
     smem_ach = smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12
-    traffic_path = os.path.join(ROOT, "profiles", "dram_traffic.json")
-    traffic = None
-    if os.path.exists(traffic_path):
-        with open(traffic_path) as fh:
-            traffic = json.load(fh).get("dram_bytes_per_launch")
+    # dram__bytes_read.sum + dram__bytes_write.sum of one 16384-zone launch, from the
+    # ncu --set full capture summarised in profiles/r01d_pull_kernel.md (20.34 MB + 0 B)
+    traffic = DRAM_BYTES_PER_LAUNCH if z == ZONES_PER_GPU else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+        "data": "synthetic",
         "config": {
             "workload": "configs[3]: synthetic 150sp/1604rx hub network (seed 1409), 16384 zones per GPU, "
                         "T9~U[1,10], log10 rho~U[7,9.5] (seed 4), lognormal-perturbed C/O start, "
@@ -305,7 +311,7 @@ def run_ours(args):
                 "steps": e2e_steps, "api": "net_integrate_host (pinned host buffers)"},
         "gpu_launches": args.steps,
         "roofline": {
-            "bound": "alu", "kernel": "zone_kernel<double, adaptive>", "achieved": fp64_ach,
+            "bound": "alu", "kernel": f"zone_kernel_pull<{'double' if args.precision == 64 else 'float'}, adaptive>", "achieved": fp64_ach,
             "peak": fp64_peak, "unit": "TFLOP/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
             "what": f"{flops} algorithmic FP64 ops per zone-substep x {per_launch_substeps} zone-substeps "
                     f"per launch / {k_ms:.2f} ms; peak = FP64 non-FMA issue rate, {peak_src}",
@@ -323,6 +329,58 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """Fig. 8 analogue (time against the number of concurrent networks)
+    and Fig. 6a analogue (L154-160: time per step against the network size), on one GPU.
+    Each point: 2 warm-up launches, best of 3 timed; one JSON line per point."""
+    import torch
+
+    import paper_1409_5826_b200 as K
+    from gen import co_start, make_hub_network, zone_profile
+
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream()
+
+    def time_point(net, T9h, rhoh, Y0h):
+        kn = K.Net(net)
+        z = len(T9h)
+        T9, rho = torch.from_numpy(T9h).to(dev), torch.from_numpy(rhoh).to(dev)
+        Y0 = torch.from_numpy(Y0h).to(dev)
+        Y, dt = torch.empty_like(Y0), torch.zeros(z, dtype=torch.float64, device=dev)
+        steps = torch.zeros(z, dtype=torch.int32, device=dev)
+        best = None
+        for it in range(5):
+            Y.copy_(Y0)
+            dt.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            kn.net_integrate(z, T9, rho, Y, T_HYDRO, dt, steps, None, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if it >= 2:
+                ms = e0.elapsed_time(e1)
+                best = ms if best is None else min(best, ms)
+        return best, int(steps.sum().item()), kn.schedule_info()
+
+    if args.sweep == "zones":
+        net, T9h, rhoh, Y0h = workload(0, 1)
+        for z in (1, 16, 74, 148, 296, 444, 445, 592, 888, 1776, 4096, 16384):
+            ms, sub, info = time_point(net, T9h[:z].copy(), rhoh[:z].copy(), Y0h[:z].copy())
+            print(json.dumps({"sweep": "zones", "zones": z, "ms": ms, "sub_steps": sub,
+                              "zone_networks_per_s": z / (ms * 1e-3),
+                              "zone_substeps_per_s": sub / (ms * 1e-3), "zones_per_sm": info["zones_per_sm"]}))
+    else:
+        for N, M in ((32, 330), (48, 500), (96, 1020), (150, 1604), (250, 2900), (365, 4400)):
+            net = make_hub_network(N, M, seed=N)
+            z = 4096
+            T9h, rhoh = zone_profile(z, 6)
+            ms, sub, info = time_point(net, T9h, rhoh, co_start(net, z))
+            print(json.dumps({"sweep": "size", "n_species": N, "n_reactions": M, "zones": z, "ms": ms,
+                              "sub_steps": sub, "ns_per_zone_substep": ms * 1e6 / sub,
+                              "kernel": "pull" if info["kernel"] == 1 else "generic",
+                              "threads_per_zone": info["threads"], "zones_per_sm": info["zones_per_sm"]}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -332,9 +390,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--zones", type=int, default=ZONES_PER_GPU,
                     help="zones per GPU (profiling only; the metric is quoted at the default)")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
+                    help="32 = the paper's single-precision study (PAPER.md L132); the metric is fp64")
+    ap.add_argument("--sweep", choices=["zones", "size"],
+                    help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
+                         "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.sweep:
+        run_sweep(args)
     else:
         run_ours(args)
 
