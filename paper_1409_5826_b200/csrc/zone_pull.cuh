@@ -538,7 +538,7 @@ pull_fn pick_pull_block(int T) {
     switch (T) {
         case 32: return zone_kernel_pull<real, 32, 12, CP, J2, ADAPT>;
         case 64: return zone_kernel_pull<real, 64, 6, CP, J2, ADAPT>;
-        case 160: return zone_kernel_pull<real, 160, KINNET_MINB160, CP, J2, ADAPT>;
+        case 160: return zone_kernel_pull<real, 160, sizeof(real) == 8 ? KINNET_MINB160 : KINNET_MINB160 + 1, CP, J2, ADAPT>;  // fp32 state halves the rate registers
         case 256: return zone_kernel_pull<real, 256, 2, CP, J2, ADAPT>;
         case 384: return zone_kernel_pull<real, 384, 1, CP, J2, ADAPT>;
         default: return zone_kernel_pull<real, 512, 1, CP, J2, ADAPT>;
