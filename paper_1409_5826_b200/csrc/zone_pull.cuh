@@ -36,9 +36,10 @@ enum Mode { kAdaptive = 0, kFixed = 1, kRhs = 2, kRates = 3 };
 constexpr int kJ2C = kinnet::kPullMaxSlots2;
 // P-slot rates beyond the first CP - kPullSpillSlots of a thread live in shared memory:
 // only the warp with the longest rows reaches them (the species are dealt to threads by
-// falling in-degree), and every thread gets the registers back.
+// falling in-degree), and every thread gets the registers back.  Measured on configs[3]
+// (zone-networks/s): 0 -> 161.7k, 4 -> 172.7k, 8 -> 165.0k, 12 -> 171.2k, 16 -> 173.1k.
 #ifndef KINNET_SPILL_SLOTS
-#define KINNET_SPILL_SLOTS 8
+#define KINNET_SPILL_SLOTS 4
 #endif
 constexpr int kPullSpillSlots = KINNET_SPILL_SLOTS;
 
