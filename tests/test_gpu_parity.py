@@ -340,3 +340,39 @@ def test_fp32_variant_report(hub150, capsys):
               f"{o32['n_steps'].sum()}/{o64['n_steps'].sum()}")
     assert np.median(dev_gpu) < 1e-3 and dev_gpu.max() < 0.2
     assert abs(int(g32["n_steps"].sum()) - int(o32["n_steps"].sum())) < 0.05 * o32["n_steps"].sum()
+
+
+# ------------------------------------------- every block-size class of the pull kernel
+@pytest.mark.parametrize("N,M,threads", [(32, 330, 32), (48, 500, 64), (96, 1020, 160), (250, 2900, 256),
+                                         (365, 4400, 384), (400, 4700, 512)])
+def test_pull_kernel_block_size_classes(N, M, threads):
+    """The pull kernel is instantiated per block-size x slot-capacity class; each class
+    runs rhs parity (1e-12), a fixed-dt run (1e-9) and an adaptive hydro step (1e-6,
+    steps within 1 %) on a seeded hub network of that size, 5 ragged zones."""
+    from gen import co_start, make_hub_network, zone_profile
+
+    net = make_hub_network(N, M, seed=N)
+    kn, o = K.Net(net), Oracle(net)
+    info = kn.schedule_info()
+    assert info["kernel"] == 1 and info["threads"] == threads, info
+    z = 5
+    T9, rho = zone_profile(z, 77)
+    Y0 = co_start(net, z)
+    # fixed dt, both branches
+    ref = o.integrate_fixed(T9, rho, Y0, 1e-9, 200)
+    assert ref["n_asym"].sum() > 0
+    err, _ = max_rel_err(gpu_fixed(kn, T9, rho, Y0, 1e-9, 200), ref["Y"], net.A)
+    assert err <= FIXED_TOL, err
+    # rhs on the evolved state
+    Fp = torch.zeros(z, N, dtype=torch.float64, device=DEV)
+    Fm = torch.zeros_like(Fp)
+    kn.net_rhs(z, dev(T9), dev(rho), dev(ref["Y"]), Fp, Fm)
+    torch.cuda.synchronize()
+    for q in range(z):
+        _, Fpo, Fmo = o.rhs(o.rates(T9[q], rho[q]), ref["Y"][q])
+        np.testing.assert_allclose(Fp[q].cpu().numpy(), Fpo, rtol=1e-12, atol=1e-300)
+        np.testing.assert_allclose(Fm[q].cpu().numpy(), Fmo, rtol=1e-12, atol=1e-300)
+    # adaptive
+    refa, delta, dsteps = oracle_with_conditioning(net, T9, rho, Y0, 1e-7)
+    g = gpu_integrate(kn, T9, rho, Y0, 1e-7)
+    print(N, check_adaptive(g, refa, delta, dsteps, net.A, f"N={N}", min_well=0.6))
