@@ -198,7 +198,7 @@ def run_ours(args):
 
     net, T9h, rhoh, Y0h = workload(rank, world, args.zones)
     z, N = Y0h.shape
-    kn = K.Net(net, K.NetParams(precision=args.precision))
+    kn = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel))
     info = kn.schedule_info()
     ynp = np.float64 if args.precision == 64 else np.float32
     ybytes = 8 if args.precision == 64 else 4
@@ -392,6 +392,9 @@ def main():
                     help="zones per GPU (profiling only; the metric is quoted at the default)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
                     help="32 = the paper's single-precision study (PAPER.md L132); the metric is fp64")
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2],
+                    help="net_params_t.kernel: 0 = automatic, 1 = generic flux-array kernel, "
+                         "2 = two-species-per-thread pull kernel (A/B runs)")
     ap.add_argument("--sweep", choices=["zones", "size"],
                     help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
                          "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")

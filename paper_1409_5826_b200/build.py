@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libkinnet.so")
-HEADERS = [os.path.join(CSRC, h) for h in ("schedule.h", "zone_pull.cuh", "device_util.cuh")] + [
+HEADERS = [os.path.join(CSRC, h) for h in ("schedule.h", "zone_pull.cuh", "zone_pull2.cuh", "device_util.cuh")] + [
     os.path.join(HERE, "..", "include", "kinnet.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2,-Wall",
@@ -28,6 +28,12 @@ UNITS = [
     (f"pull_f{bits}_{mode}.o", "pull_inst.cu",
      [f"-DPULL_REAL={real}", f"-DPULL_ADAPT={int(mode == 'adaptive')}",
       f"-DPULL_FN=pull_kernel_f{bits}_{mode}"])
+    for bits, real in ((64, "double"), (32, "float")) for mode in ("adaptive", "fixed")
+] + [
+    (f"pull2_f{bits}_{mode}.o", "pull2_inst.cu",
+     [f"-DPULL_REAL={real}", f"-DPULL_ADAPT={int(mode == 'adaptive')}",
+      f"-DPULL_FN=pull2_kernel_f{bits}_{mode}",
+      *(["-DPULL2_DEFINE_SUPPORTED"] if (bits, mode) == (64, "adaptive") else [])])
     for bits, real in ((64, "double"), (32, "float")) for mode in ("adaptive", "fixed")
 ]
 

@@ -30,6 +30,7 @@
 #include "device_util.cuh"
 #include "schedule.h"
 #include "zone_pull.cuh"
+#include "zone_pull2.cuh"
 
 namespace {
 
@@ -301,6 +302,56 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
 }
 
 
+// Launch order of the zones: hottest first.  The number of sub-steps a zone needs over
+// one hydro step grows steeply with its temperature (rates are exponential in T9; on
+// configs[3] 12 .. 7900 sub-steps, rank correlation with T9 0.99), and the block scheduler
+// hands out CTAs in index order, so in caller order the long zones that happen to start
+// late run alone on their SMs at the end.  Longest-processing-time-first on the T9 proxy
+// removes that tail (PAPER.md L200 leaves the load balance of unequal networks open).  A
+// counting sort on T9 quantised to 1/64 (one CTA, shared-memory histogram); the order
+// inside a bucket is whatever the atomics give -- it only moves WHEN a zone runs, never
+// what it computes.
+constexpr int kOrderBuckets = 1024;
+constexpr int kOrderMinZones = 1024;
+__global__ void __launch_bounds__(1024) zone_order_kernel(const double* T9, int zones, int* order) {
+    __shared__ int hist[kOrderBuckets];
+    __shared__ int warp_tot[32];
+    const int tid = threadIdx.x;
+    hist[tid] = 0;
+    __syncthreads();
+    auto bucket = [](double t9) {  // descending temperature -> ascending bucket; NaN and <= 0 last
+        const double k = t9 * 64.0;
+        int b = (k > 0.0) ? (k < 1023.0 ? static_cast<int>(k) : 1023) : 0;
+        return kOrderBuckets - 1 - b;
+    };
+    for (int z = tid; z < zones; z += 1024) atomicAdd(&hist[bucket(T9[z])], 1);
+    __syncthreads();
+    // exclusive scan of the 1024 counts: warp scan + scan of the 32 warp totals
+    const int lane = tid & 31, warp = tid >> 5;
+    const int mine = hist[tid];
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
+    }
+    if (lane == 31) warp_tot[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        int w = warp_tot[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += up;
+        }
+        warp_tot[lane] = w - warp_tot[lane];  // exclusive
+    }
+    __syncthreads();
+    hist[tid] = warp_tot[warp] + incl - mine;
+    __syncthreads();
+    for (int z = tid; z < zones; z += 1024) order[atomicAdd(&hist[bucket(T9[z])], 1)] = z;
+}
+
 struct DeviceTables {
     int32_t* flux_rxn = nullptr;
     ushort4* flux_react = nullptr;
@@ -330,9 +381,13 @@ struct net {
     net_params_t P;
     bool has_device = false;
     bool force_generic = false;  // params.kernel == 1: keep the table-driven kernel (A/B tests)
+    bool pull2 = false;          // PS is compiled for virtual threads: two species per thread
+    int pull2_spill = 0;         // side-a slot rates kept in shared memory by that kernel
     int device = -1;
     int zones_per_sm = 0;
     DeviceTables D;
+    int* d_order = nullptr;  // launch order scratch of net_integrate, grown on demand
+    int order_cap = 0;
     // scratch of net_integrate_host
     cudaStream_t host_stream = nullptr;
     int scratch_zones = 0;
@@ -362,7 +417,16 @@ kernel_fn pick_block(int T) {
 
 bool use_pull_kernel(const net* n) { return n->PS.ok && !n->force_generic; }
 
+int pull_block(const net* n) { return n->pull2 ? n->PS.T / 2 : n->PS.T; }
+
 pull_fn pick_pull(const net* n, bool adaptive) {
+    if (n->pull2) {
+        if (adaptive)
+            return n->P.precision == 32 ? kinnet::pull2_kernel_f32_adaptive(n->PS)
+                                        : kinnet::pull2_kernel_f64_adaptive(n->PS);
+        return n->P.precision == 32 ? kinnet::pull2_kernel_f32_fixed(n->PS)
+                                    : kinnet::pull2_kernel_f64_fixed(n->PS);
+    }
     if (adaptive)
         return n->P.precision == 32 ? kinnet::pull_kernel_f32_adaptive(n->PS)
                                     : kinnet::pull_kernel_f64_adaptive(n->PS);
@@ -371,6 +435,10 @@ pull_fn pick_pull(const net* n, bool adaptive) {
 }
 
 size_t pull_smem(const net* n) {
+    if (n->pull2)
+        return n->P.precision == 32
+                   ? kinnet::pull2_smem_bytes<float>(n->PS.T / 2, n->S.M, n->pull2_spill)
+                   : kinnet::pull2_smem_bytes<double>(n->PS.T / 2, n->S.M, n->pull2_spill);
     return n->P.precision == 32 ? pull_smem_bytes<float>(n->PS.T, n->PS.W, n->S.M)
                                 : pull_smem_bytes<double>(n->PS.T, n->PS.W, n->S.M);
 }
@@ -404,7 +472,7 @@ int prepare_kernels(net* n) {
                                       static_cast<int>(pull_smem(n))));
         CUDA_TRY(cudaFuncSetAttribute(f2, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       static_cast<int>(pull_smem(n))));
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, n->PS.T, pull_smem(n)));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, pull_block(n), pull_smem(n)));
     } else {
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
             &nb, reinterpret_cast<const void*>(fns[0]), n->S.T, smem));
@@ -432,7 +500,7 @@ void fill_pull(const net* n, KPull& k) {
 
 int launch_pull(net* n, int zones, KPull& k, void* stream) {
     pull_fn f = pick_pull(n, k.mode == kAdaptive);
-    f<<<zones, n->PS.T, pull_smem(n), static_cast<cudaStream_t>(stream)>>>(k);
+    f<<<zones, pull_block(n), pull_smem(n), static_cast<cudaStream_t>(stream)>>>(k);
     CUDA_TRY(cudaGetLastError());
     return NET_OK;
 }
@@ -555,6 +623,22 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         delete n;
         return fail(NET_ENOMEM, "out of host memory");
     }
+    if (n->P.kernel == 2 && n->PS.ok) {  // two species per thread, when an instantiation covers it
+        kinnet::PullSchedule P2;
+        try {
+            kinnet::build_pull_schedule(N, M, n_react, react, n_prod, prod,
+                                        n->P.precision == 32 ? 4 : 8, P2, (N + 63) / 64 * 64);
+        } catch (const std::bad_alloc&) {
+            delete n;
+            return fail(NET_ENOMEM, "out of host memory");
+        }
+        int spill = 0;
+        if (P2.ok && kinnet::pull2_supported(P2, &spill)) {
+            n->PS = P2;
+            n->pull2 = true;
+            n->pull2_spill = spill;
+        }
+    }
     if (net_smem(n) > 227 * 1024) {
         delete n;
         return fail(NET_EINVAL, "network too large for one CTA's shared memory");
@@ -629,7 +713,7 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.p_slot_rxn); cudaFree(n->D.p_f1); cudaFree(n->D.p_f2);
         cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
-        cudaFree(n->ssteps); cudaFree(n->sstatus);
+        cudaFree(n->ssteps); cudaFree(n->sstatus); cudaFree(n->d_order);
         if (n->host_stream) cudaStreamDestroy(n->host_stream);
     }
     delete n;
@@ -649,6 +733,18 @@ int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void
         q.mode = kAdaptive;
         q.T9 = T9; q.rho = rho; q.Y = Y; q.dt = dt; q.n_steps = n_steps; q.status = status;
         q.t_hydro = t_hydro;
+        if (zones >= kOrderMinZones) {  // more zones than a couple of waves: hottest first
+            if (zones > n->order_cap) {
+                cudaFree(n->d_order);
+                n->d_order = nullptr;
+                n->order_cap = 0;
+                CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->d_order), sizeof(int) * zones));
+                n->order_cap = zones;
+            }
+            zone_order_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(stream)>>>(T9, zones, n->d_order);
+            CUDA_TRY(cudaGetLastError());
+            q.order = n->d_order;
+        }
         return launch_pull(n, zones, q, stream);
     }
     KParams k;
@@ -756,7 +852,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     const Schedule& S = n->S;
     info->n_species = S.N;
     info->n_reactions = S.M;
-    info->threads = use_pull_kernel(n) ? n->PS.T : S.T;
+    info->threads = use_pull_kernel(n) ? pull_block(n) : S.T;
     info->flux_slots = S.rs;
     info->slots_2body = S.j2;
     info->slots_3body = S.j3;
@@ -767,7 +863,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     info->readback_max = S.readback_max;
     info->smem_bytes = static_cast<int>(net_smem(n));
     info->zones_per_sm = n->zones_per_sm;
-    info->kernel = use_pull_kernel(n) ? 1 : 0;
+    info->kernel = use_pull_kernel(n) ? (n->pull2 ? 2 : 1) : 0;
     info->pull_ok = n->PS.ok ? 1 : 0;
     info->pull_hubs = n->PS.nbs;
     info->pull_slots = n->PS.slots;

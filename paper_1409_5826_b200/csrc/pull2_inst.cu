@@ -1,0 +1,22 @@
+// pull2_inst.cu -- the two-species-per-thread pull kernel instantiated for one
+// (state type, mode) pair; compiled four times by build.py like pull_inst.cu, with
+//   -DPULL_REAL=double|float -DPULL_ADAPT=1|0 -DPULL_FN=pull2_kernel_f{64,32}_{adaptive,fixed}
+#define KINNET_PULL_INSTANTIATE
+#include "zone_pull2.cuh"
+
+#if !defined(PULL_REAL) || !defined(PULL_ADAPT) || !defined(PULL_FN)
+#error "compile with -DPULL_REAL=... -DPULL_ADAPT=... -DPULL_FN=..."
+#endif
+
+namespace kinnet {
+
+pull_fn PULL_FN(const PullSchedule& P) { return pick_pull2<PULL_REAL, PULL_ADAPT != 0>(P); }
+
+#if PULL_ADAPT != 0 && defined(PULL2_DEFINE_SUPPORTED)
+bool pull2_supported(const PullSchedule& P, int* spill) {
+    if (spill) *spill = KINNET_P2_SPA + KINNET_P2_SPB;
+    return pick_pull2<double, true>(P) != nullptr;
+}
+#endif
+
+}  // namespace kinnet

@@ -400,7 +400,7 @@ void place_piece(const std::vector<std::vector<SlotT>>& slots, int t0, int lanes
 }  // namespace
 
 void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
-                         const int* prod, int elem_bytes, PullSchedule& P) {
+                         const int* prod, int elem_bytes, PullSchedule& P, int force_T) {
     P = PullSchedule();
     auto reject = [&](const std::string& why) {
         P.ok = false;
@@ -410,7 +410,8 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
     int T = 0;
     for (int cls : {32, 64, 160, 256, 384, 512})
         if (T == 0 && N <= cls) T = cls;
-    if (T == 0) return reject("more than 512 species");
+    if (force_T > 0) T = (force_T % 32 == 0 && force_T >= N) ? force_T : 0;
+    if (T == 0) return reject("more than 512 species (or a bad forced thread count)");
     P.T = T;
     P.W = T / 32;
     if (M > 65535) return reject("more than 65535 reactions");

@@ -113,7 +113,9 @@ struct PullSchedule {
 //   10..12 G0_h  reactions of this thread with hub h as a product and no hub co-reactant
 //   13..18 Gx_h,j  hub h as a product, one hub co-reactant: the j-th of the other two hubs
 // elem_bytes = size of one abundance (8 or 4): it fixes the shared-memory bank of a word.
+// force_T > 0 compiles for exactly that many (virtual) threads instead of the first block-size
+// class >= N (the two-species-per-thread kernel plays two virtual threads per thread).
 void build_pull_schedule(int N, int M, const int* n_react, const int* react, const int* n_prod,
-                         const int* prod, int elem_bytes, PullSchedule& out);
+                         const int* prod, int elem_bytes, PullSchedule& out, int force_T = 0);
 
 }  // namespace kinnet

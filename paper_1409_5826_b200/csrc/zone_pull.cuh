@@ -63,6 +63,7 @@ struct KPull {
     const int32_t* agg_ent;   // [agg_max][T]
     const double* T9;
     const double* rho;
+    const int* order;         // [zones] launch order (zone of CTA b), NULL = identity
     void* Y;
     double* dt;
     int* n_steps;
@@ -164,7 +165,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = p.N, M = p.M, nbs = p.nbs;
-    const int z = blockIdx.x;
+    const int z = p.order ? p.order[blockIdx.x] : blockIdx.x;
 
     double* redmin = reinterpret_cast<double*>(smem_raw);        // [32] per-warp dt minima
     real* red = reinterpret_cast<real*>(redmin + 32);            // [NW][8] per-warp hub-row sums

@@ -1,0 +1,516 @@
+// zone_pull2.cuh -- the pull kernel with TWO species per thread (internal).
+//
+// Same method, tables and shared-memory protocol as zone_pull.cuh; what changes is
+// the mapping: the pull schedule is compiled for 2*TB "virtual threads" and physical
+// thread (warp w, lane l) plays the virtual threads (w, l) -- side a, the rows with
+// many incoming reactions -- and (2*NW-1-w, l) -- side b, the short rows.  Why: one
+// sub-step is a chain of dependent FP64 operations at 8 clk each (profiles/r01d),
+// and a warp issues in order, so with one species per thread most issue slots of a
+// warp wait on its own previous instruction.  Two species per thread are two
+// independent chains in every phase (rate sums, gathers, update), the hub-row
+// shares of the two are added before ONE butterfly, and the redundant finalize runs
+// in NW = TB/32 warps instead of twice as many.
+#pragma once
+#include "zone_pull.cuh"
+
+namespace kinnet {
+
+// The G coefficients (hub F+ rows, C[10..18]) of both species live in shared memory: read
+// once per sub-step, conflict-free, they would otherwise hold 36 registers of the 168
+// that let four CTAs share an SM (16 K registers per scheduler: 3 warps of <= 168).
+constexpr int kPull2SmemCoefs = 9;
+
+template <typename real>
+__host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill) {  // spill = slot rates of both sides kept in shared memory
+    return 32 * sizeof(double) +
+           sizeof(real) * (static_cast<size_t>(TB / 32) * 8 + 8 * TB + 4 + static_cast<size_t>(spill) * TB +
+                           static_cast<size_t>(kPull2SmemCoefs) * 2 * TB) +
+           sizeof(double) * static_cast<size_t>(M);
+}
+
+pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P);
+pull_fn pull2_kernel_f64_fixed(const PullSchedule& P);
+pull_fn pull2_kernel_f32_adaptive(const PullSchedule& P);
+pull_fn pull2_kernel_f32_fixed(const PullSchedule& P);
+// slots of the two sides of a schedule compiled for virtual threads; false when no
+// instantiation covers it (the caller then compiles the one-species schedule)
+bool pull2_supported(const PullSchedule& P, int* spill);
+
+#ifdef KINNET_PULL_INSTANTIATE
+
+// One side (one species) of a thread: everything that is loop invariant.
+template <typename real, int CP, int CPR, int J2>
+struct PullSide {
+    real R[CPR > 0 ? CPR : 1];
+    real C[kPullCoefs - kPull2SmemCoefs];  // K by class; G0, Gx are in shared memory
+    uint32_t f1[CP / 2], f2[J2 / 2];
+    int wn, wn2, own;
+    uint32_t s_pub;
+};
+
+// k = F-/y and the six hub-row shares of one species (see zone_pull.cuh)
+template <typename real, int TV>
+__device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPull2SmemCoefs], uint32_t s_G,
+                                               real y, real p1, real p2, real p3, real yh0, real yh1,
+                                               real yh2, real& k, real (&share)[6]) {
+    real G[kPull2SmemCoefs];
+#pragma unroll
+    for (int j = 0; j < kPull2SmemCoefs; ++j) G[j] = lds_at<real>(s_G + j * TV * sizeof(real));
+    real e0 = fma(C[4], yh0, C[1]);
+    e0 = fma(C[5], yh1, e0);
+    e0 = fma(C[6], yh2, e0);
+    real e1 = fma(C[7], yh1, C[2]);
+    e1 = fma(C[8], yh2, e1);
+    const real e2 = fma(C[9], yh2, C[3]);
+    k = fma(yh0, e0, C[0]);
+    k = fma(yh1, e1, k);
+    k = fma(yh2, e2, k);
+    const real m0 = fma(C[4], yh0, e0);
+    real m1 = fma(C[5], yh0, e1);
+    m1 = fma(C[7], yh1, m1);
+    real m2 = fma(C[6], yh0, e2);
+    m2 = fma(C[8], yh1, m2);
+    m2 = fma(C[9], yh2, m2);
+    real g0 = fma(G[3], yh1, G[0]);
+    g0 = fma(G[4], yh2, g0);
+    real g1 = fma(G[5], yh0, G[1]);
+    g1 = fma(G[6], yh2, g1);
+    real g2 = fma(G[7], yh0, G[2]);
+    g2 = fma(G[8], yh1, g2);
+    share[0] = y * g0;
+    share[1] = y * g1;
+    share[2] = y * g2;
+    share[3] = p1 * m0;
+    share[4] = p2 * m1;
+    share[5] = p3 * m2;
+}
+
+template <typename real, int TB, int MINB, int CPA, int SPA, int CPB, int SPB, int J2, bool ADAPT>
+__global__ void __launch_bounds__(TB) __maxnreg__(65536 / (TB * MINB) / 8 * 8 > 255 ? 255 : 65536 / (TB * MINB) / 8 * 8)
+    zone_kernel_pull2(const KPull p) {
+    static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
+                  "slot capacities");
+    constexpr int T = TB, NW = TB / 32, TV = 2 * TB;  // physical threads, warps; virtual threads
+    constexpr int CPRA = CPA - SPA, CPRB = CPB - SPB;  // slots whose rate stays in a register
+    constexpr uint32_t SZ = sizeof(real);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = p.N, M = p.M, nbs = p.nbs;
+    const int z = p.order ? p.order[blockIdx.x] : blockIdx.x;
+    const int va = tid, vb = (2 * NW - 1 - warp) * 32 + lane;  // the two virtual threads played here
+
+    double* redq = reinterpret_cast<double*>(smem_raw);       // [32] per-warp q maxima, [16..18] own terms
+    real* red = reinterpret_cast<real*>(redq + 32);           // [NW][8] per-warp hub-row sums
+    real* YP = red + NW * 8;                                  // [4][TV] published products, then 1
+    real* Rx = YP + 4 * TV + 4;                               // [SPA + SPB][T] spilled slot rates
+    real* Gs = Rx + (SPA + SPB) * T;                                  // [9][TV] G0, Gx of every virtual thread
+    double* Rbuf = reinterpret_cast<double*>(Gs + kPull2SmemCoefs * TV);  // [M] rates, set-up only
+    uint32_t s_redq;
+    asm volatile("mov.u32 %0, %1;"
+                 : "=r"(s_redq)
+                 : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(smem_raw))));
+    const uint32_t s_red = s_redq + 32 * 8;
+    const uint32_t s_YP = s_red + NW * 8 * SZ;
+    const uint32_t s_Rx = s_YP + (4 * TV + 4) * SZ + tid * SZ;
+    const uint32_t s_own = s_redq + 16 * 8;
+    const uint32_t s_G = s_YP + (4 * TV + 4 + (SPA + SPB) * T) * SZ;
+    if (s_YP + (4 * TV + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
+
+    PullSide<real, CPA, CPRA, J2> A;
+    PullSide<real, CPB, CPRB, J2> B;
+#pragma unroll
+    for (int e = 0; e < CPA / 2; ++e) A.f1[e] = p.f1_pack[e * TV + va] + s_YP * 0x10001u;
+#pragma unroll
+    for (int e = 0; e < CPB / 2; ++e) B.f1[e] = p.f1_pack[e * TV + vb] + s_YP * 0x10001u;
+#pragma unroll
+    for (int e = 0; e < J2 / 2; ++e) {
+        A.f2[e] = p.f2_pack[e * TV + va] + s_YP * 0x10001u;
+        B.f2[e] = p.f2_pack[e * TV + vb] + s_YP * 0x10001u;
+    }
+    {
+        const uint32_t ca = p.cnt[va], cb = p.cnt[vb];
+        A.wn = __reduce_max_sync(0xffffffffu, ca & 255u);  // warp-wide trip counts
+        A.wn2 = __reduce_max_sync(0xffffffffu, (ca >> 8) & 255u);
+        B.wn = __reduce_max_sync(0xffffffffu, cb & 255u);
+        B.wn2 = __reduce_max_sync(0xffffffffu, (cb >> 8) & 255u);
+    }
+    A.s_pub = s_YP + va * SZ;
+    B.s_pub = s_YP + vb * SZ;
+
+    // ---- S1: rates, once per zone per call -----------
+    {
+        const double T9 = p.T9[z], rho = p.rho[z];
+        const double t13 = cbrt(T9);
+        const double t53 = T9 * t13 * t13;
+        const double lnT = log(T9), lnrho = log(rho);
+        for (int r = tid; r < M; r += T) {
+            const double* c = p.coef + r;
+            const double lnR = c[0] + c[1 * (size_t)M] / T9 + c[2 * (size_t)M] / t13 +
+                               c[3 * (size_t)M] * t13 + c[4 * (size_t)M] * T9 +
+                               c[5 * (size_t)M] * t53 + c[6 * (size_t)M] * lnT;
+            Rbuf[r] = exp(c[7 * (size_t)M] * lnrho + lnR);
+        }
+    }
+    if (tid < 4) YP[4 * TV + tid] = static_cast<real>(1);
+    __syncthreads();
+
+    auto slot_rate = [&](int e, int v) -> real {
+        const int32_t w = p.slot_rxn[e * TV + v];
+        return w < 0 ? static_cast<real>(0)
+                     : static_cast<real>(static_cast<double>(w >> 24) * Rbuf[w & 0xffffff]);
+    };
+#pragma unroll
+    for (int e = 0; e < CPA; ++e) {
+        const real r = slot_rate(e, va);
+        if (e < CPRA) A.R[e] = r;
+        else Rx[(e - CPRA) * T + tid] = r;
+    }
+#pragma unroll
+    for (int e = 0; e < CPB; ++e) {
+        const real r = slot_rate(e, vb);
+        if (e < CPRB) B.R[e] = r;
+        else Rx[(SPA + e - CPRB) * T + tid] = r;
+    }
+    auto rate_sums = [&](real (&C)[kPullCoefs - kPull2SmemCoefs], int v) {
+        int q = p.agg_ptr[v];
+#pragma unroll
+        for (int s = 0; s < kPullCoefs; ++s) {
+            const int qe = p.agg_ptr[(s + 1) * TV + v];
+            double acc = 0.0;
+            for (; q < qe; ++q) {  // fixed (reaction) order
+                const int32_t w = p.agg_ent[(size_t)q * TV + v];
+                acc += static_cast<double>(w >> 24) * Rbuf[w & 0xffffff];
+            }
+            if (s < kPullCoefs - kPull2SmemCoefs) C[s] = static_cast<real>(acc);
+            else Gs[(s - (kPullCoefs - kPull2SmemCoefs)) * TV + v] = static_cast<real>(acc);
+        }
+    };
+    rate_sums(A.C, va);
+    rate_sums(B.C, vb);
+
+    // ---- S6: zone state in ---------------------------------------------------------
+    real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
+    A.own = p.owner[va];
+    B.own = p.owner[vb];
+    const bool hub_owner = tid < nbs;  // hub h is owned by virtual thread h = side a of thread h
+    const bool plain_a = A.own >= 0 && !hub_owner, plain_b = B.own >= 0;
+    real ya = (A.own >= 0) ? Yg[A.own] : static_cast<real>(0);
+    real yb = (B.own >= 0) ? Yg[B.own] : static_cast<real>(0);
+    real yh0 = nbs > 0 ? Yg[p.hub[0]] : static_cast<real>(0);
+    real yh1 = nbs > 1 ? Yg[p.hub[1]] : static_cast<real>(0);
+    real yh2 = nbs > 2 ? Yg[p.hub[2]] : static_cast<real>(0);
+
+    const real kappa = static_cast<real>(p.kappa);
+    const real eps_y = static_cast<real>(p.eps_y);
+    const real y_floor = static_cast<real>(p.y_floor);
+    const real yfl_eps = eps_y * y_floor;
+    const double growth = p.growth, t_hydro = p.t_hydro;
+    const bool rhs_only = p.mode == kRhs;
+
+    double t = 0.0, q_prev = 0.0, dt_out = 0.0;
+    int steps = 0;
+    int status = 0;
+    bool run = true;
+    if (ADAPT) {
+        const double dt_in = p.dt ? p.dt[z] : 0.0;
+        run = t_hydro > 0.0;
+        dt_out = dt_in;  // nothing to do: the trial dt is returned unchanged
+        if (run) q_prev = 1.0 / ((dt_in > 0.0) ? dt_in : t_hydro);
+    } else if (!rhs_only) {
+        run = p.n_fixed > 0;
+    }
+    const int max_steps = ADAPT ? p.max_steps : p.n_fixed;
+    const double ginv = 1.0 / growth;
+    const double q_fixed = ADAPT ? 0.0 : 1.0 / p.dt_fixed;
+
+    while (run) {
+        // ---- publish y x {1, hubs}, both species -------------------------------------------
+        const real pa1 = ya * yh0, pa2 = ya * yh1, pa3 = ya * yh2;
+        const real pb1 = yb * yh0, pb2 = yb * yh1, pb3 = yb * yh2;
+        sts(A.s_pub, ya);
+        sts(B.s_pub, yb);
+        sts(A.s_pub + TV * SZ, pa1);
+        sts(B.s_pub + TV * SZ, pb1);
+        sts(A.s_pub + 2 * TV * SZ, pa2);
+        sts(B.s_pub + 2 * TV * SZ, pb2);
+        sts(A.s_pub + 3 * TV * SZ, pa3);
+        sts(B.s_pub + 3 * TV * SZ, pb3);
+
+        // ---- rate sums: k = F-/y (Eq. (1)) and the hub-row shares, added over the two ----------
+        real ka, kb, share[6];
+        {
+            real sb[6];
+            pull_rate_sums<real, TV>(A.C, s_G + va * SZ, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
+            pull_rate_sums<real, TV>(B.C, s_G + vb * SZ, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+#pragma unroll
+            for (int i = 0; i < 6; ++i) share[i] += sb[i];
+        }
+        if (hub_owner) sts(s_own + tid * SZ, ka * ya);  // own consumption in a hub-only reaction
+
+        real inva = 0, invb = 0;  // reciprocal factors of the dt candidates, off the critical path
+        if (ADAPT) {
+            inva = rcp_pos(ya > y_floor ? eps_y * ya : yfl_eps);
+            invb = rcp_pos(yb > y_floor ? eps_y * yb : yfl_eps);
+            if (!plain_a) inva = 0;  // hub owners are judged on their full rows in finalize
+            if (!plain_b) invb = 0;
+        }
+        __syncthreads();
+
+        // ---- S2+S3: P-slot gathers of both species, interleaved with the hub-row butterfly -----
+        real Fpa, Fpb;
+        {
+            real sa0, sa1, sa2, sa3, a0, a1, a2, a3;
+            real sb0 = 0, sb1 = 0, sb2 = 0, sb3 = 0, b0, b1, b2, b3;
+#define KINNET_LOADS(S, CP_, g, x0, x1, x2, x3)                                            \
+    if ((4 * (g) < CP_) && ((g) == 0 || 4 * (g) < S.wn)) {                                 \
+        const uint32_t w0 = S.f1[(2 * (g)) % (CP_ / 2)], w1 = S.f1[(2 * (g) + 1) % (CP_ / 2)]; \
+        x0 = lds_at<real>(lo16(w0));                                                       \
+        x1 = lds_at<real>(hi16(w0));                                                       \
+        x2 = lds_at<real>(lo16(w1));                                                       \
+        x3 = lds_at<real>(hi16(w1));                                                       \
+        if (4 * (g) < J2 && 4 * (g) < S.wn2) { /* second factors (three-body reactions) */ \
+            const uint32_t v0 = S.f2[(2 * (g)) % (J2 / 2)], v1 = S.f2[(2 * (g) + 1) % (J2 / 2)]; \
+            x0 *= lds_at<real>(lo16(v0));                                                  \
+            x1 *= lds_at<real>(hi16(v0));                                                  \
+            x2 *= lds_at<real>(lo16(v1));                                                  \
+            x3 *= lds_at<real>(hi16(v1));                                                  \
+        }                                                                                  \
+    }
+#define KINNET_XOFF(e) (static_cast<uint32_t>((e) >= CPRA ? (e) - CPRA : 0) * T * SZ)
+#define KINNET_FMAS_A(g)                                                        \
+    if ((g) == 0) {                                                             \
+        sa0 = A.R[0] * a0;                                                      \
+        sa1 = A.R[1] * a1;                                                      \
+        sa2 = A.R[2] * a2;                                                      \
+        sa3 = A.R[3] * a3;                                                      \
+    } else if (4 * (g) < CPRA && 4 * (g) < A.wn) {                              \
+        sa0 = fma(A.R[(4 * (g)) % CPRA], a0, sa0);                              \
+        sa1 = fma(A.R[(4 * (g) + 1) % CPRA], a1, sa1);                          \
+        sa2 = fma(A.R[(4 * (g) + 2) % CPRA], a2, sa2);                          \
+        sa3 = fma(A.R[(4 * (g) + 3) % CPRA], a3, sa3);                          \
+    } else if (4 * (g) < CPA && 4 * (g) < A.wn) {                               \
+        sa0 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g))), a0, sa0);          \
+        sa1 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 1)), a1, sa1);      \
+        sa2 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 2)), a2, sa2);      \
+        sa3 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 3)), a3, sa3);      \
+    }
+#define KINNET_XOFFB(e) (static_cast<uint32_t>(SPA + ((e) >= CPRB ? (e) - CPRB : 0)) * T * SZ)
+#define KINNET_FMAS_B(g)                                                        \
+    if (4 * (g) < CPRB && ((g) == 0 || 4 * (g) < B.wn)) {                       \
+        sb0 = fma(B.R[(4 * (g)) % CPRB], b0, sb0);                              \
+        sb1 = fma(B.R[(4 * (g) + 1) % CPRB], b1, sb1);                          \
+        sb2 = fma(B.R[(4 * (g) + 2) % CPRB], b2, sb2);                          \
+        sb3 = fma(B.R[(4 * (g) + 3) % CPRB], b3, sb3);                          \
+    } else if (4 * (g) < CPB && 4 * (g) < B.wn) {                               \
+        sb0 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g))), b0, sb0);         \
+        sb1 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 1)), b1, sb1);     \
+        sb2 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 2)), b2, sb2);     \
+        sb3 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 3)), b3, sb3);     \
+    }
+#define KINNET_STAGE(g)                               \
+    KINNET_LOADS(A, CPA, g, a0, a1, a2, a3)           \
+    KINNET_LOADS(B, CPB, g, b0, b1, b2, b3)
+#define KINNET_FMAS(g) \
+    KINNET_FMAS_A(g)   \
+    KINNET_FMAS_B(g)
+            static_assert(CPRA >= 4 && CPRB >= 4, "group 0 reads its rates from registers");
+            const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
+            // level 16 of the butterfly (rows 0..2 = F+ shares of the hubs, 3..5 = F- shares)
+            real r0 = __shfl_xor_sync(0xffffffffu, up16 ? share[0] : share[3], 16);
+            real r1 = __shfl_xor_sync(0xffffffffu, up16 ? share[1] : share[4], 16);
+            real r2 = __shfl_xor_sync(0xffffffffu, up16 ? share[2] : share[5], 16);
+            KINNET_STAGE(0)
+            const real b0_ = (up16 ? share[3] : share[0]) + r0;
+            const real b1_ = (up16 ? share[4] : share[1]) + r1;
+            const real b2_ = (up16 ? share[5] : share[2]) + r2;
+            r0 = __shfl_xor_sync(0xffffffffu, up8 ? b0_ : b1_, 8);  // level 8
+            r1 = __shfl_xor_sync(0xffffffffu, b2_, 8);
+            KINNET_FMAS(0)
+            KINNET_STAGE(1)
+            const real c0_ = (up8 ? b1_ : b0_) + r0;
+            const real c1_ = b2_ + r1;
+            r0 = __shfl_xor_sync(0xffffffffu, up4 ? c0_ : c1_, 4);  // level 4
+            KINNET_FMAS(1)
+            KINNET_STAGE(2)
+            real tot = (up4 ? c1_ : c0_) + r0;
+            r0 = __shfl_xor_sync(0xffffffffu, tot, 2);
+            KINNET_FMAS(2)
+            KINNET_STAGE(3)
+            tot += r0;
+            r0 = __shfl_xor_sync(0xffffffffu, tot, 1);
+            KINNET_FMAS(3)
+            KINNET_STAGE(4)
+            tot += r0;
+            KINNET_FMAS(4)
+            KINNET_STAGE(5)
+            KINNET_FMAS(5)
+#undef KINNET_STAGE
+#undef KINNET_FMAS
+#undef KINNET_FMAS_A
+#undef KINNET_FMAS_B
+#undef KINNET_LOADS
+#undef KINNET_XOFF
+#undef KINNET_XOFFB
+            // lanes 0, 8, 4, 16, 24, 20 hold the warp totals of rows 0, 1, 2, 3, 4, 5
+            const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
+            if ((lane & 3) == 0 && (lane & 12) != 12) sts(s_red + (warp * 8 + row) * SZ, tot);
+            Fpa = (sa0 + sa1) + (sa2 + sa3);
+            Fpb = (sb0 + sb1) + (sb2 + sb3);
+        }
+
+        // ---- S5: q candidates of the non-hub species: |F+ - F-| / (eps max(y, floor)) ------
+        const real cha = fma(-ka, ya, Fpa), chb = fma(-kb, yb, Fpb);
+        if (ADAPT) {
+            const real qa = abs_of(cha) * inva, qb = abs_of(chb) * invb;
+            const double c = warp_max_pos(static_cast<double>(qa > qb ? qa : qb));
+            if (lane == 0) sts(s_redq + warp * 8, c);
+        }
+        __syncthreads();
+
+        // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
+        const real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
+        real invh = 0;
+        double q_rem = 0.0, rem = 0.0;
+        if (ADAPT) {  // these depend on nothing the barrier waited for: they run beside the loads
+            invh = rcp_pos(yme > y_floor ? eps_y * yme : yfl_eps);
+            rem = t_hydro - t;
+            q_rem = rcp_pos(rem);
+        }
+        real hFp = 0, hFm = 0;
+        if (lane < nbs) {  // three active lanes: one wavefront per load instead of two
+            real vp[NW], vm[NW];
+#pragma unroll
+            for (int w = 0; w < NW; ++w) {
+                vp[w] = lds_at<real>(s_red + (w * 8 + lane) * SZ);
+                vm[w] = lds_at<real>(s_red + (w * 8 + 3 + lane) * SZ);
+            }
+            const real own_term = lds_at<real>(s_own + lane * SZ);
+#pragma unroll
+            for (int s = 1; s < NW; s *= 2)  // fixed pairwise order over warps (log depth)
+#pragma unroll
+                for (int w = 0; w + s < NW; w += 2 * s) {
+                    vp[w] += vp[w + s];
+                    vm[w] += vm[w + s];
+                }
+            hFp = vp[0];
+            hFm = vm[0] + own_term;
+        }
+        if (!ADAPT && rhs_only) {
+            real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
+            real* Fmo = reinterpret_cast<real*>(p.Fminus) + (size_t)z * N;
+            if (hub_owner) {
+                Fpo[A.own] = hFp;
+                Fmo[A.own] = hFm;
+            } else if (A.own >= 0) {
+                Fpo[A.own] = Fpa;
+                Fmo[A.own] = ka * ya;
+            }
+            if (B.own >= 0) {
+                Fpo[B.own] = Fpb;
+                Fmo[B.own] = kb * yb;
+            }
+            return;
+        }
+
+        double q, hd;
+        bool last;
+        if (ADAPT) {
+            double cand = 0.0;
+            if (lane >= 8 && lane < 8 + NW) cand = lds_at<double>(s_redq + (lane - 8) * 8);
+            const double qh = static_cast<double>(abs_of(hFp - hFm) * invh);
+            if (lane < nbs) cand = qh;
+            const double qmax = warp_max_pos(cand);
+            const double qg = q_prev * ginv;                 // growth cap: dt <= g dt_prev
+            const double q_ctrl = (qmax > qg) ? qmax : qg;   // a NaN candidate loses
+            last = q_ctrl <= q_rem * (1.0 / (1.0 - 1e-12));  // dt_ctrl >= rem (1 - 1e-12)
+            q = last ? q_rem : q_ctrl;
+            hd = last ? rem : rcp_pos(q_ctrl);
+            q_prev = q_ctrl;
+        } else {
+            q = q_fixed;
+            hd = p.dt_fixed;
+            last = (steps + 1 >= max_steps);
+        }
+        const real h = static_cast<real>(hd), qr = static_cast<real>(q);
+
+        // ---- S4: update (Eq. (3)), Eq. (3) as (y q + F+) / (q + k) -----------
+        real yna, ynb;
+        {
+            const real aa = fma(ya, qr, Fpa) * rcp_pos(qr + ka);
+            const real ab = fma(yb, qr, Fpb) * rcp_pos(qr + kb);
+            const real ea = fma(h, cha, ya), eb = fma(h, chb, yb);
+            yna = (ya > 0 && ka * h >= kappa) ? aa : ea;
+            ynb = (yb > 0 && kb * h >= kappa) ? ab : eb;
+        }
+        {  // hub species, on lanes 0..nbs-1 of every warp: Y (Y q + F+) / (Y q + F-)
+            const bool pos = yme > Tiny<real>::v();
+            const real den = fma(yme, qr, hFm);
+            const real as = fma(yme, qr, hFp) * (yme * rcp_pos(pos ? den : static_cast<real>(1)));
+            const real es = fma(h, hFp - hFm, yme);
+            real hn = (pos && h * hFm >= kappa * yme) ? as : es;
+            if (lane >= nbs) hn = 0;  // a missing hub reads as abundance 0
+            yh0 = __shfl_sync(0xffffffffu, hn, 0);
+            yh1 = __shfl_sync(0xffffffffu, hn, 1);
+            yh2 = __shfl_sync(0xffffffffu, hn, 2);
+            ya = hub_owner ? hn : yna;  // hub h lives on side a of thread h: warp 0, lane h
+            yb = ynb;
+        }
+        t = last ? t_hydro : t + hd;
+        ++steps;
+        if (last) run = false;
+        else if (ADAPT && steps >= max_steps) {
+            status |= NET_STATUS_MAX_STEPS;
+            run = false;
+        }
+    }
+    if (ADAPT && steps > 0) dt_out = 1.0 / q_prev;
+
+    // ---- S6: zone state out ------------------------------------------------------------------
+    const int bad = ((A.own >= 0) && !isfinite(static_cast<double>(ya))) ||
+                    ((B.own >= 0) && !isfinite(static_cast<double>(yb)));
+    if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    if (A.own >= 0) Yg[A.own] = ya;
+    if (B.own >= 0) Yg[B.own] = yb;
+    if (tid == 0) {
+        if (ADAPT && p.dt) p.dt[z] = dt_out;
+        if (p.n_steps) p.n_steps[z] = steps;
+        if (p.status) p.status[z] = status;
+    }
+}
+
+// Instantiations: physical block size (virtual threads / 2) x slot capacities of the
+// two sides.  MINB = CTAs per SM the register budget 65536 / (TB * MINB) is cut for.
+#ifndef KINNET_P2_MINB96
+#define KINNET_P2_MINB96 4
+#endif
+#ifndef KINNET_P2_SPA
+#define KINNET_P2_SPA 8
+#endif
+#ifndef KINNET_P2_SPB
+#define KINNET_P2_SPB 4
+#endif
+
+inline bool pull2_sides(const PullSchedule& P, int& slots_a, int& slots_b, int& slots2) {
+    if (!P.ok || P.T % 64 != 0) return false;
+    const int nwv = P.T / 32;
+    slots_a = slots_b = slots2 = 0;
+    for (int t = 0; t < P.T; ++t) {
+        int& dst = (t / 32 < nwv / 2) ? slots_a : slots_b;
+        dst = dst > P.n_slots[t] ? dst : P.n_slots[t];
+        slots2 = slots2 > P.n_slots2[t] ? slots2 : P.n_slots2[t];
+    }
+    return true;
+}
+
+template <typename real, bool ADAPT>
+pull_fn pick_pull2(const PullSchedule& P) {
+    int sa, sb, s2;
+    if (!pull2_sides(P, sa, sb, s2)) return nullptr;
+    if (P.T == 192 && sa <= 20 && sb <= 12 && s2 <= 4)
+        return zone_kernel_pull2<real, 96, KINNET_P2_MINB96, 20, KINNET_P2_SPA, 12, KINNET_P2_SPB, 4, ADAPT>;
+    return nullptr;
+}
+
+#endif  // KINNET_PULL_INSTANTIATE
+
+}  // namespace kinnet
