@@ -309,9 +309,11 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "api": "net_integrate_host (pinned host buffers)"},
-        "gpu_launches": args.steps,
+        "gpu_launches": 2 * args.steps,  # per step: the launch-order kernel and the zone kernel
         "roofline": {
-            "bound": "alu", "kernel": f"zone_kernel_pull<{'double' if args.precision == 64 else 'float'}, adaptive>", "achieved": fp64_ach,
+            "bound": "alu",
+            "kernel": {0: "zone_kernel", 1: "zone_kernel_pull", 2: "zone_kernel_pull2"}[info["kernel"]]
+                      + f"<{'double' if args.precision == 64 else 'float'}, adaptive>", "achieved": fp64_ach,
             "peak": fp64_peak, "unit": "TFLOP/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
             "what": f"{flops} algorithmic FP64 ops per zone-substep x {per_launch_substeps} zone-substeps "
                     f"per launch / {k_ms:.2f} ms; peak = FP64 non-FMA issue rate, {peak_src}",
@@ -377,7 +379,7 @@ def run_sweep(args):
             ms, sub, info = time_point(net, T9h, rhoh, co_start(net, z))
             print(json.dumps({"sweep": "size", "n_species": N, "n_reactions": M, "zones": z, "ms": ms,
                               "sub_steps": sub, "ns_per_zone_substep": ms * 1e6 / sub,
-                              "kernel": "pull" if info["kernel"] == 1 else "generic",
+                              "kernel": {0: "generic", 1: "pull (1 species/thread)", 2: "pull (2 species/thread)"}[info["kernel"]],
                               "threads_per_zone": info["threads"], "zones_per_sm": info["zones_per_sm"]}))
 
 
@@ -394,7 +396,7 @@ def main():
                     help="32 = the paper's single-precision study (PAPER.md L132); the metric is fp64")
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2],
                     help="net_params_t.kernel: 0 = automatic, 1 = generic flux-array kernel, "
-                         "2 = two-species-per-thread pull kernel (A/B runs)")
+                         "2 = one-species-per-thread pull kernel (A/B runs)")
     ap.add_argument("--sweep", choices=["zones", "size"],
                     help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
                          "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")

@@ -22,9 +22,12 @@
  *     failure.
  *   - "host" / "device" below says where a pointer must live.  The caller owns
  *     every array it passes.  net_create copies the host tables; the net_t owns
- *     its device copies.  net_integrate* allocate nothing, are asynchronous on
- *     `cuda_stream` (a cudaStream_t cast to void*, NULL = default stream) and
- *     never synchronise.  net_integrate_host is the synchronous end-to-end
+ *     its device copies.  net_integrate* are asynchronous on `cuda_stream` (a
+ *     cudaStream_t cast to void*, NULL = default stream) and never synchronise;
+ *     the only allocation is net_integrate's launch-order scratch (4 bytes per
+ *     zone, owned by the net_t, grown when a call brings more zones than any
+ *     before).  One net_t serves one stream at a time: calls on the same net_t
+ *     from different streams must be ordered by the caller.  net_integrate_host is the synchronous end-to-end
  *     variant taking host buffers.
  *   - Y is zone-major [zones * n_species], molar abundances Y_i = X_i / A_i
  *     (Eq. (2) with X the mass fraction); double when the net was
@@ -63,9 +66,11 @@ typedef struct {
     double growth;       /* dt control: dt may grow by at most this factor per step (2)   */
     long long max_steps; /* per call and zone (1e7)                                       */
     int precision;       /* 64 (default) or 32                                            */
-    int kernel;          /* 0 = automatic: pull kernel when the network qualifies (every reaction
-                            has at most one non-hub reactant); 1 = always the
-                            generic flux-array kernel (A/B tests and fallback) */
+    int kernel;          /* 0 = automatic: the two-species-per-thread pull kernel when an instantiation
+                            covers the network, else the one-species pull kernel when the network
+                            qualifies (every reaction has at most one non-hub reactant),
+                            else the generic flux-array kernel; 1 = always the generic kernel;
+                            2 = the one-species pull kernel when the network qualifies (A/B tests) */
 } net_params_t;
 
 /* Fill *p with the defaults listed above. */
@@ -152,7 +157,8 @@ typedef struct {
     int zones_per_sm;    /* co-resident CTAs per SM (0 without a device)             */
     /* the fields above except threads/smem_bytes/zones_per_sm describe the generic
        flux-array schedule; the ones below the pull schedule */
-    int kernel;          /* kernel net_integrate* will launch: 1 = pull, 0 = generic  */
+    int kernel;          /* kernel net_integrate* will launch: 0 = generic, 1 = pull (one species
+                            per thread), 2 = pull (two species per thread)             */
     int pull_ok;         /* the network qualifies for the pull kernel                 */
     int pull_hubs;       /* hub species tracked in registers by every thread (0..3)   */
     int pull_slots;      /* longest per-thread list of incoming reactions (P-slots)   */
@@ -160,6 +166,8 @@ typedef struct {
     int pull_agg_max;    /* longest per-thread rate-sum list                          */
     int pull_wavefronts;       /* predicted shared-memory wavefronts of the fp64 P-slot gathers */
     int pull_wavefronts_ideal; /* ... without bank conflicts                          */
+    int pull_threads;    /* (virtual) threads the pull tables are compiled for: = threads for
+                            kernel 1, 2 * threads for kernel 2 (a thread plays two of them) */
 } net_schedule_info_t;
 
 int net_schedule_info(const net_t *net, net_schedule_info_t *info);
@@ -176,7 +184,7 @@ int net_schedule_info(const net_t *net, net_schedule_info_t *info);
  *   "big_species" [n_big_species]
  *   "big_cnt"     [2*n_big_species*threads] readback entries of thread t for row 2*s+{0:+,1:-}
  *   "big_slot"    [readback_max*threads]   own flux slot of readback entry e of thread t
- * Pull schedule (only when pull_ok; T = threads, word = index into the published
+ * Pull schedule (only when pull_ok; T = pull_threads, word = index into the published
  * table YP[4][T] followed by the constant one at 4*T):
  *   "pull_hub"      [pull_hubs]            hub species; hub h is owned by thread h
  *   "pull_owner"    [T]                    species owned by thread t, -1 = none

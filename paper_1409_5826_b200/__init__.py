@@ -40,7 +40,7 @@ class net_schedule_info_t(C.Structure):
         "n_species", "n_reactions", "threads", "flux_slots", "slots_2body", "slots_3body",
         "n_entries", "n_big_species", "n_entries_big", "small_max", "readback_max", "smem_bytes",
         "zones_per_sm", "kernel", "pull_ok", "pull_hubs", "pull_slots", "pull_slots2",
-        "pull_agg_max", "pull_wavefronts", "pull_wavefronts_ideal")]
+        "pull_agg_max", "pull_wavefronts", "pull_wavefronts_ideal", "pull_threads")]
 
 
 class KinnetError(RuntimeError):
@@ -94,7 +94,7 @@ class NetParams:
     growth: float = 2.0
     max_steps: int = 10_000_000
     precision: int = 64
-    kernel: int = 0  # 0 = automatic, 1 = table-driven kernel only
+    kernel: int = 0  # 0 = automatic, 1 = generic kernel only, 2 = one-species pull kernel
 
     def to_c(self) -> net_params_t:
         return net_params_t(self.kappa, self.eps_y, self.y_floor, self.growth, self.max_steps,

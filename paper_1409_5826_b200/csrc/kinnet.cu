@@ -623,7 +623,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         delete n;
         return fail(NET_ENOMEM, "out of host memory");
     }
-    if (n->P.kernel == 2 && n->PS.ok) {  // two species per thread, when an instantiation covers it
+    if (n->P.kernel == 0 && n->PS.ok) {  // two species per thread, when an instantiation covers it
         kinnet::PullSchedule P2;
         try {
             kinnet::build_pull_schedule(N, M, n_react, react, n_prod, prod,
@@ -871,6 +871,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     info->pull_agg_max = n->PS.agg_max;
     info->pull_wavefronts = static_cast<int>(n->PS.conflict_wavefronts);
     info->pull_wavefronts_ideal = static_cast<int>(n->PS.ideal_wavefronts);
+    info->pull_threads = n->PS.ok ? n->PS.T : 0;
     return NET_OK;
 }
 

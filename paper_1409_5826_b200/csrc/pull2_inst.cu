@@ -14,8 +14,10 @@ pull_fn PULL_FN(const PullSchedule& P) { return pick_pull2<PULL_REAL, PULL_ADAPT
 
 #if PULL_ADAPT != 0 && defined(PULL2_DEFINE_SUPPORTED)
 bool pull2_supported(const PullSchedule& P, int* spill) {
-    if (spill) *spill = KINNET_P2_SPA + KINNET_P2_SPB;
-    return pick_pull2<double, true>(P) != nullptr;
+    int sa, sb, s2;
+    if (!pull2_sides(P, sa, sb, s2) || pick_pull2<double, true>(P) == nullptr) return false;
+    if (spill) *spill = pull2_cap_a(sa) - kPull2RegA + kPull2SpillB;
+    return true;
 }
 #endif
 

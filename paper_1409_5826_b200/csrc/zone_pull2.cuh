@@ -85,8 +85,11 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
     share[5] = p3 * m2;
 }
 
-template <typename real, int TB, int MINB, int CPA, int SPA, int CPB, int SPB, int J2, bool ADAPT>
-__global__ void __launch_bounds__(TB) __maxnreg__(65536 / (TB * MINB) / 8 * 8 > 255 ? 255 : 65536 / (TB * MINB) / 8 * 8)
+// Twelve warps per SM -- three per scheduler, whose 16 K registers then give each thread
+// 168 (ptxas derives exactly that from the launch bounds): four 96-thread CTAs, two
+// 192-thread ones.
+template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, bool ADAPT>
+__global__ void __launch_bounds__(TB, 384 / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
@@ -478,17 +481,12 @@ __global__ void __launch_bounds__(TB) __maxnreg__(65536 / (TB * MINB) / 8 * 8 > 
     }
 }
 
-// Instantiations: physical block size (virtual threads / 2) x slot capacities of the
-// two sides.  MINB = CTAs per SM the register budget 65536 / (TB * MINB) is cut for.
-#ifndef KINNET_P2_MINB96
-#define KINNET_P2_MINB96 4
-#endif
-#ifndef KINNET_P2_SPA
-#define KINNET_P2_SPA 8
-#endif
-#ifndef KINNET_P2_SPB
-#define KINNET_P2_SPB 4
-#endif
+// Instantiations: physical block size (virtual threads / 2) x slot capacity of side a x
+// second-factor capacity.  Twelve side-a and eight side-b slot rates stay in registers,
+// the rest in shared memory (measured on configs[3], zone-networks/s: a/b spill 8/4 ->
+// 216.7k, 8/8 -> 218.2k, 12/8 -> 206.8k, 4/4 -> 206.2k).  Networks outside these classes
+// run on the one-species kernel.
+constexpr int kPull2CapB = 12, kPull2SpillB = 4, kPull2RegA = 12;
 
 inline bool pull2_sides(const PullSchedule& P, int& slots_a, int& slots_b, int& slots2) {
     if (!P.ok || P.T % 64 != 0) return false;
@@ -501,14 +499,30 @@ inline bool pull2_sides(const PullSchedule& P, int& slots_a, int& slots_b, int& 
     }
     return true;
 }
+inline int pull2_cap_a(int slots_a) { return slots_a <= 20 ? 20 : 24; }
 
+template <typename real, int TB, int CPA, bool ADAPT>
+pull_fn pick_pull2_j2(int s2) {
+    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 4, ADAPT>;
+    return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, ADAPT>;
+}
+template <typename real, int TB, bool ADAPT>
+pull_fn pick_pull2_cap(int sa, int s2) {
+    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2);
+    return pick_pull2_j2<real, TB, 24, ADAPT>(s2);
+}
 template <typename real, bool ADAPT>
 pull_fn pick_pull2(const PullSchedule& P) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2)) return nullptr;
-    if (P.T == 192 && sa <= 20 && sb <= 12 && s2 <= 4)
-        return zone_kernel_pull2<real, 96, KINNET_P2_MINB96, 20, KINNET_P2_SPA, 12, KINNET_P2_SPB, 4, ADAPT>;
-    return nullptr;
+    if (sa > 24 || sb > kPull2CapB || s2 > kJ2C) return nullptr;
+    switch (P.T / 2) {
+        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2);
+        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2);
+        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2);
+        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2);
+        default: return nullptr;
+    }
 }
 
 #endif  // KINNET_PULL_INSTANTIATE

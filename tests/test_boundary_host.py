@@ -120,7 +120,7 @@ def schedule_entries(net, kn):
 @pytest.mark.parametrize("name", ["g16", "hub150", "hub365"])
 def test_schedule_round_trip(name):
     net = network(name)
-    kn = K.Net(net, host_only=True)
+    kn = K.Net(net, K.NetParams(kernel=1), host_only=True)  # the generic schedule
     got, info = schedule_entries(net, kn)
     want = expected_entries(net)
     assert got == want
@@ -150,7 +150,7 @@ def test_schedule_round_trip(name):
 
 def test_schedule_hub_rows_are_the_big_ones(hub150):
     """p, n, 4He have hundreds of fluxes, the rest a few tens."""
-    kn = K.Net(hub150, host_only=True)
+    kn = K.Net(hub150, K.NetParams(kernel=1), host_only=True)
     info = kn.schedule_info()
     assert list(kn.schedule_table("big_species")) == [0, 1, 2]
     assert info["n_entries_big"] > 0.35 * info["n_entries"]
@@ -162,7 +162,7 @@ def test_schedule_hub_rows_are_the_big_ones(hub150):
 def test_three_alpha_multiplicity_in_schedule():
     """3a -> C and back: the alpha rows receive the flux three times (S:Q2)."""
     net = make_toy([4, 12], [((0, 0, 0), (1,)), ((1,), (0, 0, 0))], [7.0, 0.5])
-    kn = K.Net(net, host_only=True)
+    kn = K.Net(net, K.NetParams(kernel=1), host_only=True)
     got, _ = schedule_entries(net, kn)
     assert got[(0, "-", 0)] == 3 and got[(0, "+", 1)] == 3 and got[(1, "+", 0)] == 1
 
@@ -178,7 +178,8 @@ def pull_entries(net, kn):
     G0/Gx give F+ of the hubs."""
     info = kn.schedule_info()
     assert info["pull_ok"] == 1
-    T = info["threads"]
+    T = info["pull_threads"]
+    assert T == info["threads"] * (2 if info["kernel"] == 2 else 1)
     hub = list(kn.schedule_table("pull_hub"))
     owner = kn.schedule_table("pull_owner")
     ns, ns2 = kn.schedule_table("pull_n_slots"), kn.schedule_table("pull_n_slots2")
@@ -229,13 +230,16 @@ def pull_entries(net, kn):
     return ent, info
 
 
+@pytest.mark.parametrize("kernel", [0, 2])
 @pytest.mark.parametrize("name", ["hub150", "hub365", "hub150+perm"])
-def test_pull_schedule_round_trip(name):
+def test_pull_schedule_round_trip(name, kernel):
+    """kernel = 0 compiles the schedule for virtual threads (two per thread, kernel 2 in
+    schedule_info) where an instantiation covers it; kernel = 2 asks for the one-species one."""
     net = network("hub150").permuted(7)[0] if name.endswith("+perm") else network(name)
-    kn = K.Net(net, host_only=True)
+    kn = K.Net(net, K.NetParams(kernel=kernel), host_only=True)
     got, info = pull_entries(net, kn)
     assert got == expected_entries(net)
-    assert info["kernel"] == 1 and info["pull_hubs"] == 3
+    assert info["kernel"] == (2 if kernel == 0 else 1) and info["pull_hubs"] == 3
     assert info["pull_wavefronts"] >= info["pull_wavefronts_ideal"] > 0
 
 
@@ -244,7 +248,7 @@ def test_pull_schedule_small_and_unsupported_networks(g16):
     net = make_toy([1, 1, 1], [((0,), (1,)), ((1,), (0,)), ((1,), (2,))], [2.0, 3.0, 0.5])
     kn = K.Net(net, host_only=True)
     got, info = pull_entries(net, kn)
-    assert got == expected_entries(net) and info["pull_hubs"] == 0 and info["kernel"] == 1
+    assert got == expected_entries(net) and info["pull_hubs"] == 0 and info["kernel"] in (1, 2)
     # two non-hub reactants: generic flux-array kernel
     info = K.Net(g16, host_only=True).schedule_info()
     assert info["pull_ok"] == 0 and info["kernel"] == 0

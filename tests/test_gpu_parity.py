@@ -241,17 +241,20 @@ def test_config5_large_network_sampled():
     print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, net.A, "config5"))
 
 
-def test_generic_kernel_on_a_pull_network(hub150):
-    """params.kernel = 1 keeps the flux-array kernel (the fallback of networks
-    that do not qualify for the pull kernel) on a network the pull kernel
-    normally takes: both must meet the same parity."""
+def test_every_kernel_on_a_pull_network(hub150):
+    """params.kernel selects the kernel: 0 = automatic (two species per thread here),
+    2 = the one-species pull kernel, 1 = the generic flux-array kernel (the fallback of
+    networks that do not qualify).  All three must meet the same parity on the same zones."""
     c = build_config(3, zones=24)
     ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
-    for kernel in (0, 1):
+    for kernel, runs in ((0, 2), (2, 1), (1, 0)):
         kn = K.Net(hub150, K.NetParams(kernel=kernel))
-        assert kn.schedule_info()["kernel"] == 1 - kernel
+        assert kn.schedule_info()["kernel"] == runs
         g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
         print(kernel, check_adaptive(g, ref, delta, dsteps, hub150.A, f"kernel={kernel}", min_well=0.5))
+        ref_f = Oracle(hub150).integrate_fixed(c["T9"], c["rho"], c["Y0"], 1e-9, 200)
+        err, _ = max_rel_err(gpu_fixed(kn, c["T9"], c["rho"], c["Y0"], 1e-9, 200), ref_f["Y"], hub150.A)
+        assert err <= FIXED_TOL, (kernel, err)
 
 
 # -------------------------------------------------------------- edge cases
@@ -343,18 +346,23 @@ def test_fp32_variant_report(hub150, capsys):
 
 
 # ------------------------------------------- every block-size class of the pull kernel
-@pytest.mark.parametrize("N,M,threads", [(32, 330, 32), (48, 500, 64), (96, 1020, 160), (250, 2900, 256),
-                                         (365, 4400, 384), (400, 4700, 512)])
-def test_pull_kernel_block_size_classes(N, M, threads):
-    """The pull kernel is instantiated per block-size x slot-capacity class; each class
+@pytest.mark.parametrize("N,M,kernel,runs,threads", [
+    # one species per thread (params.kernel = 2): every block-size class
+    (32, 330, 2, 1, 32), (48, 500, 2, 1, 64), (96, 1020, 2, 1, 160), (250, 2900, 2, 1, 256),
+    (365, 4400, 2, 1, 384), (400, 4700, 2, 1, 512),
+    # automatic: two species per thread where an instantiation exists, every block size of it
+    (96, 1020, 0, 2, 64), (150, 1604, 0, 2, 96), (250, 2900, 0, 2, 128), (365, 4400, 0, 2, 192),
+    (48, 500, 0, 1, 64), (400, 4700, 0, 1, 512)])
+def test_pull_kernel_block_size_classes(N, M, kernel, runs, threads):
+    """The pull kernels are instantiated per block-size x slot-capacity class; each class
     runs rhs parity (1e-12), a fixed-dt run (1e-9) and an adaptive hydro step (1e-6,
     steps within 1 %) on a seeded hub network of that size, 5 ragged zones."""
     from gen import co_start, make_hub_network, zone_profile
 
-    net = make_hub_network(N, M, seed=N)
-    kn, o = K.Net(net), Oracle(net)
+    net = make_hub_network(N, M, seed=N if N != 150 else 1409)
+    kn, o = K.Net(net, K.NetParams(kernel=kernel)), Oracle(net)
     info = kn.schedule_info()
-    assert info["kernel"] == 1 and info["threads"] == threads, info
+    assert info["kernel"] == runs and info["threads"] == threads, info
     z = 5
     T9, rho = zone_profile(z, 77)
     Y0 = co_start(net, z)
