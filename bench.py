@@ -28,7 +28,7 @@ UNIT = "zone-networks/s"
 ZONES_PER_GPU = 16384
 T_HYDRO = 1e-6
 PROFILE_SEED = 4
-DRAM_BYTES_PER_LAUNCH = 20342784
+DRAM_BYTES_PER_LAUNCH = 20463360
 
 # Algorithmic work per zone per sub-step: one multiply per
 # reactant of every reaction, one add per F+/F- entry, ~10 flops per species for
@@ -287,7 +287,7 @@ def run_ours(args):
     fp64_ach = flops * per_launch_substeps / (k_ms * 1e-3) / 1e12
     smem_ach = smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of one 16384-zone launch, from the
-    # ncu --set full capture summarised in profiles/r01d_pull_kernel.md (20.34 MB + 0 B)
+    # ncu --set full capture summarised in profiles/r01e_pull2_kernel.md (20.46 MB read + 3.8 KB written)
     traffic = DRAM_BYTES_PER_LAUNCH if z == ZONES_PER_GPU else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
