@@ -5,6 +5,7 @@ numpy arrays and holds none of the integrator's arithmetic.
 """
 from .network import Network, make_g16, make_hub_network, make_toy
 from .profiles import (
+    binding_energies,
     co_start,
     config1_state,
     perturbed_co_start,
@@ -17,6 +18,7 @@ __all__ = [
     "make_g16",
     "make_hub_network",
     "make_toy",
+    "binding_energies",
     "co_start",
     "config1_state",
     "perturbed_co_start",

@@ -35,6 +35,19 @@ def co_start(net: Network, zones: int) -> np.ndarray:
     return Y
 
 
+def binding_energies(net: Network, seed: int = 7) -> np.ndarray:
+    """Synthetic per-species binding energies B_i (MeV per nucleus) for the energy-release
+    output: a smooth liquid-drop-like curve in A with made-up coefficients plus seeded
+    isobar-to-isobar noise.  Not nuclear data: it only gives the energy test inputs with
+    the right size and sign structure (B/A rising to a plateau near A ~ 56)."""
+    rng = np.random.default_rng(seed)
+    A = net.A.astype(np.float64)
+    per_nucleon = 8.9 - 9.5 / np.cbrt(np.maximum(A, 1.0)) - 0.004 * np.abs(A - 56.0)
+    B = A * np.maximum(per_nucleon, 0.0) + rng.normal(0.0, 0.3, A.shape)
+    B[A <= 1] = 0.0  # free nucleons
+    return B
+
+
 def perturbed_co_start(net: Network, zones: int, seed: int, sigma: float = 0.1) -> np.ndarray:
     """Config 4: each non-zero Y_i times exp(sigma*N(0,1)), then / sum(A_i Y_i)."""
     rng = np.random.default_rng(seed)

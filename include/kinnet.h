@@ -119,6 +119,21 @@ void net_destroy(net_t *net);
 int net_integrate(net_t *net, int zones, const double *T9, const double *rho, void *Y,
                   double t_hydro, double *dt, int *n_steps, int *status, void *cuda_stream);
 
+/*
+ * Integrated energy release (the network returns the abundances, the
+ * energy released over the hydro step and the final timestep).  The paper gives no formula;
+ * DESIGN.md reading Q19: energy[z] = sum_i B_i * (Y_i(t_hydro) - Y_i(0)) with B a per-species
+ * binding-energy table supplied by the caller (units: those of B per mole of species, per
+ * gram of matter -- e.g. B in MeV gives MeV mol/g; multiply by N_A to get MeV/g).
+ *   net_set_binding_energy  B host [n_species]; copied; may be called again to replace it
+ *   net_integrate_energy    net_integrate plus energy device [zones] out (NULL = net_integrate);
+ *                           fails with NET_EINVAL if no table has been set
+ */
+int net_set_binding_energy(net_t *net, const double *B);
+int net_integrate_energy(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                         double t_hydro, double *dt, int *n_steps, int *status, double *energy,
+                         void *cuda_stream);
+
 /* Exactly n_steps sub-steps of size dt_fixed for every zone (parity mode). */
 int net_integrate_fixed(net_t *net, int zones, const double *T9, const double *rho, void *Y,
                         double dt_fixed, long long n_steps, void *cuda_stream);

@@ -147,6 +147,19 @@ class Oracle:
         assert rc == 0
         return dict(Y=Y, dt=dt_io, n_steps=n_steps, status=status, n_asym=n_asym)
 
+    @staticmethod
+    def energy(B, Y0, Y):
+        """Integrated energy release per zone (reading Q19), the
+        definition written out in fp64: E_z = sum_i B_i * (Y_i(t_hydro) - Y_i(0))."""
+        B = np.asarray(B, np.float64)
+        Y0 = np.atleast_2d(np.asarray(Y0, np.float64))
+        Y = np.atleast_2d(np.asarray(Y, np.float64))
+        E = np.zeros(Y.shape[0])
+        for z in range(Y.shape[0]):
+            for i in range(Y.shape[1]):  # species order
+                E[z] += B[i] * (Y[z, i] - Y0[z, i])
+        return E
+
     def integrate_fixed(self, T9, rho, Y, dt_fixed, n_steps, precision=64, n_threads=1):
         """Exactly n_steps sub-steps of dt_fixed.  Returns dict(Y, n_asym)."""
         Y = self._state(Y, precision)

@@ -22,7 +22,7 @@ NET_STATUS_MAX_STEPS, NET_STATUS_NONFINITE = 1, 2
 
 EXPORTS = (
     "net_default_params", "net_create", "net_create_host", "net_destroy", "net_integrate",
-    "net_integrate_fixed", "net_integrate_host", "net_rates", "net_rhs", "net_schedule_info",
+    "net_integrate_fixed", "net_integrate_host", "net_set_binding_energy", "net_integrate_energy", "net_rates", "net_rhs", "net_schedule_info",
     "net_schedule_table", "net_last_error",
 )
 
@@ -63,6 +63,8 @@ def _load() -> C.CDLL:
     lib.net_destroy.argtypes = [vp]
     lib.net_destroy.restype = None
     lib.net_integrate.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp]
+    lib.net_set_binding_energy.argtypes = [vp, dp]
+    lib.net_integrate_energy.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp, vp]
     lib.net_integrate_fixed.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, C.c_longlong, vp]
     lib.net_integrate_host.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp]
     lib.net_rates.argtypes = [vp, C.c_int, vp, vp, vp, vp]
@@ -176,6 +178,17 @@ class Net:
                       stream=None):
         _check(lib.net_integrate(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y), float(t_hydro),
                                  _ptr(dt), _ptr(n_steps), _ptr(status), _stream(stream)))
+
+    def net_set_binding_energy(self, B):
+        B = np.ascontiguousarray(B, np.float64)
+        assert B.shape == (self.N,)
+        _check(lib.net_set_binding_energy(self._h, B.ctypes.data_as(C.POINTER(C.c_double))))
+
+    def net_integrate_energy(self, zones, T9, rho, Y, t_hydro, dt=None, n_steps=None, status=None,
+                             energy=None, stream=None):
+        _check(lib.net_integrate_energy(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y),
+                                        float(t_hydro), _ptr(dt), _ptr(n_steps), _ptr(status),
+                                        _ptr(energy), _stream(stream)))
 
     def net_integrate_fixed(self, zones, T9, rho, Y, dt_fixed, n_steps, stream=None):
         _check(lib.net_integrate_fixed(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y),

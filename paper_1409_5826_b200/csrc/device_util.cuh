@@ -35,4 +35,21 @@ __device__ __forceinline__ double warp_max_pos(double c) {
     return __hiloint2double(static_cast<int>(mh), static_cast<int>(ml));
 }
 
+// Integrated energy release of one zone (reading Q19):
+// sum over the CTA of the per-thread terms B_i (Y_i - Y_i(0)), in a fixed order (warp
+// butterfly, then warps in index order).  scratch: >= 32 doubles of shared memory that
+// nobody else touches any more; every thread of the CTA must call.
+__device__ __forceinline__ void zone_energy_out(double e, double* scratch, double* out) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = (blockDim.x + 31) >> 5;
+    e = warp_sum(e);
+    __syncthreads();
+    if (lane == 0) scratch[warp] = e;
+    __syncthreads();
+    if (tid == 0) {
+        double s = 0.0;
+        for (int w = 0; w < nw; ++w) s += scratch[w];
+        *out = s;
+    }
+}
+
 }  // namespace kinnet

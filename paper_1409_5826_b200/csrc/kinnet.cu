@@ -82,6 +82,8 @@ struct KParams {
     double* dt;
     int* n_steps;
     int* status;
+    const double* bind;
+    double* energy;
     void* Fplus;
     void* Fminus;
     double* Rout;
@@ -293,6 +295,12 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
     // ---- S6: zone state out ----------------------------------------------
     const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    if (p.energy) {  // uniform; Yg still holds the start-of-call abundances
+        double e = 0.0;
+        for (int i = tid; i < N; i += T)
+            e += p.bind[i] * (static_cast<double>(Ybuf[i]) - static_cast<double>(Yg[i]));
+        kinnet::zone_energy_out(e, redmin, p.energy + z);
+    }
     for (int i = tid; i < N; i += T) Yg[i] = Ybuf[i];
     if (tid == 0) {
         if (MODE == kAdaptive && p.dt) p.dt[z] = dt_prev;
@@ -371,6 +379,7 @@ struct DeviceTables {
     uint32_t* p_f2 = nullptr;
     uint16_t* p_agg_ptr = nullptr;
     int32_t* p_agg_ent = nullptr;
+    double* bind = nullptr;  // [N] binding energies (net_set_binding_energy)
 };
 
 }  // namespace
@@ -711,7 +720,7 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.small_src); cudaFree(n->D.big_cnt); cudaFree(n->D.big_slot);
         cudaFree(n->D.coef_rxn); cudaFree(n->D.p_owner); cudaFree(n->D.p_cnt);
         cudaFree(n->D.p_slot_rxn); cudaFree(n->D.p_f1); cudaFree(n->D.p_f2);
-        cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent);
+        cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent); cudaFree(n->D.bind);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
         cudaFree(n->ssteps); cudaFree(n->sstatus); cudaFree(n->d_order);
         if (n->host_stream) cudaStreamDestroy(n->host_stream);
@@ -719,9 +728,27 @@ void net_destroy(net_t* n) {
     delete n;
 }
 
+int net_set_binding_energy(net_t* n, const double* B) {
+    if (!n || !B) return fail(NET_EINVAL, "null argument");
+    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    for (int i = 0; i < n->S.N; ++i)
+        if (!std::isfinite(B[i])) return fail(NET_EINVAL, "non-finite binding energy");
+    if (!n->D.bind) CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->D.bind), sizeof(double) * n->S.N));
+    CUDA_TRY(cudaMemcpy(n->D.bind, B, sizeof(double) * n->S.N, cudaMemcpyHostToDevice));
+    return NET_OK;
+}
+
 int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                   double t_hydro, double* dt, int* n_steps, int* status, void* stream) {
+    return net_integrate_energy(n, zones, T9, rho, Y, t_hydro, dt, n_steps, status, nullptr, stream);
+}
+
+int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                         double t_hydro, double* dt, int* n_steps, int* status, double* energy,
+                         void* stream) {
     if (!n) return fail(NET_EINVAL, "null net");
+    if (energy && !n->D.bind)
+        return fail(NET_EINVAL, "energy asked for before net_set_binding_energy");
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
     if (!(t_hydro == t_hydro)) return fail(NET_EINVAL, "t_hydro is NaN");
     if (n->has_device && use_pull_kernel(n)) {
@@ -733,6 +760,7 @@ int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void
         q.mode = kAdaptive;
         q.T9 = T9; q.rho = rho; q.Y = Y; q.dt = dt; q.n_steps = n_steps; q.status = status;
         q.t_hydro = t_hydro;
+        q.bind = n->D.bind; q.energy = energy;
         if (zones >= kOrderMinZones) {  // more zones than a couple of waves: hottest first
             if (zones > n->order_cap) {
                 cudaFree(n->d_order);
@@ -751,6 +779,7 @@ int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void
     fill_params(n, k);
     k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
     k.t_hydro = t_hydro;
+    k.bind = n->D.bind; k.energy = energy;
     return launch<kAdaptive>(n, zones, k, stream);
 }
 

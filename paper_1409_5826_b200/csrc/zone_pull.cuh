@@ -68,6 +68,8 @@ struct KPull {
     double* dt;
     int* n_steps;
     int* status;
+    const double* bind;       // [N] binding energies, NULL unless energy is asked for
+    double* energy;           // [zones] out: sum_i bind_i (Y_i - Y_i(0)), or NULL
     void* Fplus;
     void* Fminus;
     double t_hydro, dt_fixed;
@@ -524,6 +526,10 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     // ---- S6: zone state out ------------------------------------------------------------------
     const int bad = (own >= 0) && !isfinite(static_cast<double>(y));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    if (p.energy) {  // uniform; Yg still holds the start-of-call abundances
+        const double e = (own >= 0) ? p.bind[own] * (static_cast<double>(y) - static_cast<double>(Yg[own])) : 0.0;
+        zone_energy_out(e, redmin, p.energy + z);
+    }
     if (own >= 0) Yg[own] = y;
     if (tid == 0) {
         if (ADAPT && p.dt) p.dt[z] = dt_out;

@@ -472,6 +472,12 @@ __global__ void __launch_bounds__(TB, 384 / TB)
     const int bad = ((A.own >= 0) && !isfinite(static_cast<double>(ya))) ||
                     ((B.own >= 0) && !isfinite(static_cast<double>(yb)));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    if (p.energy) {  // uniform; Yg still holds the start-of-call abundances
+        double e = 0.0;
+        if (A.own >= 0) e = p.bind[A.own] * (static_cast<double>(ya) - static_cast<double>(Yg[A.own]));
+        if (B.own >= 0) e += p.bind[B.own] * (static_cast<double>(yb) - static_cast<double>(Yg[B.own]));
+        zone_energy_out(e, redq, p.energy + z);
+    }
     if (A.own >= 0) Yg[A.own] = ya;
     if (B.own >= 0) Yg[B.own] = yb;
     if (tid == 0) {

@@ -401,3 +401,38 @@ def test_pull_kernel_block_size_classes(N, M, kernel, runs, threads):
     refa, delta, dsteps = oracle_with_conditioning(net, T9, rho, Y0, 1e-7)
     g = gpu_integrate(kn, T9, rho, Y0, 1e-7)
     print(N, check_adaptive(g, refa, delta, dsteps, net.A, f"N={N}", min_well=0.6))
+
+
+# ------------------------------------------------------- energy release (reading Q19)
+@pytest.mark.parametrize("kernel", [0, 2, 1])
+def test_energy_release_parity(hub150, kernel):
+    """net_integrate_energy: E_z = sum_i B_i (Y_i(t_hydro) - Y_i(0)) on every kernel.  Two
+    comparisons: against the definition applied to the GPU's own abundances (only the
+    reduction order differs: 1e-12 of sum |terms|), and against the oracle's run (the
+    adaptive tolerance, scaled the same way).  2048 zones: the sorted launch path."""
+    from gen import binding_energies
+
+    c = build_config(4, zones=2048)
+    B = binding_energies(hub150)
+    kn = K.Net(hub150, K.NetParams(kernel=kernel))
+    z = c["zones"]
+    with pytest.raises(K.KinnetError):  # no table yet
+        kn.net_integrate_energy(z, dev(c["T9"]), dev(c["rho"]), dev(c["Y0"]), c["t_hydro"],
+                                energy=torch.zeros(z, dtype=torch.float64, device=DEV))
+    kn.net_set_binding_energy(B)
+    Yd, E = dev(c["Y0"]), torch.full((z,), np.nan, dtype=torch.float64, device=DEV)
+    steps = torch.zeros(z, dtype=torch.int32, device=DEV)
+    kn.net_integrate_energy(z, dev(c["T9"]), dev(c["rho"]), Yd, c["t_hydro"], None, steps, None, E)
+    torch.cuda.synchronize()
+    Yg, Eg = Yd.cpu().numpy(), E.cpu().numpy()
+    scale = (np.abs(B)[None, :] * np.abs(Yg - c["Y0"])).sum(axis=1)
+    assert (scale > 0).all() and np.isfinite(Eg).all()
+    assert (np.abs(Eg - Oracle.energy(B, c["Y0"], Yg)) <= 1e-12 * scale).all()
+    idx = np.arange(0, z, 16)  # the oracle's own run on a sample
+    ref = Oracle(hub150).integrate(c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"],
+                                   n_threads=max_threads())
+    Eo = Oracle.energy(B, c["Y0"][idx], ref["Y"])
+    same = steps.cpu().numpy()[idx] == ref["n_steps"]  # zones both sides stepped identically
+    assert same.mean() > 0.9
+    assert (np.abs(Eg[idx] - Eo)[same] <= 1e-6 * scale[idx][same]).all()
+    assert (Eg != 0).all()  # (the sign is a property of the synthetic rates and table, not asserted)

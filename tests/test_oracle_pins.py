@@ -393,3 +393,52 @@ def test_fp32_variant_tracks_fp64(hub150):
     m = X > 1e-12
     assert np.abs(b["Y"][0][m] / a["Y"][0][m] - 1).max() < 1e-2
     assert abs(int(a["n_steps"][0]) - int(b["n_steps"][0])) <= max(2, a["n_steps"][0] // 50)
+
+
+from gen import build_config  # noqa: E402
+
+
+# ---------------------------------------------------------------- energy release (Q19)
+def test_energy_single_decay_closed_form():
+    """A -> B with rate k, fixed dt in the Euler regime: Y_A(n) = Y0 (1 - k dt)^n exactly, so
+    E = (B_B - B_A) * Y0 * (1 - (1 - k dt)^n)."""
+    k, dt, n, y0 = 3.0, 0.01, 40, 0.25
+    net = make_toy([1, 1], [((0,), (1,))], [k])
+    o = Oracle(net)
+    Y0 = np.array([[y0, 0.0]])
+    out = o.integrate_fixed(1.0, 1.0, Y0, dt, n)
+    B = np.array([1.5, 9.25])
+    want = (B[1] - B[0]) * y0 * (1.0 - (1.0 - k * dt) ** n)
+    assert Oracle.energy(B, Y0, out["Y"])[0] == pytest.approx(want, rel=1e-13)
+
+
+def test_energy_is_sum_of_q_values_times_integrated_fluxes(g16):
+    """In the all-Euler regime dY_i = dt * sum_r nu_ir f_r, so the energy release equals
+    sum_r Q_r * (integrated flux of r) with Q_r = B(products) - B(reactants): an identity
+    through the reaction list, independent of the species sums the definition uses."""
+    c = build_config(1)
+    o = Oracle(g16)
+    rng = np.random.default_rng(5)
+    B = g16.A * 8.0 + rng.normal(0, 1.0, g16.n_species)
+    Q = np.array([sum(B[s] for s in g16.prod[r, :g16.n_prod[r]]) - sum(B[s] for s in g16.react[r, :g16.n_react[r]])
+                  for r in range(g16.n_reactions)])
+    R = o.rates(c["T9"][0], c["rho"][0])
+    Y = c["Y0"].copy()
+    dt, n, acc = 1e-10, 400, 0.0
+    for _ in range(n):
+        f, _, _ = o.rhs(R, Y[0])
+        acc += dt * float(Q @ f)
+        step = o.integrate_fixed(c["T9"], c["rho"], Y, dt, 1)
+        assert step["n_asym"][0] == 0
+        Y = step["Y"]
+    E = Oracle.energy(B, c["Y0"], Y)[0]
+    assert E != 0.0 and E == pytest.approx(acc, rel=1e-9)
+
+
+def test_energy_vanishes_when_binding_is_proportional_to_mass_number(g16):
+    """B_i = c A_i makes E = c * delta(sum A_i Y_i), which the Euler regime conserves (P5)."""
+    c = build_config(1)
+    out = Oracle(g16).integrate_fixed(c["T9"], c["rho"], c["Y0"], 1e-10, 2000)
+    assert out["n_asym"][0] == 0
+    E = Oracle.energy(7.5 * g16.A, c["Y0"], out["Y"])[0]
+    assert abs(E) < 1e-11
