@@ -87,9 +87,10 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 
 // Twelve warps per SM -- three per scheduler, whose 16 K registers then give each thread
 // 168 (ptxas derives exactly that from the launch bounds): four 96-thread CTAs, two
-// 192-thread ones.
+// 192-thread ones.  With fp32 state the rates take half the registers: 128 registers, four
+// warps per scheduler, five 96-thread CTAs (270k -> 300k zone-networks/s on configs[3]).
 template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, bool ADAPT>
-__global__ void __launch_bounds__(TB, 384 / TB)
+__global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
