@@ -16,21 +16,25 @@ namespace kinnet {
 enum Mode { kAdaptive = 0, kFixed = 1, kRhs = 2, kRates = 3 };
 
 // ---------------------------------------------------------------------------
-// Pull kernel (the one bench.py times when the network qualifies, see
-// schedule.h "Pull schedule"): no flux array, two barriers per sub-step.
+// Pull kernel, one species per thread (zone_pull2.cuh is its two-species form; see
+// schedule.h "Pull schedule" and DESIGN.md 4.2-4.3): no flux array, two barriers per
+// sub-step, the dt controller carried as q = 1/dt.
 //
 //   publish   YP[c][t] = y * {1, Y_hub0, Y_hub1, Y_hub2}[c]            4 STS
-//   rate sums k = F-/y and the six hub-row partials from the per-thread
-//             coefficients K, G0, Gx (sums of rates formed once per call)
-//   ------------------------------------------------------------------- barrier
-//   P-slots   F+ = sum_e R[e] * YP[f1[e]] (* YP[f2[e]])   fluxes at the consumer
-//   dt        candidate eps*max(y,floor)/|F+ - k y|, warp min -> redmin[warp]
-//   hub rows  transposed warp butterfly of the six partials -> red[warp][row]
-//   ------------------------------------------------------------------- barrier
+//   rate sums k = F-/y and the six hub-row shares from the per-thread
+//             coefficients K, G0, Gx (sums of rates formed once per call);
+//             inv = 1 / (eps max(y, floor)) for the dt candidate
+//   ------------------------------------------------------------------- barrier A
+//   P-slots   F+ = sum_e R[e] * YP[f1[e]] (* YP[f2[e]])   fluxes at the consumer,
+//   hub rows  interleaved with the transposed warp butterfly of the six shares
+//             -> red[warp][row]
+//   dt        candidate |F+ - k y| * inv, warp max -> redmin[warp]
+//   ------------------------------------------------------------------- barrier B
 //   finalize  every warp redundantly: lanes 0..2 sum the hub rows over warps,
-//             zone-wide dt, hub update, shuffle-broadcast of the new hub Y
-//   update    k dt >= kappa ? (y + dt F+)/(1 + k dt) : y + dt (F+ - k y)
-// Rates, rate sums and every gather offset of a thread stay in registers for
+//             zone-wide q = max(candidates, q_prev / g), end clamp, hub update,
+//             shuffle-broadcast of the new hub Y
+//   update    k dt >= kappa ? (y q + F+)/(q + k) : y + dt (F+ - k y)
+// Rates, rate sums and every gather address of a thread stay in registers for
 // the whole hydro step (topology is static, sub-steps number 1e2..1e4).
 // ---------------------------------------------------------------------------
 constexpr int kJ2C = kinnet::kPullMaxSlots2;
