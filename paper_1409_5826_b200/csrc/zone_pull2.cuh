@@ -527,6 +527,7 @@ pull_fn pick_pull2(const PullSchedule& P) {
         case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2);
         case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2);
         case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2);
+        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2);
         case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2);
         default: return nullptr;
     }
