@@ -524,6 +524,7 @@ pull_fn pick_pull2(const PullSchedule& P) {
     if (!pull2_sides(P, sa, sb, s2)) return nullptr;
     if (sa > 24 || sb > kPull2CapB || s2 > kJ2C) return nullptr;
     switch (P.T / 2) {
+        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2);
         case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2);
         case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2);
         case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2);

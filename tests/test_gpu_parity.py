@@ -368,9 +368,9 @@ def test_fp32_variant_report(hub150, capsys):
     (32, 330, 2, 1, 32), (48, 500, 2, 1, 64), (96, 1020, 2, 1, 160), (250, 2900, 2, 1, 256),
     (365, 4400, 2, 1, 384), (400, 4700, 2, 1, 512),
     # automatic: two species per thread where an instantiation exists, every block size of it
-    (96, 1020, 0, 2, 64), (150, 1604, 0, 2, 96), (250, 2900, 0, 2, 128), (300, 3400, 0, 2, 160),
+    (32, 330, 0, 1, 32), (48, 500, 0, 2, 32), (96, 1020, 0, 2, 64), (150, 1604, 0, 2, 96), (250, 2900, 0, 2, 128), (300, 3400, 0, 2, 160),
     (365, 4400, 0, 2, 192),
-    (48, 500, 0, 1, 64), (400, 4700, 0, 1, 512)])
+    (400, 4700, 0, 1, 512)])
 def test_pull_kernel_block_size_classes(N, M, kernel, runs, threads):
     """The pull kernels are instantiated per block-size x slot-capacity class; each class
     runs rhs parity (1e-12), a fixed-dt run (1e-9) and an adaptive hydro step (1e-6,
