@@ -437,3 +437,23 @@ def test_energy_release_parity(hub150, kernel):
     assert same.mean() > 0.9
     assert (np.abs(Eg[idx] - Eo)[same] <= 1e-6 * scale[idx][same]).all()
     assert (Eg != 0).all()  # (the sign is a property of the synthetic rates and table, not asserted)
+
+
+@pytest.mark.parametrize("kernel", [0, 2, 1])
+def test_non_default_integrator_parameters(hub150, kernel):
+    """kappa, eps_y, y_floor, growth and max_steps other than the defaults reach the kernels
+    (the growth cap 1.5 is not a power of two: q_prev / g and g * dt_prev round differently)."""
+    c = build_config(3, zones=12)
+    par = dict(kappa=2.0, eps_y=0.02, y_floor=1e-8, growth=1.5, max_steps=1_000_000)
+    net = hub150
+    o = Oracle(net, OracleParams(**par))
+    kn = K.Net(net, K.NetParams(kernel=kernel, **par))
+    ref = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], n_threads=max_threads())
+    g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    assert (g["status"] == 0).all()
+    same = g["n_steps"] == ref["n_steps"]
+    assert same.mean() >= 0.75 and (np.abs(g["n_steps"] - ref["n_steps"]) <= np.maximum(1, ref["n_steps"] // 100)).all()
+    err = zone_err(g["Y"], ref["Y"], net.A)
+    assert (err[same] <= ADAPT_TOL).all(), err
+    # the parameters do reach the integrator: the default ones take other step counts
+    assert (ref["n_steps"] != Oracle(net).integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"])["n_steps"]).all()
