@@ -122,7 +122,7 @@ class Oracle:
         return f, Fp, Fm
 
     def _state(self, Y, precision):
-        dt = np.float64 if precision == 64 else np.float32
+        dt = np.float32 if precision == 32 else np.float64  # 64, and 80 (the long-double arbiter)
         Y = np.array(Y, dtype=dt, order="C", copy=True)
         if Y.ndim == 1:
             Y = Y[None, :]

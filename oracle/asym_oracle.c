@@ -30,6 +30,15 @@
  * networks; P9 permutation invariance; P10 three-body multiplicity.
  * precision == 32 has no bound in the paper: PARITY UNPINNED for it.
  *
+ * precision == 80 is the ARBITER: the same O1-O9, textually the same sub-step, with
+ * Y, f, F+, F-, k, the update, the rates (cbrtl/logl/expl), t, dt and the dt minimum
+ * in x87 long double (64-bit significand).  It is not a different method and not a
+ * reference for the CUDA path's arithmetic; it answers one question in the parity
+ * tests: in a zone where the adaptive trajectory amplifies rounding,
+ * is the CUDA result as close to the extended-precision trajectory as the fp64
+ * oracle's own results are?  Abundances go in and come out as double.  Pinned by
+ * the same closed forms as precision 64 (tests/test_oracle_pins.py).
+ *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
  * OpenMP only runs independent zones on different cores; it never touches the
  * arithmetic of one zone.
@@ -66,6 +75,7 @@ typedef struct {
     int *n_react, *react; /* [M], [M*3] */
     double *coef;         /* [M*7]      */
     double *ln_pref;      /* [M] ln(1/prod m!) */
+    long double *ln_pref_ld; /* the same in long double (arbiter) */
     edge_t *edges;
     oracle_params p;
 } oracle_net;
@@ -81,6 +91,12 @@ void oracle_default_params(oracle_params *p) {
 static double ln_factorial(int m) {
     double s = 0.0;
     for (int q = 2; q <= m; ++q) s += log((double)q);
+    return s;
+}
+
+static long double ln_factorial_ld(int m) {
+    long double s = 0.0L;
+    for (int q = 2; q <= m; ++q) s += logl((long double)q);
     return s;
 }
 
@@ -114,6 +130,7 @@ void *oracle_create(int N, const int *A, int M, const int *n_react, const int *r
     net->react = (int *)malloc(sizeof(int) * (M * MAX_REACT + 1));
     net->coef = (double *)malloc(sizeof(double) * (M * N_COEF + 1));
     net->ln_pref = (double *)malloc(sizeof(double) * (M + 1));
+    net->ln_pref_ld = (long double *)malloc(sizeof(long double) * (M + 1));
     net->edges = (edge_t *)malloc(sizeof(edge_t) * (M * (MAX_REACT + MAX_PROD) + 1));
     memcpy(net->n_react, n_react, sizeof(int) * M);
     memcpy(net->react, react, sizeof(int) * M * MAX_REACT);
@@ -123,6 +140,7 @@ void *oracle_create(int N, const int *A, int M, const int *n_react, const int *r
     int ne = 0;
     for (int r = 0; r < M; ++r) {
         double lp = 0.0;
+        long double lp_ld = 0.0L;
         /* reactant side: one edge per distinct species, nu = multiplicity */
         for (int q = 0; q < n_react[r]; ++q) {
             int s = react[r * MAX_REACT + q], first = 1, m = 0;
@@ -130,6 +148,7 @@ void *oracle_create(int N, const int *A, int M, const int *n_react, const int *r
             if (!first) continue;
             for (int u = 0; u < n_react[r]; ++u) if (react[r * MAX_REACT + u] == s) ++m;
             lp -= ln_factorial(m);
+            lp_ld -= ln_factorial_ld(m);
             net->edges[ne++] = (edge_t){r, s, -1, m};
         }
         for (int q = 0; q < n_prod[r]; ++q) {
@@ -140,6 +159,7 @@ void *oracle_create(int N, const int *A, int M, const int *n_react, const int *r
             net->edges[ne++] = (edge_t){r, s, +1, m};
         }
         net->ln_pref[r] = lp;
+        net->ln_pref_ld[r] = lp_ld;
     }
     net->n_edges = ne;
     return net;
@@ -149,7 +169,7 @@ void oracle_destroy(void *h) {
     oracle_net *net = (oracle_net *)h;
     if (!net) return;
     free(net->A); free(net->n_react); free(net->react); free(net->coef);
-    free(net->ln_pref); free(net->edges); free(net);
+    free(net->ln_pref); free(net->ln_pref_ld); free(net->edges); free(net);
 }
 
 int oracle_num_edges(void *h) { return ((oracle_net *)h)->n_edges; }
@@ -170,8 +190,25 @@ int oracle_rates(void *h, double T9, double rho, double *R) {
     return 0;
 }
 
+/* O2 in long double (arbiter). */
+static void rates_ld(const oracle_net *net, double T9d, double rhod, long double *R) {
+    long double T9 = (long double)T9d, rho = (long double)rhod;
+    long double t13 = cbrtl(T9);
+    long double t53 = T9 * t13 * t13;
+    long double lnT = logl(T9), lnrho = logl(rho);
+    for (int r = 0; r < net->M; ++r) {
+        const double *a = net->coef + r * N_COEF;
+        long double lnR = (long double)a[0] + (long double)a[1] / T9 + (long double)a[2] / t13 +
+                          (long double)a[3] * t13 + (long double)a[4] * T9 +
+                          (long double)a[5] * t53 + (long double)a[6] * lnT;
+        R[r] = expl(net->ln_pref_ld[r] + (long double)(net->n_react[r] - 1) * lnrho + lnR);
+    }
+}
+
 /* ---- the sub-step, written once per state type ------------------------- */
 #define REAL double
+#define RATE double
+#define TIME double
 #define SUFFIX(name) name##_f64
 #include "asym_substep.inc"
 #undef REAL
@@ -180,6 +217,17 @@ int oracle_rates(void *h, double T9, double rho, double *R) {
 #define SUFFIX(name) name##_f32
 #include "asym_substep.inc"
 #undef REAL
+#undef RATE
+#undef TIME
+#undef SUFFIX
+#define REAL long double
+#define RATE long double
+#define TIME long double
+#define SUFFIX(name) name##_f80
+#include "asym_substep.inc"
+#undef REAL
+#undef RATE
+#undef TIME
 #undef SUFFIX
 
 /* O4+O5 exposed for the pins: fluxes and sums for one state (double). */
@@ -192,7 +240,7 @@ static int run_zones(oracle_net *net, int zones, const double *T9, const double 
                      int adaptive, double t_hydro, double *dt, double dt_fixed,
                      long long n_fixed, long long *n_steps, int *status, long long *n_asym,
                      int precision, int n_threads) {
-    if (precision != 64 && precision != 32) return -1;
+    if (precision != 64 && precision != 32 && precision != 80) return -1;
     if (n_threads < 1) n_threads = 1;
     int N = net->N, M = net->M;
 #ifdef _OPENMP
@@ -200,21 +248,31 @@ static int run_zones(oracle_net *net, int zones, const double *T9, const double 
 #endif
     {
         double *R = (double *)malloc(sizeof(double) * (M + 1));
-        void *work = malloc(sizeof(double) * (size_t)(M + 4 * N + 4));
+        void *work = malloc(sizeof(long double) * (size_t)(M + 4 * N + 4));
+        long double *R_ld = (long double *)malloc(sizeof(long double) * (M + 1));
+        long double *Y_ld = (long double *)malloc(sizeof(long double) * (N + 1));
 #ifdef _OPENMP
 #pragma omp for schedule(dynamic, 1)
 #endif
         for (int z = 0; z < zones; ++z) {
-            oracle_rates(net, T9[z], rho[z], R);
+            if (precision == 80) rates_ld(net, T9[z], rho[z], R_ld);
+            else oracle_rates(net, T9[z], rho[z], R);
             double dt_io = (dt != NULL) ? dt[z] : 0.0;
             long long steps = 0, asym = 0;
             int st;
             if (precision == 64)
                 st = zone_f64(net, R, (double *)Y + (size_t)z * N, adaptive, t_hydro, &dt_io,
                               dt_fixed, n_fixed, &steps, &asym, work);
-            else
+            else if (precision == 32)
                 st = zone_f32(net, R, (float *)Y + (size_t)z * N, adaptive, t_hydro, &dt_io,
                               dt_fixed, n_fixed, &steps, &asym, work);
+            else { /* arbiter: abundances in and out as double */
+                double *Yz = (double *)Y + (size_t)z * N;
+                for (int i = 0; i < N; ++i) Y_ld[i] = (long double)Yz[i];
+                st = zone_f80(net, R_ld, Y_ld, adaptive, t_hydro, &dt_io, dt_fixed, n_fixed,
+                              &steps, &asym, work);
+                for (int i = 0; i < N; ++i) Yz[i] = (double)Y_ld[i];
+            }
             if (dt) dt[z] = dt_io;
             if (n_steps) n_steps[z] = steps;
             if (status) status[z] = st;
@@ -222,6 +280,8 @@ static int run_zones(oracle_net *net, int zones, const double *T9, const double 
         }
         free(R);
         free(work);
+        free(R_ld);
+        free(Y_ld);
     }
     return 0;
 }

@@ -752,7 +752,7 @@ int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rh
     if (energy && !n->D.bind)
         return fail(NET_EINVAL, "energy asked for before net_set_binding_energy");
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
-    if (!(t_hydro == t_hydro)) return fail(NET_EINVAL, "t_hydro is NaN");
+    if (!std::isfinite(t_hydro)) return fail(NET_EINVAL, "t_hydro is not finite");
     if (n->has_device && use_pull_kernel(n)) {
         if (zones < 0) return fail(NET_EINVAL, "zones < 0");
         if (zones == 0) return NET_OK;

@@ -329,9 +329,6 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             share[4] = p2 * m1;
             share[5] = p3 * m2;
         }
-        // the owner's own consumption in a hub-only reaction joins its F- row in finalize
-        if (hub_owner) sts(s_own + tid * SZ, k * y);
-
         // reciprocal factors of the dt candidates, off the critical path
         real inv = 0;
         if (ADAPT) {
@@ -339,6 +336,10 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             if (!plain_owner) inv = 0;  // hub owners are judged on their full rows in finalize
         }
         __syncthreads();
+        // the owner's own consumption in a hub-only reaction joins its F- row in finalize.  Stored
+        // between the barriers: B orders it before this step's reads, the next A orders those
+        // reads before the next store.
+        if (hub_owner) sts(s_own + tid * SZ, k * y);
 
         // ---- S2+S3 interleaved with the hub-row butterfly -------------------------------------
         // F+ = sum of the incoming fluxes, each evaluated here (groups of four P-slots), and
@@ -485,7 +486,9 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             const double qmax = warp_max_pos(cand);
             const double qg = q_prev * ginv;             // growth cap: dt <= g dt_prev
             const double q_ctrl = (qmax > qg) ? qmax : qg;  // a NaN candidate loses
-            last = q_ctrl <= q_rem * (1.0 / (1.0 - 1e-12));  // dt_ctrl >= rem (1 - 1e-12)
+            // dt_ctrl >= rem (1 - 1e-12); written so that rem <= 0 (t rounded onto t_hydro:
+            // q_rem is then NaN or negative) also ends the call, with a zero-length step
+            last = !(q_ctrl > q_rem * (1.0 / (1.0 - 1e-12))) || !(rem > 0.0);
             q = last ? q_rem : q_ctrl;
             hd = last ? rem : rcp_pos(q_ctrl);
             q_prev = q_ctrl;

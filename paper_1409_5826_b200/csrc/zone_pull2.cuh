@@ -249,8 +249,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
 #pragma unroll
             for (int i = 0; i < 6; ++i) share[i] += sb[i];
         }
-        if (hub_owner) sts(s_own + tid * SZ, ka * ya);  // own consumption in a hub-only reaction
-
         real inva = 0, invb = 0;  // reciprocal factors of the dt candidates, off the critical path
         if (ADAPT) {
             inva = rcp_pos(ya > y_floor ? eps_y * ya : yfl_eps);
@@ -259,6 +257,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             if (!plain_b) invb = 0;
         }
         __syncthreads();
+        // own consumption of a hub owner in a hub-only reaction, read in finalize.  Stored between
+        // the barriers: B orders it before this step's reads, the next A orders those reads
+        // before the next store.
+        if (hub_owner) sts(s_own + tid * SZ, ka * ya);
 
         // ---- S2+S3: P-slot gathers of both species, interleaved with the hub-row butterfly -----
         real Fpa, Fpb;
@@ -426,7 +428,9 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             const double qmax = warp_max_pos(cand);
             const double qg = q_prev * ginv;                 // growth cap: dt <= g dt_prev
             const double q_ctrl = (qmax > qg) ? qmax : qg;   // a NaN candidate loses
-            last = q_ctrl <= q_rem * (1.0 / (1.0 - 1e-12));  // dt_ctrl >= rem (1 - 1e-12)
+            // dt_ctrl >= rem (1 - 1e-12); written so that rem <= 0 (t rounded onto t_hydro:
+            // q_rem is then NaN or negative) also ends the call, with a zero-length step
+            last = !(q_ctrl > q_rem * (1.0 / (1.0 - 1e-12))) || !(rem > 0.0);
             q = last ? q_rem : q_ctrl;
             hd = last ? rem : rcp_pos(q_ctrl);
             q_prev = q_ctrl;
