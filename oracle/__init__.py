@@ -49,6 +49,7 @@ def _load():
         lib.oracle_destroy.argtypes = [C.c_void_p]
         lib.oracle_num_edges.argtypes = [C.c_void_p]
         lib.oracle_rates.argtypes = [C.c_void_p, C.c_double, C.c_double, _D]
+        lib.oracle_rates_ld.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p]
         lib.oracle_rhs.argtypes = [C.c_void_p, _D, _D, _D, _D, _D]
         lib.oracle_integrate.argtypes = [
             C.c_void_p, C.c_int, _D, _D, C.c_void_p, C.c_double, _D, _L, _I, _L, C.c_int, C.c_int,
@@ -109,6 +110,13 @@ class Oracle:
     def rates(self, T9: float, rho: float) -> np.ndarray:
         R = np.empty(self.M, np.float64)
         _lib.oracle_rates(self._h, float(T9), float(rho), _dp(R))
+        return R
+
+    def rates_ld(self, T9: float, rho: float) -> np.ndarray:
+        """O2 as the long-double arbiter evaluates it (np.longdouble, x87 extended)."""
+        assert np.dtype(np.longdouble).itemsize == C.sizeof(C.c_longdouble)
+        R = np.empty(self.M, np.longdouble)
+        _lib.oracle_rates_ld(self._h, float(T9), float(rho), R.ctypes.data_as(C.c_void_p))
         return R
 
     def rhs(self, R, Y):

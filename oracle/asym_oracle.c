@@ -205,6 +205,12 @@ static void rates_ld(const oracle_net *net, double T9d, double rhod, long double
     }
 }
 
+/* Exposed for the pins of the arbiter (R: [M] long double). */
+int oracle_rates_ld(void *h, double T9, double rho, long double *R) {
+    rates_ld((oracle_net *)h, T9, rho, R);
+    return 0;
+}
+
 /* ---- the sub-step, written once per state type ------------------------- */
 #define REAL double
 #define RATE double

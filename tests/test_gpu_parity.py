@@ -129,64 +129,77 @@ def zone_err(Yg, Yo, A):
     return rel.max(axis=1)
 
 
-def oracle_with_conditioning(net, T9, rho, Y0, t_hydro, dt=None, seeds=(101, 202)):
-    """Oracle result plus, per zone, how far the ORACLE moves when only the
-    summation order changes (same network with reactions shuffled and species
-    relabelled: every order is an equally valid result, reading Q14).
+def oracle_with_arbiter(net, T9, rho, Y0, t_hydro, dt=None, seeds=(101, 202), params=None):
+    """The fp64 oracle's result (what parity is asserted against) plus what the long-double
+    ARBITER says about each zone (oracle/asym_oracle.c, precision = 80; oracle side only).
 
-    The explicit asymptotic step is discontinuous in dt (Euler/Eq. (3) switch at
-    k dt = kappa, end-of-interval clamp) and dt feeds back through the
-    controller, so in zones close to equilibrium a one-ulp difference grows to
-    1e-5..1e-3 within one hydro step (measured; table in DESIGN.md).  delta_z
-    below is that intrinsic spread; parity is asked to 1e-6 where the problem is
-    that well conditioned, and to the spread where it is not."""
+    The explicit asymptotic step is discontinuous in dt (Euler/Eq. (3) switch at k dt = kappa,
+    end-of-interval clamp) and dt feeds back through the controller, so in zones close to
+    equilibrium a one-ulp difference grows to 1e-5..1e-3 within one hydro step.
+    Any summation order is a valid result (reading Q14), so where the GPU and the fp64 oracle
+    differ by more than the north_star's 1e-6 the question is which of them, if either, left
+    the method's trajectory.  The arbiter is that trajectory computed with 2048x finer
+    rounding.  Returned per zone:
+      e_o   the largest distance from the arbiter of three equally valid fp64 oracle runs
+            (the caller's order, and two with reactions shuffled and species relabelled)
+      ds_o  the same for the step counts."""
     n = max_threads()
-    ref = Oracle(net).integrate(T9, rho, Y0, t_hydro, dt=dt, n_threads=n)
-    delta = np.zeros(Y0.shape[0])
-    dsteps = np.zeros(Y0.shape[0], dtype=np.int64)
+    ref = Oracle(net, params).integrate(T9, rho, Y0, t_hydro, dt=dt, n_threads=n)
+    arb = Oracle(net, params).integrate(T9, rho, Y0, t_hydro, dt=dt, n_threads=n, precision=80)
+    e_o = zone_err(ref["Y"], arb["Y"], net.A)
+    ds_o = np.abs(ref["n_steps"] - arb["n_steps"])
     for seed in seeds:
         net2, sigma = net.permuted(seed)
         Yp = np.zeros_like(Y0)
         Yp[:, sigma] = Y0
-        alt = Oracle(net2).integrate(T9, rho, Yp, t_hydro, dt=dt, n_threads=n)
-        delta = np.maximum(delta, zone_err(alt["Y"][:, sigma], ref["Y"], net.A))
-        dsteps = np.maximum(dsteps, np.abs(alt["n_steps"] - ref["n_steps"]))
-    return ref, delta, dsteps
+        alt = Oracle(net2, params).integrate(T9, rho, Yp, t_hydro, dt=dt, n_threads=n)
+        e_o = np.maximum(e_o, zone_err(alt["Y"][:, sigma], arb["Y"], net.A))
+        ds_o = np.maximum(ds_o, np.abs(alt["n_steps"] - arb["n_steps"]))
+    return ref, dict(arb=arb, e_o=e_o, ds_o=ds_o)
 
 
-SPREAD_FACTOR = 10.0  # two rounding perturbations of equal size grow chaotically to the same decade
+ARBITER_FACTOR = 4.0
 
 
-def check_adaptive(g, ref, delta, dsteps, A, label="", min_well=0.75):
-    """north_star: <= 1e-6 and steps within 1 %; relaxed per zone to the oracle's
-    own reassociation spread where that is larger."""
+def check_adaptive(g, ref, arbiter, A, label="", min_direct=0.75):
+    """north_star: mass fractions above 1e-12 within 1e-6 of the oracle, step counts within
+    1 %.  Every zone must either meet that directly against the fp64 oracle, or -- DESIGN.md
+    reading Q14 and section 5 -- be no further from the long-double arbiter than 4x the fp64
+    oracle's own worst distance from it (abundances and step counts alike).  At least
+    min_direct of the zones must pass directly, or the test means nothing."""
     assert (g["status"] == 0).all() and (ref["status"] == 0).all()
-    err = zone_err(g["Y"], ref["Y"], A)
-    tol = np.maximum(ADAPT_TOL, SPREAD_FACTOR * delta)
-    well = delta <= 1e-8
-    assert well.mean() >= min_well, "most zones must be well conditioned for this test to mean anything"
-    bad = np.nonzero(err > tol)[0]
-    assert bad.size == 0, (label, bad[:8], err[bad[:8]], delta[bad[:8]])
-    ds = np.abs(g["n_steps"] - ref["n_steps"])
-    ds_tol = np.maximum(np.maximum(1, ref["n_steps"] // 100), 4 * dsteps)
-    assert (ds <= ds_tol).all(), (label, ds.max())
-    m = well & (ds == 0)
-    np.testing.assert_allclose(g["dt"][m], ref["dt"][m], rtol=1e-6)
     assert np.isfinite(g["Y"]).all() and (g["Y"] >= 0).all()
-    return dict(max_err_well=float(err[well].max()) if well.any() else 0.0, n_ill=int((~well).sum()),
-                max_err_ill=float(err[~well].max()) if (~well).any() else 0.0,
-                max_delta=float(delta.max()))
+    arb, e_o, ds_o = arbiter["arb"], arbiter["e_o"], arbiter["ds_o"]
+    err = zone_err(g["Y"], ref["Y"], A)
+    ds = np.abs(g["n_steps"] - ref["n_steps"])
+    direct = (err <= ADAPT_TOL) & (ds <= np.maximum(1, ref["n_steps"] // 100))
+    assert direct.mean() >= min_direct, (label, float(direct.mean()))
+    # the rest goes to the arbiter
+    err_a = zone_err(g["Y"], arb["Y"], A)
+    ds_a = np.abs(g["n_steps"] - arb["n_steps"])
+    ok_a = (err_a <= np.maximum(ADAPT_TOL, ARBITER_FACTOR * e_o)) & \
+           (ds_a <= np.maximum(np.maximum(1, arb["n_steps"] // 100), ARBITER_FACTOR * ds_o))
+    bad = np.nonzero(~direct & ~ok_a)[0]
+    assert bad.size == 0, (label, bad[:8], err[bad[:8]], err_a[bad[:8]], e_o[bad[:8]], ds_a[bad[:8]], ds_o[bad[:8]])
+    m = direct & (ds == 0)
+    np.testing.assert_allclose(g["dt"][m], ref["dt"][m], rtol=1e-6)
+    arbitrated = ~direct
+    ratio = err_a[arbitrated] / np.maximum(e_o[arbitrated], ADAPT_TOL / ARBITER_FACTOR)
+    return dict(zones=int(err.size), max_err_direct=float(err[direct].max()) if direct.any() else 0.0,
+                n_arbitrated=int(arbitrated.sum()),
+                worst_gpu_vs_arbiter=float(err_a[arbitrated].max()) if arbitrated.any() else 0.0,
+                worst_oracle_vs_arbiter=float(e_o.max()),
+                worst_ratio=float(ratio.max()) if arbitrated.any() else 0.0)
 
 
 def test_config2_adaptive_long(hub150):
     c = build_config(2)
     kn = K.Net(hub150)
-    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     assert ref["n_steps"][0] > 10_000
-    # one zone, ~29 000 sub-steps: its own reassociation spread is ~3e-7, still inside 1e-6
-    assert delta[0] < ADAPT_TOL
-    print(check_adaptive(g, ref, delta, dsteps, hub150.A, "config2", min_well=0.0))
+    # one zone, ~29 000 sub-steps: the fp64 oracle itself sits ~3e-7 from the arbiter
+    print("config2", check_adaptive(g, ref, arb, hub150.A, "config2", min_direct=0.0))
 
 
 def test_config3_operator_split_carry_dt(hub150):
@@ -198,9 +211,9 @@ def test_config3_operator_split_carry_dt(hub150):
     Yo, dto = c["Y0"], None
     Yg, dtg = c["Y0"], None
     for call in range(c["calls"]):
-        ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], Yo, c["t_hydro"], dto)
+        ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], Yo, c["t_hydro"], dto)
         g = gpu_integrate(kn, c["T9"], c["rho"], Yo, c["t_hydro"], dt=dto)
-        print(call, check_adaptive(g, ref, delta, dsteps, hub150.A, f"config3 call {call}"))
+        print("config3 call", call, check_adaptive(g, ref, arb, hub150.A, f"config3 call {call}"))
         chained = gpu_integrate(kn, c["T9"], c["rho"], Yg, c["t_hydro"], dt=dtg)
         Yg, dtg = chained["Y"], chained["dt"]
         Yo, dto = ref["Y"], ref["dt"]
@@ -222,9 +235,8 @@ def test_config4_full_batch_sampled(hub150):
     longest = np.argsort(g["n_steps"])[-16:]
     rest = rng.choice(c["zones"], 240, replace=False)
     idx = np.unique(np.concatenate([longest, rest]))
-    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"][idx], c["rho"][idx], c["Y0"][idx],
-                                                  c["t_hydro"])
-    print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, hub150.A, "config4"))
+    ref, arb = oracle_with_arbiter(hub150, c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"])
+    print("config4", check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, hub150.A, "config4"))
 
 
 def test_config5_large_network_sampled():
@@ -236,9 +248,8 @@ def test_config5_large_network_sampled():
     rng = np.random.default_rng(55)
     idx = np.unique(np.concatenate([np.argsort(g["n_steps"])[-4:],
                                     rng.choice(c["zones"], 60, replace=False)]))
-    ref, delta, dsteps = oracle_with_conditioning(net, c["T9"][idx], c["rho"][idx], c["Y0"][idx],
-                                                  c["t_hydro"])
-    print(check_adaptive({k: v[idx] for k, v in g.items()}, ref, delta, dsteps, net.A, "config5"))
+    ref, arb = oracle_with_arbiter(net, c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"])
+    print("config5", check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, net.A, "config5"))
 
 
 def test_every_kernel_on_a_pull_network(hub150):
@@ -246,12 +257,12 @@ def test_every_kernel_on_a_pull_network(hub150):
     2 = the one-species pull kernel, 1 = the generic flux-array kernel (the fallback of
     networks that do not qualify).  All three must meet the same parity on the same zones."""
     c = build_config(3, zones=24)
-    ref, delta, dsteps = oracle_with_conditioning(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     for kernel, runs in ((0, 2), (2, 1), (1, 0)):
         kn = K.Net(hub150, K.NetParams(kernel=kernel))
         assert kn.schedule_info()["kernel"] == runs
         g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
-        print(kernel, check_adaptive(g, ref, delta, dsteps, hub150.A, f"kernel={kernel}", min_well=0.5))
+        print("kernel", kernel, check_adaptive(g, ref, arb, hub150.A, f"kernel={kernel}", min_direct=0.5))
         ref_f = Oracle(hub150).integrate_fixed(c["T9"], c["rho"], c["Y0"], 1e-9, 200)
         err, _ = max_rel_err(gpu_fixed(kn, c["T9"], c["rho"], c["Y0"], 1e-9, 200), ref_f["Y"], hub150.A)
         assert err <= FIXED_TOL, (kernel, err)
@@ -266,6 +277,47 @@ def test_gpu_single_decay_closed_forms():
         Y = gpu_fixed(kn, 1.0, 1.0, np.array([[Y0, 0.0]]), dt, n)[0]
         want = Y0 * (1 - dt) ** n if dt < 1 else Y0 / (1 + dt) ** n
         assert Y[0] == pytest.approx(want, rel=1e-13)
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_gpu_controller_closed_forms(kernel):
+    """The hand-worked controller cases of tests/test_oracle_pins.py on the GPU path itself
+    (pull kernel and generic kernel): the abundance floor, the growth cap, the 1e-12 end
+    guard on both sides, and the returned unclamped dt (readings Q7, Q9, Q10)."""
+    toy = make_toy([1, 1], [((0,), (1,))], [1.0])
+    one = np.array([1.0])
+
+    def run(par, Y0, t_hydro, dt=None):
+        kn = K.Net(toy, K.NetParams(kernel=kernel, **par))
+        return gpu_integrate(kn, one, one, np.array([Y0]), t_hydro, dt=dt)
+
+    # floor: Y_A = Y_floor/4 -> dt = 0.2, 0.25, then 1/3 clamped to 1/6: 3 steps, Y_A halves
+    for y_floor, Y0 in ((1e-10, 2.5e-11), (1e-3, 2.5e-4)):
+        g = run(dict(eps_y=0.05, y_floor=y_floor), [Y0, 1.0], 0.2 + 0.25 + 1.0 / 6.0)
+        assert g["n_steps"][0] == 3 and g["status"][0] == 0
+        assert g["Y"][0, 0] == pytest.approx(Y0 / 2, rel=1e-12)
+        assert g["dt"][0] == pytest.approx(1.0 / 3.0, rel=1e-12)
+    # growth cap 1.5 from a trial dt of 0.01: 0.015, 0.0225, 0.03375, 0.05, 0.05
+    g = run(dict(eps_y=0.05, growth=1.5), [1.0, 100.0], 0.17125, dt=np.array([0.01]))
+    assert g["n_steps"][0] == 5 and g["dt"][0] == pytest.approx(0.05, rel=1e-12)
+    assert g["Y"][0, 0] == pytest.approx(0.985 * 0.9775 * 0.96625 * 0.95**2, rel=1e-12)
+    # end guard: dt_ctrl = 0.05 against rem = 0.05 (1 + 5e-13) is the last step, (1 + 5e-12) is not
+    for excess, want in ((5e-13, 1), (5e-12, 2)):
+        g = run(dict(eps_y=0.05), [1.0, 100.0], 0.05 * (1.0 + excess))
+        assert g["n_steps"][0] == want and g["dt"][0] == pytest.approx(0.05, rel=1e-12)
+    # 20 steps of 0.05 to t = 1: the sum of the steps lands within rounding of t_hydro and the
+    # call must end there (never a zero or negative remainder spun to max_steps)
+    g = run(dict(eps_y=0.05), [1.0, 100.0], 1.0)
+    assert g["n_steps"][0] == 20 and g["status"][0] == 0
+    assert g["Y"][0, 0] == pytest.approx(0.95**20, rel=1e-12)
+
+
+def test_non_finite_t_hydro_is_rejected(g16):
+    kn = K.Net(g16)
+    c = build_config(1)
+    for bad in (float("nan"), float("inf")):
+        with pytest.raises(K.KinnetError):
+            kn.net_integrate(1, dev(c["T9"]), dev(c["rho"]), dev(c["Y0"]), bad)
 
 
 def test_empty_and_degenerate_calls(g16):
@@ -399,9 +451,9 @@ def test_pull_kernel_block_size_classes(N, M, kernel, runs, threads):
         np.testing.assert_allclose(Fp[q].cpu().numpy(), Fpo, rtol=1e-12, atol=1e-300)
         np.testing.assert_allclose(Fm[q].cpu().numpy(), Fmo, rtol=1e-12, atol=1e-300)
     # adaptive
-    refa, delta, dsteps = oracle_with_conditioning(net, T9, rho, Y0, 1e-7)
+    refa, arb = oracle_with_arbiter(net, T9, rho, Y0, 1e-7)
     g = gpu_integrate(kn, T9, rho, Y0, 1e-7)
-    print(N, check_adaptive(g, refa, delta, dsteps, net.A, f"N={N}", min_well=0.6))
+    print("N", N, check_adaptive(g, refa, arb, net.A, f"N={N}", min_direct=0.6))
 
 
 # ------------------------------------------------------- energy release (reading Q19)
@@ -446,14 +498,9 @@ def test_non_default_integrator_parameters(hub150, kernel):
     c = build_config(3, zones=12)
     par = dict(kappa=2.0, eps_y=0.02, y_floor=1e-8, growth=1.5, max_steps=1_000_000)
     net = hub150
-    o = Oracle(net, OracleParams(**par))
     kn = K.Net(net, K.NetParams(kernel=kernel, **par))
-    ref = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], n_threads=max_threads())
+    ref, arb = oracle_with_arbiter(net, c["T9"], c["rho"], c["Y0"], c["t_hydro"], params=OracleParams(**par))
     g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
-    assert (g["status"] == 0).all()
-    same = g["n_steps"] == ref["n_steps"]
-    assert same.mean() >= 0.75 and (np.abs(g["n_steps"] - ref["n_steps"]) <= np.maximum(1, ref["n_steps"] // 100)).all()
-    err = zone_err(g["Y"], ref["Y"], net.A)
-    assert (err[same] <= ADAPT_TOL).all(), err
+    print("non-default parameters, kernel", kernel, check_adaptive(g, ref, arb, net.A, f"params kernel={kernel}"))
     # the parameters do reach the integrator: the default ones take other step counts
     assert (ref["n_steps"] != Oracle(net).integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"])["n_steps"]).all()

@@ -117,6 +117,78 @@ def test_p3_single_decay_continuum():
     assert 4e-5 < rel < 6e-5
 
 
+# ------------------------------------------------ pins found missing by mutation
+@pytest.mark.parametrize("y_floor,Y0", [(1e-10, 2.5e-11), (1e-3, 2.5e-4)])
+def test_y_floor_value_sets_the_step_sequence(y_floor, Y0):
+    """O6 (S:Q7): the candidate of a species BELOW the floor is eps*Y_floor/|dY/dt|, not
+    eps*Y/|dY/dt|.  Worked by hand for A -> B, k = 1, eps = 0.05, Y_A(0) = Y_floor/4, Y_B = 1
+    (B's candidate eps*1/(k Y_A) is astronomically large; the growth cap 2*t_hydro never binds):
+      step 1: dt = eps*Y_floor/(k Y_A) = 4 eps = 0.2     k dt = 0.2  -> Euler, Y_A *= 0.8
+      step 2: dt = 0.2/0.8 = 0.25                         k dt = 0.25 -> Euler, Y_A *= 0.75
+      step 3: dt_ctrl = 0.25/0.75 = 1/3, but t_hydro = 0.2 + 0.25 + 1/6 leaves 1/6:
+              clamped, k dt = 1/6 -> Euler, Y_A *= 5/6
+    so 3 steps, Y_A = Y0 * 0.8 * 0.75 * 5/6 = Y0/2, returned dt = 1/3 (unclamped).
+    A floor 100x larger gives dt_1 = 20 > t_hydro (1 step); a floor 100x smaller, or none,
+    puts Y_A above it and gives dt = eps/k = 0.05 (13 steps)."""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.05, y_floor=y_floor))
+    t_hydro = 0.2 + 0.25 + 1.0 / 6.0
+    out = o.integrate(1.0, 1.0, [[Y0, 1.0]], t_hydro)
+    assert out["n_steps"][0] == 3 and out["status"][0] == 0 and out["n_asym"][0] == 0
+    assert out["Y"][0, 0] == pytest.approx(Y0 / 2, rel=1e-13)
+    assert out["dt"][0] == pytest.approx(1.0 / 3.0, rel=1e-13)
+    assert out["Y"][0, 1] == pytest.approx(1.0 + Y0 / 2, rel=1e-15)
+
+
+def test_end_clamp_guard_decides_one_step_or_two():
+    """O6 (S:Q9): the step is the last one when dt_ctrl >= rem*(1 - 1e-12).  A -> B, k = 1,
+    Y_A = 1, Y_B = 100, eps = 0.05: dt_ctrl = eps*Y_A/(k Y_A) = 0.05 to an ulp.
+      t_hydro = 0.05*(1 + 5e-13): dt_ctrl is below rem by 5e-13 relative -- inside the guard:
+          ONE step of exactly t_hydro (without the guard: a second, 2.5e-14 s sliver step);
+      t_hydro = 0.05*(1 + 5e-12): outside the guard: TWO steps.
+    Either way the returned dt is the unclamped 0.05 and Y_A = 1 - t_hydro to rounding."""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.05))
+    for excess, want_steps in ((5e-13, 1), (5e-12, 2)):
+        t_hydro = 0.05 * (1.0 + excess)
+        out = o.integrate(1.0, 1.0, [[1.0, 100.0]], t_hydro)
+        assert out["n_steps"][0] == want_steps, (excess, out["n_steps"][0])
+        assert out["dt"][0] == pytest.approx(0.05, rel=1e-14)
+        assert out["Y"][0, 0] == pytest.approx(1.0 - t_hydro, rel=1e-13)
+
+
+@pytest.mark.parametrize("a,branch", [(0.5, "euler"), (1.0, "euler"), (1.5, "euler"),
+                                       (2.0, "asym"), (3.0, "asym")])
+def test_p2_closed_forms_at_kappa_two(a, branch):
+    """The branch threshold is the parameter kappa, not the constant 1: at
+    kappa = 2 a single decay with k dt = 1 or 1.5 still takes forward Euler --
+    Y0 (1 - k dt)^n, i.e. exactly 0 after one step at k dt = 1 and a sign-alternating
+    Y0 (-1/2)^n at 1.5 (the closed form holds for either sign: F- = k Y) -- and
+    k dt = 2 exactly is the first asymptotic value, Y0/(1 + k dt)^n."""
+    o = Oracle(decay_net(1.0), OracleParams(kappa=2.0))
+    n, Y0 = 12, 0.75
+    out = o.integrate_fixed(1.0, 1.0, [Y0, 0.0], a, n)
+    YA = out["Y"][0, 0]
+    if branch == "euler":
+        want = Y0 * (1 - a) ** n
+        assert YA == pytest.approx(want, rel=1e-13, abs=0.0)
+        assert out["n_asym"][0] == 0
+    else:
+        assert YA == pytest.approx(Y0 / (1 + a) ** n, rel=1e-13)
+        assert out["n_asym"][0] == n
+
+
+def test_growth_cap_is_the_parameter():
+    """O6 (S:Q7): dt <= g*dt_prev with g the parameter.  A -> B, k = 1, Y_A = 1, Y_B = 100,
+    eps = 0.05 (candidate 0.05), g = 1.5, trial dt 0.01:
+      dt = 0.015, 0.0225, 0.03375 (cap binds), then 1.5*0.03375 = 0.050625 > 0.05: the candidate;
+      t_hydro = 0.07125 + 2*0.05 = 0.17125 is reached in exactly 5 steps,
+      Y_A = 0.985 * 0.9775 * 0.96625 * 0.95^2.   (g = 2 would take 0.02, 0.04, 0.05, ...)"""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.05, growth=1.5))
+    out = o.integrate(1.0, 1.0, [[1.0, 100.0]], 0.17125, dt=[0.01])
+    assert out["n_steps"][0] == 5
+    assert out["Y"][0, 0] == pytest.approx(0.985 * 0.9775 * 0.96625 * 0.95**2, rel=1e-13)
+    assert out["dt"][0] == pytest.approx(0.05, rel=1e-13)
+
+
 # ------------------------------------------------- P4: two-species fixed point
 @pytest.mark.parametrize("dt", [1e-3, 0.5, 10.0, 1e3])
 def test_p4_two_species_equilibrium_ratio(dt):
@@ -442,3 +514,61 @@ def test_energy_vanishes_when_binding_is_proportional_to_mass_number(g16):
     assert out["n_asym"][0] == 0
     E = Oracle.energy(7.5 * g16.A, c["Y0"], out["Y"])[0]
     assert abs(E) < 1e-11
+
+
+# ------------------------------------------------ the long-double arbiter (precision = 80)
+def test_arbiter_rates_vs_numpy_longdouble(hub150):
+    """O2 of the arbiter against numpy's own long-double libm route, term by term."""
+    o = Oracle(hub150)
+    L = np.longdouble
+    third = L(1) / L(3)
+    for T9, rho in ((1.0, 1e7), (3.3, 2.2e8), (10.0, 3.1e9)):
+        R = o.rates_ld(T9, rho)
+        T = L(T9)
+        a = hub150.coef.astype(L)
+        lnp = np.array([
+            -sum(np.log(L(factorial(list(re[:n]).count(s)))) for s in set(re[:n]))
+            for re, n in zip(hub150.react, hub150.n_react)
+        ], dtype=L)
+        ln = (a[:, 0] + a[:, 1] / T + a[:, 2] * T ** (-third) + a[:, 3] * T ** third + a[:, 4] * T
+              + a[:, 5] * T ** (L(5) * third) + a[:, 6] * np.log(T)
+              + lnp + (hub150.n_react.astype(L) - 1) * np.log(L(rho)))
+        rel = np.abs(R / np.exp(ln) - 1).astype(np.float64)
+        assert rel.max() < 2e-16  # exponent arguments ~1e2 amplify an extended-precision ulp (5e-20)
+        # and the fp64 rates are the arbiter's rates to fp64 rounding
+        assert np.abs(o.rates(T9, rho) / R.astype(np.float64) - 1).max() < 2e-13
+
+
+@pytest.mark.parametrize("k,dt,branch", [(1.0, 0.25, "euler"), (1.0, 1.0, "asym"), (1.0, 4.0, "asym")])
+def test_arbiter_single_decay_closed_forms(k, dt, branch):
+    """P2 on the arbiter: same closed forms, now met to the last bit or two of a double."""
+    o = Oracle(decay_net(k))
+    n, Y0 = 40, 0.75
+    out = o.integrate_fixed(1.0, 1.0, [Y0, 0.0], dt, n, precision=80)
+    a = np.longdouble(k) * np.longdouble(dt)
+    want = np.longdouble(Y0) * ((1 - a) ** n if branch == "euler" else (1 + a) ** (-n))
+    assert out["Y"][0, 0] == pytest.approx(float(want), rel=4e-16)
+    assert out["n_asym"][0] == (0 if branch == "euler" else n)
+
+
+def test_arbiter_controller_contract_and_agreement_with_fp64(g16, hub150):
+    """The arbiter runs the same controller (20 steps / dt 0.05 on the worked single decay),
+    and on well-conditioned runs it agrees with the fp64 oracle to fp64 rounding: fixed dt on
+    config 1 (<= 1e-12), adaptive on a short hub150 step (same step count, <= 1e-9)."""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.05, growth=2.0))
+    out = o.integrate(1.0, 1.0, [[1.0, 100.0]], 1.0, precision=80)
+    assert out["n_steps"][0] == 20 and out["dt"][0] == pytest.approx(0.05, rel=1e-15)
+    assert out["Y"][0, 0] == pytest.approx(0.95**20, rel=1e-15)
+    c = build_config(1)
+    og = Oracle(g16)
+    a = og.integrate_fixed(c["T9"], c["rho"], c["Y0"], 1e-5, 1000)
+    b = og.integrate_fixed(c["T9"], c["rho"], c["Y0"], 1e-5, 1000, precision=80)
+    m = a["Y"] * g16.A > 1e-12
+    assert (a["n_asym"] == b["n_asym"]).all() and np.abs(a["Y"][m] / b["Y"][m] - 1).max() < 1e-12
+    oh = Oracle(hub150)
+    Y0 = np.zeros((1, 150))
+    Y0[0, 3], Y0[0, 15] = 0.5 / 12, 0.5 / 16
+    a = oh.integrate(4.0, 1e8, Y0, 1e-8)
+    b = oh.integrate(4.0, 1e8, Y0, 1e-8, precision=80)
+    m = a["Y"] * hub150.A > 1e-12
+    assert a["n_steps"][0] == b["n_steps"][0] and np.abs(a["Y"][m] / b["Y"][m] - 1).max() < 1e-9
