@@ -103,14 +103,14 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU):
+def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU, name: str = "hub150"):
     """Weak scaling: the global batch is world x 16384 zones of one seeded profile;
     rank r integrates the contiguous shard r (no data-path collective)."""
     from gen import perturbed_co_start, zone_profile
     from gen.configs import network
     from paper_1409_5826_b200.shard import zone_shard
 
-    net = network("hub150")
+    net = network(name)
     total = zones_per_gpu * world
     lo, hi = zone_shard(total, rank, world)
     T9, rho = zone_profile(total, PROFILE_SEED)
@@ -196,7 +196,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
 
-    net, T9h, rhoh, Y0h = workload(rank, world, args.zones)
+    net, T9h, rhoh, Y0h = workload(rank, world, args.zones, args.network)
     z, N = Y0h.shape
     kn = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel))
     info = kn.schedule_info()
@@ -397,6 +397,9 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2],
                     help="net_params_t.kernel: 0 = automatic, 1 = generic flux-array kernel, "
                          "2 = one-species-per-thread pull kernel (A/B runs)")
+    ap.add_argument("--network", default="hub150", choices=["hub150", "hub150hh"],
+                    help="hub150 = the metric's network; hub150hh = the same plus 16 heavy + heavy reactions "
+                         "and their inverses (the fast path must survive them, DESIGN.md 4.8)")
     ap.add_argument("--sweep", choices=["zones", "size"],
                     help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
                          "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")

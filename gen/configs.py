@@ -23,6 +23,8 @@ def network(name: str) -> Network:
         return make_g16(16)
     if name == "hub150":
         return make_hub_network(150, 1604, seed=1409)
+    if name == "hub150hh":  # hub150 plus 16 heavy + heavy fusions and their inverses
+        return make_hub_network(150, 1604, seed=1409, heavy_pairs=16)
     if name == "hub365":
         return make_hub_network(365, 4400, seed=365)
     raise KeyError(name)

@@ -193,6 +193,7 @@ def make_hub_network(
     hi: float = 10.0,
     T9ref: float = 5.0,
     rhoref: float = 1e9,
+    heavy_pairs: int = 0,
 ) -> Network:
     """Hub network G(N, M, seed, lo, hi, T9ref, rhoref) of SURVEY §8(d).
 
@@ -205,6 +206,11 @@ def make_hub_network(
       exchange X + l -> X'' + l' paired with its inverse;
       three-body X + l + l' -> X'';
       fixed pair 3 alpha -> (first A=12) and back.
+    heavy_pairs = k appends k heavy + heavy fusions X + X' -> X'' (+ l) among the light end of
+    the heavy species (A <= 24: the 12C+12C, 12C+16O, 16O+16O class of the paper's Type Ia
+    network), each paired with its inverse, from a separate seeded stream, at
+    seeded positions of the reaction list: M + 2k reactions in all, the first M tables
+    identical to heavy_pairs = 0.
     """
     assert N >= 32
     rng = np.random.default_rng(seed)
@@ -306,7 +312,39 @@ def make_hub_network(
         "first_A12": c12,
         "first_A16": iso[16][0],
     }
+    if heavy_pairs:
+        rng2 = np.random.default_rng([seed, 0x4848])
+        light_end = [s for s in range(3, N) if A[s] <= 24]
+        extra = []
+        tries = 0
+        while len(extra) < 2 * heavy_pairs:
+            tries += 1
+            assert tries < 1000 * (heavy_pairs + 10), "generator could not place the heavy pairs"
+            X, X1 = (light_end[int(v)] for v in rng2.integers(0, len(light_end), size=2))
+            if not extra:
+                X1 = X  # the first pair is an identical one (the 12C+12C shape: flux R Y^2/2, F- = 2f)
+            l = int(rng2.integers(-1, 3))  # -1: pure fusion, else the emitted light particle
+            X2 = pick_from(rng2, iso, A[X] + A[X1] - (a_light[l] if l >= 0 else 0))
+            if X2 is None:
+                continue
+            pr = (X2,) if l < 0 else (X2, l)
+            if try_add(((X, X1), pr), (pr, (X, X1))):
+                extra += reactions[-2:]
+                del reactions[-2:]
+        coefs = list(coefs) + _draw_coefs(rng2, extra, lo, hi, T9ref, rhoref, charged=(1, 2))
+        reactions = list(reactions) + extra
+        order2 = rng2.permutation(len(reactions))
+        reactions = [reactions[o] for o in order2]
+        coefs = [coefs[o] for o in order2]
+        meta["heavy_pairs"] = heavy_pairs
+        return _pack(A, reactions, coefs, f"hub{N}_{M}hh{heavy_pairs}", meta)
     return _pack(A, reactions, coefs, f"hub{N}_{M}", meta)
+
+
+def pick_from(rng, iso, Aq):
+    """A seeded species of mass number Aq, or None."""
+    pool = iso.get(Aq)
+    return None if not pool else pool[int(rng.integers(0, len(pool)))]
 
 
 def make_toy(A, reactions, rates, name="toy") -> Network:

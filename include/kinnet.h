@@ -68,7 +68,8 @@ typedef struct {
     int precision;       /* 64 (default) or 32                                            */
     int kernel;          /* 0 = automatic: the two-species-per-thread pull kernel when an instantiation
                             covers the network, else the one-species pull kernel when the network
-                            qualifies (every reaction has at most one non-hub reactant),
+                            qualifies (every reaction has at most one non-hub reactant, DESIGN.md 4.2;
+                            the two-species kernel also takes reactions with two),
                             else the generic flux-array kernel; 1 = always the generic kernel;
                             2 = the one-species pull kernel when the network qualifies (A/B tests) */
 } net_params_t;
@@ -183,6 +184,8 @@ typedef struct {
     int pull_wavefronts_ideal; /* ... without bank conflicts                          */
     int pull_threads;    /* (virtual) threads the pull tables are compiled for: = threads for
                             kernel 1, 2 * threads for kernel 2 (a thread plays two of them) */
+    int pull_nslots;     /* longest per-thread N-slot list (reactions with two non-hub reactants);
+                            0 = the network has none                                    */
 } net_schedule_info_t;
 
 int net_schedule_info(const net_t *net, net_schedule_info_t *info);
@@ -206,7 +209,11 @@ int net_schedule_info(const net_t *net, net_schedule_info_t *info);
  *   "pull_n_slots"  [T]   "pull_n_slots2" [T]
  *   "pull_slot_rxn" [max(1,pull_slots)*T]  slot e of thread t: reaction | nu << 24, -1 = empty
  *   "pull_slot_f1"  [max(1,pull_slots)*T]  word class*T + thread of its first factor
- *   "pull_slot_f2"  [max(1,pull_slots2)*T] word of its second factor (4*T = one)
+ *   "pull_slot_f2"  [max(1,pull_slots2)*T] word of its second factor (4*T + 3 = one)
+ *   "pull_n_nslots" [T]                    N-slots of thread t: reactions its species enters with
+ *                                          another non-hub reactant (k += nu R Y_partner)
+ *   "pull_nslot_rxn" [4*T]                 reaction | nu << 24, -1 = empty
+ *   "pull_nslot_f1" [4*T]                  word of the partner's abundance
  *   "pull_agg_ptr"  [20*T]                 rate-sum coefficient s of thread t sums entries
  *                                          [ptr[s][t], ptr[s+1][t]) of its list
  *   "pull_agg_ent"  [max(1,pull_agg_max)*T] reaction | nu << 24

@@ -531,11 +531,20 @@ int upload_pull(net* n) {
             coef[static_cast<size_t>(c) * M + r] = S.coef[static_cast<size_t>(c) * slots + idx];
     }
     const uint32_t one_off = static_cast<uint32_t>(4 * T) * elem;
-    std::vector<uint32_t> cnt(T), f1(static_cast<size_t>(kinnet::kPullMaxSlots / 2) * T),
+    // P-slot rows up to the largest capacity, then the N-slot rows
+    constexpr int kRows = kinnet::kPullMaxSlots + kinnet::kPullNSlots;
+    std::vector<uint32_t> cnt(T), f1(static_cast<size_t>(kRows / 2) * T),
         f2(static_cast<size_t>(kinnet::kPullMaxSlots2 / 2) * T);
-    std::vector<int32_t> rxn(static_cast<size_t>(kinnet::kPullMaxSlots) * T, -1);
+    std::vector<int32_t> rxn(static_cast<size_t>(kRows) * T, -1);
     for (int t = 0; t < T; ++t) {
-        cnt[t] = P.n_slots[t] | static_cast<uint32_t>(P.n_slots2[t]) << 8;
+        cnt[t] = P.n_slots[t] | static_cast<uint32_t>(P.n_slots2[t]) << 8 |
+                 static_cast<uint32_t>(P.n_nslots[t]) << 16;
+        for (int e = 0; e < kinnet::kPullNSlots; ++e) {
+            const int row = kinnet::kPullMaxSlots + e;
+            rxn[static_cast<size_t>(row) * T + t] = P.nslot_rxn[static_cast<size_t>(e) * T + t];
+            f1[static_cast<size_t>(row / 2) * T + t] |=
+                (P.nslot_f1[static_cast<size_t>(e) * T + t] * elem) << (16 * (row & 1));
+        }
         for (int e = 0; e < kinnet::kPullMaxSlots; ++e) {
             uint32_t off = one_off;
             if (e < P.slots) {
@@ -649,6 +658,10 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
             n->pull2 = true;
             n->pull2_spill = spill;
         }
+    }
+    if (n->PS.ok && n->PS.nslots > 0 && !n->pull2) {
+        n->PS.ok = false;  // only the two-species kernel is instantiated with N-slots
+        n->PS.why = "reactions with two non-hub reactants need the two-species-per-thread kernel";
     }
     if (net_smem(n) > 227 * 1024) {
         delete n;
@@ -903,6 +916,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     info->pull_wavefronts = static_cast<int>(n->PS.conflict_wavefronts);
     info->pull_wavefronts_ideal = static_cast<int>(n->PS.ideal_wavefronts);
     info->pull_threads = n->PS.ok ? n->PS.T : 0;
+    info->pull_nslots = n->PS.ok ? n->PS.nslots : 0;
     return NET_OK;
 }
 
@@ -943,6 +957,9 @@ int net_schedule_table(const net_t* n, const char* name, int* out, int cap) {
         else if (key == "pull_slot_rxn") emit(P.slot_rxn, 1, 1);
         else if (key == "pull_slot_f1") emit(P.slot_f1, 1, 1);
         else if (key == "pull_slot_f2") emit(P.slot_f2, 1, 1);
+        else if (key == "pull_n_nslots") emit(P.n_nslots, 1, 1);
+        else if (key == "pull_nslot_rxn") emit(P.nslot_rxn, 1, 1);
+        else if (key == "pull_nslot_f1") emit(P.nslot_f1, 1, 1);
         else if (key == "pull_agg_ptr") emit(P.agg_ptr, 1, 1);
         else if (key == "pull_agg_ent") emit(P.agg_ent, 1, 1);
         else return fail(NET_EINVAL, "unknown schedule table '" + key + "'");

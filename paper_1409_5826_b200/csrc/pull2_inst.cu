@@ -16,7 +16,7 @@ pull_fn PULL_FN(const PullSchedule& P) { return pick_pull2<PULL_REAL, PULL_ADAPT
 bool pull2_supported(const PullSchedule& P, int* spill) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2) || pick_pull2<double, true>(P) == nullptr) return false;
-    if (spill) *spill = pull2_cap_a(sa) - kPull2RegA + kPull2SpillB;
+    if (spill) *spill = pull2_cap_a(sa) - kPull2RegA + kPull2SpillB + (P.nslots > 0 ? 2 * kPullNSlots : 0);
     return true;
 }
 #endif

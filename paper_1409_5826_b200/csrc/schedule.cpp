@@ -445,20 +445,31 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
     // ---- per reaction: owner, co-reactant class, factors ---------------------------
     struct Rx {
         int owner, cls, co[2], nco;
+        int hh_a = -1, hh_b = -1;  // the two non-hub reactants of a heavy + heavy reaction
     };
     std::vector<Rx> rx(M);
     for (int r = 0; r < M; ++r) {
-        int heavy = -1, nheavy = 0;
+        int heavy = -1, heavy0 = -1, nheavy = 0;
         for (int q = 0; q < n_react[r]; ++q) {
             const int s = react[r * kMaxReact + q];
             if (hub_index[s] < 0) {
+                if (nheavy == 0) heavy0 = s;
                 heavy = s;
                 ++nheavy;
             }
         }
-        if (nheavy > 1)
-            return reject("reaction " + std::to_string(r) + " has more than one non-hub reactant");
+        if (nheavy > 2 || (nheavy == 2 && n_react[r] > 2))
+            return reject("reaction " + std::to_string(r) +
+                          " has two non-hub reactants next to a third reactant");
         Rx& x = rx[r];
+        if (nheavy == 2) {  // heavy + heavy: N-slots and two-factor P-slots, no rate-sum class
+            x.owner = heavy0;
+            x.hh_a = heavy0;
+            x.hh_b = heavy;
+            x.nco = 0;
+            x.cls = -1;
+            continue;
+        }
         x.owner = nheavy == 1 ? heavy : react[r * kMaxReact];
         x.nco = 0;
         bool skipped = false;
@@ -494,6 +505,33 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         for (int i = 0; i < N; ++i)
             if (hub_index[i] < 0) rest.push_back(i);
         std::stable_sort(rest.begin(), rest.end(), [&](int a, int b) { return indeg[a] > indeg[b]; });
+        // Species with N-slots (reactants of heavy + heavy reactions) go next to each other, at
+        // the rank of the first of them, shifted so that the block stays inside one warp when
+        // it fits: the N-slot gathers are skipped by every warp that has none.
+        std::vector<char> special(N, 0);
+        for (int r = 0; r < M; ++r)
+            if (rx[r].hh_a >= 0) special[rx[r].hh_a] = special[rx[r].hh_b] = 1;
+        std::vector<int> sp, ord;
+        int first_rank = -1;
+        for (size_t k = 0; k < rest.size(); ++k) {
+            if (special[rest[k]]) {
+                if (first_rank < 0) first_rank = static_cast<int>(ord.size());
+                sp.push_back(rest[k]);
+            } else {
+                ord.push_back(rest[k]);
+            }
+        }
+        if (!sp.empty()) {
+            int start = first_rank + P.nbs;  // thread index of the block
+            const int ns = static_cast<int>(sp.size());
+            if (ns <= 32 && start / 32 != (start + ns - 1) / 32) {
+                const int back = (start / 32 + 1) * 32 - ns;  // slide back to end at the warp's last lane
+                start = back >= P.nbs ? back : (start / 32 + 1) * 32;
+            }
+            rest.assign(ord.begin(), ord.begin() + std::min<size_t>(ord.size(), start - P.nbs));
+            rest.insert(rest.end(), sp.begin(), sp.end());
+            rest.insert(rest.end(), ord.begin() + std::min<size_t>(ord.size(), start - P.nbs), ord.end());
+        }
         int t = P.nbs;
         for (int i : rest) {
             P.owner[t] = i;
@@ -575,7 +613,12 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         uint16_t f1, f2;
         bool two;
     };
+    struct NSlot {
+        int32_t rxn;
+        uint16_t f1;
+    };
     std::vector<std::vector<Slot>> slots(T);
+    std::vector<std::vector<NSlot>> nsl(T);
     std::vector<std::vector<std::vector<int32_t>>> agg(T, std::vector<std::vector<int32_t>>(kPullCoefs));
     // the constant one: YP[4T .. 4T+3]; second factors default to the copy in bank 3,
     // clear of the hub words 0..2 they are gathered next to
@@ -584,7 +627,17 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
     for (int r = 0; r < M; ++r) {  // reaction order = fixed, documented summation order
         const Rx& x = rx[r];
         const int t_own = P.thread_of[x.owner];
-        agg[t_own][x.cls].push_back(r | (1 << 24));
+        const bool hh = x.hh_a >= 0;
+        if (hh) {  // F- of the two reactants: k_a += nu R Y_b (twice the flux over Y_a when a == b)
+            const int ta = P.thread_of[x.hh_a], tb = P.thread_of[x.hh_b];
+            if (ta == tb) nsl[ta].push_back({r | (2 << 24), static_cast<uint16_t>(ta)});
+            else {
+                nsl[ta].push_back({r | (1 << 24), static_cast<uint16_t>(tb)});
+                nsl[tb].push_back({r | (1 << 24), static_cast<uint16_t>(ta)});
+            }
+        } else {
+            agg[t_own][x.cls].push_back(r | (1 << 24));
+        }
         for (int q = 0; q < n_prod[r]; ++q) {
             const int s = prod[r * kMaxProd + q];
             bool first = true;
@@ -593,7 +646,14 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
             if (!first) continue;
             for (int u = 0; u < n_prod[r]; ++u) nu += prod[r * kMaxProd + u] == s;
             const int h = hub_index[s];
-            if (h >= 0) {
+            if (hh) {  // any product, a hub's own thread included: R * Y_a * Y_b at the consumer
+                Slot sl;
+                sl.rxn = r | (nu << 24);
+                sl.f1 = static_cast<uint16_t>(P.thread_of[x.hh_a]);
+                sl.two = true;
+                sl.f2 = static_cast<uint16_t>(P.thread_of[x.hh_b]);
+                slots[P.thread_of[s]].push_back(sl);
+            } else if (h >= 0) {
                 int slot;
                 if (x.nco == 0) slot = 10 + h;
                 else if (x.nco == 1 && x.co[0] != h) {
@@ -633,6 +693,10 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
         return reject("a non-hub species has more than " + std::to_string(kPullMaxSlots2) +
                       " incoming three-body reactions");
     if (P.agg_max > 65535) return reject("rate-sum list too long");
+    for (int t = 0; t < T; ++t) P.nslots = std::max<int>(P.nslots, nsl[t].size());
+    if (P.nslots > kPullNSlots)
+        return reject("a species enters more than " + std::to_string(kPullNSlots) +
+                      " reactions with another non-hub reactant");
 
     // ---- positions: bank-conflict-aware order of every thread's slots ------------------
     const int lanes = 128 / elem_bytes;
@@ -683,6 +747,16 @@ void build_pull_schedule(int N, int M, const int* n_react, const int* react, con
             for (int32_t v : agg[t][c]) P.agg_ent[static_cast<size_t>(q++) * T + t] = v;
         }
         P.agg_ptr[static_cast<size_t>(kPullCoefs) * T + t] = static_cast<uint16_t>(q);
+    }
+    P.n_nslots.assign(T, 0);
+    P.nslot_rxn.assign(static_cast<size_t>(kPullNSlots) * T, -1);
+    P.nslot_f1.assign(static_cast<size_t>(kPullNSlots) * T, one_word);
+    for (int t = 0; t < T; ++t) {
+        P.n_nslots[t] = static_cast<uint8_t>(nsl[t].size());
+        for (size_t e = 0; e < nsl[t].size(); ++e) {
+            P.nslot_rxn[e * T + t] = nsl[t][e].rxn;
+            P.nslot_f1[e * T + t] = nsl[t][e].f1;
+        }
     }
     // holes (rate 0): read a word some lane of the same piece reads at that position
     // anyway, so that the hole costs no wavefront of its own

@@ -76,15 +76,21 @@ int build_schedule(int N, const int* A, int M, const int* n_react, const int* re
 //     zone per call (T9 and rho are frozen over the hydro step, PAPER.md L47,
 //     L197, L202);
 //   * the hub rows are reduced over the CTA in a fixed order (no atomics).
-// A network qualifies (ok) when every reaction has at most one non-hub reactant,
-// reactions with a hub product have at most one hub co-reactant different from
-// that product, and the capacities below hold; anything else runs on the generic
-// flux-array kernel.
+//   * a reaction with TWO non-hub reactants a + b (the 12C+12C, 12C+16O, 16O+16O class of
+//     the paper's Type Ia network) has no rate-sum form: its flux needs the
+//     abundance of another thread.  Its products -- hubs included, on the hub's own thread --
+//     get two-factor P-slots R * YP[0][t_a] * YP[0][t_b]; each reactant gets an "N-slot"
+//     k_a += nu R * YP[0][t_b], gathered beside the P-slots (k = F-/y, Eq. (1)).
+// A network qualifies (ok) when every reaction has at most two non-hub reactants, those
+// with two have no hub co-reactant, reactions with one non-hub reactant and a hub product
+// have at most one hub co-reactant different from that product, and the capacities below
+// hold; anything else runs on the generic flux-array kernel.
 constexpr int kPullHubs = 3;
 constexpr int kPullClasses = 10;  // co-reactant classes: {}, {h}, {h,h'} (h <= h')
 constexpr int kPullCoefs = 19;    // K[10], G0[3], Gx[3][2]
 constexpr int kPullMaxSlots = 24; // P-slots per thread (largest kernel instantiation)
 constexpr int kPullMaxSlots2 = 8; // P-slots per thread with a second factor
+constexpr int kPullNSlots = 4;    // N-slots per thread (reactions it enters with another non-hub reactant)
 
 struct PullSchedule {
     bool ok = false;
@@ -100,6 +106,10 @@ struct PullSchedule {
     std::vector<int32_t> slot_rxn;     // [slots][T] reaction | nu << 24, -1 = hole
     std::vector<uint16_t> slot_f1;     // [slots][T] YP word index c*T + t of the first factor
     std::vector<uint16_t> slot_f2;     // [slots2][T] YP word index of the second factor (4T+3 = one)
+    int nslots = 0;                    // max N-slots of any thread (0: no reaction has two non-hub reactants)
+    std::vector<uint8_t> n_nslots;     // [T]
+    std::vector<int32_t> nslot_rxn;    // [kPullNSlots][T] reaction | nu << 24, -1 = hole
+    std::vector<uint16_t> nslot_f1;    // [kPullNSlots][T] YP word index of the partner's abundance
     // rate sums: coefficient s of thread t = sum of nu * R over agg_ent[agg_ptr[s][t] .. agg_ptr[s+1][t])
     int agg_max = 0;
     std::vector<uint16_t> agg_ptr;     // [kPullCoefs + 1][T]

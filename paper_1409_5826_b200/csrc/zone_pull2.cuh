@@ -39,12 +39,12 @@ bool pull2_supported(const PullSchedule& P, int* spill);
 #ifdef KINNET_PULL_INSTANTIATE
 
 // One side (one species) of a thread: everything that is loop invariant.
-template <typename real, int CP, int CPR, int J2>
+template <typename real, int CP, int CPR, int J2, int NS>
 struct PullSide {
     real R[CPR > 0 ? CPR : 1];
     real C[kPullCoefs - kPull2SmemCoefs];  // K by class; G0, Gx are in shared memory
-    uint32_t f1[CP / 2], f2[J2 / 2];
-    int wn, wn2, own;
+    uint32_t f1[(CP + NS) / 2], f2[J2 / 2];  // P-slot offsets, then the N-slot offsets
+    int wn, wn2, wnn, own;
     uint32_t s_pub;
 };
 
@@ -89,11 +89,15 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 // 168 (ptxas derives exactly that from the launch bounds): four 96-thread CTAs, two
 // 192-thread ones.  With fp32 state the rates take half the registers: 128 registers, four
 // warps per scheduler, five 96-thread CTAs (270k -> 300k zone-networks/s on configs[3]).
-template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, bool ADAPT>
+// NS = 4 compiles the N-slots in (networks with heavy + heavy reactions, schedule.h): four more
+// gathers per side into k, skipped by the warps none of whose species has one, and the hub
+// owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
+template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT>
 __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
+    static_assert(NS == 0 || NS == kPullNSlots, "N-slot capacity");
     constexpr int T = TB, NW = TB / 32, TV = 2 * TB;  // physical threads, warps; virtual threads
     constexpr int CPRA = CPA - SPA, CPRB = CPB - SPB;  // slots whose rate stays in a register
     constexpr uint32_t SZ = sizeof(real);
@@ -106,8 +110,8 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     double* redq = reinterpret_cast<double*>(smem_raw);       // [32] per-warp q maxima, [16..18] own terms
     real* red = reinterpret_cast<real*>(redq + 32);           // [NW][8] per-warp hub-row sums
     real* YP = red + NW * 8;                                  // [4][TV] published products, then 1
-    real* Rx = YP + 4 * TV + 4;                               // [SPA + SPB][T] spilled slot rates
-    real* Gs = Rx + (SPA + SPB) * T;                                  // [9][TV] G0, Gx of every virtual thread
+    real* Rx = YP + 4 * TV + 4;                               // [SPA + SPB + 2 NS][T] spilled slot rates, N-slot rates
+    real* Gs = Rx + (SPA + SPB + 2 * NS) * T;                         // [9][TV] G0, Gx of every virtual thread
     double* Rbuf = reinterpret_cast<double*>(Gs + kPull2SmemCoefs * TV);  // [M] rates, set-up only
     uint32_t s_redq;
     asm volatile("mov.u32 %0, %1;"
@@ -116,12 +120,13 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     const uint32_t s_red = s_redq + 32 * 8;
     const uint32_t s_YP = s_red + NW * 8 * SZ;
     const uint32_t s_Rx = s_YP + (4 * TV + 4) * SZ + tid * SZ;
-    const uint32_t s_own = s_redq + 16 * 8;
-    const uint32_t s_G = s_YP + (4 * TV + 4 + (SPA + SPB) * T) * SZ;
+    const uint32_t s_own = s_redq + 16 * 8;   // [3] own-consumption terms of the hub owners
+    const uint32_t s_ownp = s_redq + 20 * 8;  // [3] their own P-slot sums (NS > 0)
+    const uint32_t s_G = s_YP + (4 * TV + 4 + (SPA + SPB + 2 * NS) * T) * SZ;
     if (s_YP + (4 * TV + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
 
-    PullSide<real, CPA, CPRA, J2> A;
-    PullSide<real, CPB, CPRB, J2> B;
+    PullSide<real, CPA, CPRA, J2, NS> A;
+    PullSide<real, CPB, CPRB, J2, NS> B;
 #pragma unroll
     for (int e = 0; e < CPA / 2; ++e) A.f1[e] = p.f1_pack[e * TV + va] + s_YP * 0x10001u;
 #pragma unroll
@@ -131,8 +136,15 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         A.f2[e] = p.f2_pack[e * TV + va] + s_YP * 0x10001u;
         B.f2[e] = p.f2_pack[e * TV + vb] + s_YP * 0x10001u;
     }
+#pragma unroll
+    for (int e = 0; e < NS / 2; ++e) {  // N-slots: the rows after the largest P-slot capacity
+        A.f1[CPA / 2 + e] = p.f1_pack[(kPullMaxSlots / 2 + e) * TV + va] + s_YP * 0x10001u;
+        B.f1[CPB / 2 + e] = p.f1_pack[(kPullMaxSlots / 2 + e) * TV + vb] + s_YP * 0x10001u;
+    }
     {
         const uint32_t ca = p.cnt[va], cb = p.cnt[vb];
+        A.wnn = __reduce_max_sync(0xffffffffu, (ca >> 16) & 255u);
+        B.wnn = __reduce_max_sync(0xffffffffu, (cb >> 16) & 255u);
         A.wn = __reduce_max_sync(0xffffffffu, ca & 255u);  // warp-wide trip counts
         A.wn2 = __reduce_max_sync(0xffffffffu, (ca >> 8) & 255u);
         B.wn = __reduce_max_sync(0xffffffffu, cb & 255u);
@@ -174,6 +186,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         const real r = slot_rate(e, vb);
         if (e < CPRB) B.R[e] = r;
         else Rx[(SPA + e - CPRB) * T + tid] = r;
+    }
+#pragma unroll
+    for (int e = 0; e < NS; ++e) {
+        Rx[(SPA + SPB + e) * T + tid] = slot_rate(kPullMaxSlots + e, va);
+        Rx[(SPA + SPB + NS + e) * T + tid] = slot_rate(kPullMaxSlots + e, vb);
     }
     auto rate_sums = [&](real (&C)[kPullCoefs - kPull2SmemCoefs], int v) {
         int q = p.agg_ptr[v];
@@ -363,6 +380,29 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             Fpa = (sa0 + sa1) + (sa2 + sa3);
             Fpb = (sb0 + sb1) + (sb2 + sb3);
         }
+        if (NS > 0) {  // N-slots: k += sum nu R Y_partner, F- of the reactants of heavy + heavy reactions
+            constexpr uint32_t NA = (SPA + SPB) * T * SZ, NB = (SPA + SPB + NS) * T * SZ, ROW = T * SZ;
+            if (A.wnn > 0) {  // warp-uniform: the schedule keeps these species in one warp
+                const uint32_t w0 = A.f1[CPA / 2], w1 = A.f1[(CPA + NS) / 2 - 1];
+                const real n0 = lds_at<real>(lo16(w0)), n1 = lds_at<real>(hi16(w0));
+                const real n2 = lds_at<real>(lo16(w1)), n3 = lds_at<real>(hi16(w1));
+                const real u0 = lds_at<real>(s_Rx + NA) * n0, u1 = lds_at<real>(s_Rx + NA + ROW) * n1;
+                const real u2 = fma(lds_at<real>(s_Rx + NA + 2 * ROW), n2, u0);
+                const real u3 = fma(lds_at<real>(s_Rx + NA + 3 * ROW), n3, u1);
+                ka += u2 + u3;
+            }
+            if (B.wnn > 0) {
+                const uint32_t w0 = B.f1[CPB / 2], w1 = B.f1[(CPB + NS) / 2 - 1];
+                const real n0 = lds_at<real>(lo16(w0)), n1 = lds_at<real>(hi16(w0));
+                const real n2 = lds_at<real>(lo16(w1)), n3 = lds_at<real>(hi16(w1));
+                const real u0 = lds_at<real>(s_Rx + NB) * n0, u1 = lds_at<real>(s_Rx + NB + ROW) * n1;
+                const real u2 = fma(lds_at<real>(s_Rx + NB + 2 * ROW), n2, u0);
+                const real u3 = fma(lds_at<real>(s_Rx + NB + 3 * ROW), n3, u1);
+                kb += u2 + u3;
+            }
+            // a hub made by heavy + heavy reactions gathers those fluxes on its own thread
+            if (hub_owner) sts(s_ownp + tid * SZ, Fpa);
+        }
 
         // ---- S5: q candidates of the non-hub species: |F+ - F-| / (eps max(y, floor)) ------
         const real cha = fma(-ka, ya, Fpa), chb = fma(-kb, yb, Fpb);
@@ -400,6 +440,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
                 }
             hFp = vp[0];
             hFm = vm[0] + own_term;
+            if (NS > 0) hFp += lds_at<real>(s_ownp + lane * SZ);
         }
         if (!ADAPT && rhs_only) {
             real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
@@ -513,14 +554,17 @@ inline bool pull2_sides(const PullSchedule& P, int& slots_a, int& slots_b, int& 
 inline int pull2_cap_a(int slots_a) { return slots_a <= 20 ? 20 : 24; }
 
 template <typename real, int TB, int CPA, bool ADAPT>
-pull_fn pick_pull2_j2(int s2) {
-    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 4, ADAPT>;
-    return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, ADAPT>;
+pull_fn pick_pull2_j2(int s2, int ns) {
+    // networks with N-slots have two-factor P-slots anyway: one second-factor class for them
+    if (ns > 0)
+        return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, kPullNSlots, ADAPT>;
+    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 4, 0, ADAPT>;
+    return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, 0, ADAPT>;
 }
 template <typename real, int TB, bool ADAPT>
-pull_fn pick_pull2_cap(int sa, int s2) {
-    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2);
-    return pick_pull2_j2<real, TB, 24, ADAPT>(s2);
+pull_fn pick_pull2_cap(int sa, int s2, int ns) {
+    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2, ns);
+    return pick_pull2_j2<real, TB, 24, ADAPT>(s2, ns);
 }
 template <typename real, bool ADAPT>
 pull_fn pick_pull2(const PullSchedule& P) {
@@ -528,12 +572,12 @@ pull_fn pick_pull2(const PullSchedule& P) {
     if (!pull2_sides(P, sa, sb, s2)) return nullptr;
     if (sa > 24 || sb > kPull2CapB || s2 > kJ2C) return nullptr;
     switch (P.T / 2) {
-        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2);
-        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2);
-        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2);
-        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2);
-        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2);
-        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2);
+        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2, P.nslots);
+        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2, P.nslots);
+        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2, P.nslots);
+        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2, P.nslots);
+        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2, P.nslots);
+        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2, P.nslots);
         default: return nullptr;
     }
 }

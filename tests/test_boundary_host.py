@@ -173,9 +173,10 @@ PAIRS = {4: (0, 0), 5: (0, 1), 6: (0, 2), 7: (1, 1), 8: (1, 2), 9: (2, 2)}
 
 def pull_entries(net, kn):
     """Every (species, sign, reaction) term the pull kernel accounts for, rebuilt
-    from its tables alone: P-slots give F+ of non-hub species; rate-sum
-    coefficient K_c gives the owner's F- and the F- of the hubs in class c;
-    G0/Gx give F+ of the hubs."""
+    from its tables alone: P-slots give F+ of non-hub species (and of hubs made by
+    heavy + heavy reactions); rate-sum coefficient K_c gives the owner's F- and the
+    F- of the hubs in class c; G0/Gx give F+ of the hubs; N-slots give F- of the two
+    non-hub reactants of a heavy + heavy reaction."""
     info = kn.schedule_info()
     assert info["pull_ok"] == 1
     T = info["pull_threads"]
@@ -198,16 +199,19 @@ def pull_entries(net, kn):
                 assert f1[e, t] <= 4 * T and (e >= f2.shape[0] or f2[e, t] == 4 * T + 3)
                 continue
             assert e < ns[t]
-            assert owner[t] >= 0 and owner[t] not in hub
+            assert owner[t] >= 0
             r, nu = int(rxn[e, t]) & 0xFFFFFF, int(rxn[e, t]) >> 24
             ent[(int(owner[t]), "+", r)] += nu
             # the factors of the slot reproduce the reactant multiset of the reaction
             c1, t1 = divmod(int(f1[e, t]), T)
             react = [int(owner[t1])] + ([hub[c1 - 1]] if c1 else [])
-            if e < f2.shape[0] and f2[e, t] != 4 * T + 3:  # second factor: a hub's own word
-                assert e < ns2[t] and f2[e, t] < len(hub)
+            if e < f2.shape[0] and f2[e, t] != 4 * T + 3:  # second factor: a species' own word
+                assert e < ns2[t] and f2[e, t] < T
                 react.append(int(owner[f2[e, t]]))
             assert sorted(react) == sorted(int(s) for s in net.react[r, : net.n_react[r]])
+            heavy = [x for x in react if x not in hub]
+            # a hub's own thread gathers only what heavy + heavy reactions make of it
+            assert owner[t] not in hub or len(heavy) == 2
         for s in range(19):
             for q in range(ptr[s, t], ptr[s + 1, t]):
                 r, nu = int(agg[q, t]) & 0xFFFFFF, int(agg[q, t]) >> 24
@@ -227,7 +231,38 @@ def pull_entries(net, kn):
                     other = [x for x in range(3) if x != h][j]
                     ent[(hub[h], "+", r)] += nu
                     assert sorted(int(x) for x in net.react[r, :2]) == sorted([int(owner[t]), hub[other]])
+    nn = kn.schedule_table("pull_n_nslots")
+    nrx = kn.schedule_table("pull_nslot_rxn").reshape(4, T)
+    nf1 = kn.schedule_table("pull_nslot_f1").reshape(4, T)
+    assert nn.max(initial=0) == info["pull_nslots"]
+    for t in range(T):
+        for e in range(4):
+            if nrx[e, t] == -1:
+                assert e >= nn[t] and nf1[e, t] == 4 * T
+                continue
+            assert e < nn[t] and owner[t] >= 0 and owner[t] not in hub and nf1[e, t] < T
+            r, nu = int(nrx[e, t]) & 0xFFFFFF, int(nrx[e, t]) >> 24
+            partner = int(owner[nf1[e, t]])
+            assert partner not in hub and net.n_react[r] == 2
+            assert sorted([int(owner[t]), partner]) == sorted(int(x) for x in net.react[r, :2])
+            assert nu == (2 if partner == owner[t] else 1)
+            ent[(int(owner[t]), "-", r)] += nu
     return ent, info
+
+
+def test_pull_schedule_heavy_pairs():
+    """hub150hh: 16 reactions with two non-hub reactants (one of them an identical pair) and
+    their inverses stay on the two-species pull kernel; every term is still there once."""
+    net = network("hub150hh")
+    heavy = [r for r in range(net.n_reactions)
+             if sum(1 for s in net.react[r, : net.n_react[r]] if s >= 3) == 2]
+    assert len(heavy) == 16 and any(net.react[r, 0] == net.react[r, 1] for r in heavy)
+    kn = K.Net(net, host_only=True)
+    got, info = pull_entries(net, kn)
+    assert got == expected_entries(net)
+    assert info["kernel"] == 2 and 1 <= info["pull_nslots"] <= 4
+    # the one-species kernel is not instantiated with N-slots: generic fallback
+    assert K.Net(net, K.NetParams(kernel=2), host_only=True).schedule_info()["kernel"] == 0
 
 
 @pytest.mark.parametrize("kernel", [0, 2])
