@@ -28,7 +28,12 @@ UNIT = "zone-networks/s"
 ZONES_PER_GPU = 16384
 T_HYDRO = 1e-6
 PROFILE_SEED = 4
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the zone kernel on the default
+# workload, from the `ncu --set full` capture summarised in the file named beside it (the
+# writes of the last zones are still in L2 when the capture ends).  Reported only for that
+# exact configuration; any other run reports null.
 DRAM_BYTES_PER_LAUNCH = 20463360
+DRAM_BYTES_SOURCE = "profiles/r01e_pull2_kernel.md"
 
 # Algorithmic work per zone per sub-step: one multiply per
 # reactant of every reaction, one add per F+/F- entry, ~10 flops per species for
@@ -39,6 +44,21 @@ def algorithmic_work(net, n_entries):
     flops = n_react_total + n_entries + 10 * net.n_species
     smem_bytes = 8 * (n_react_total + net.n_reactions + n_entries + 5 * net.n_species)
     return flops, smem_bytes
+
+
+def pull_design_smem_bytes(kn, info, ybytes):
+    """Shared-memory bytes per zone-substep that the PULL design itself must move (DESIGN.md
+    section 6), counted from the compiled schedule, not from the kernel: every species publishes
+    4 words; every P-slot reads one word, plus one per second factor; every N-slot reads one;
+    the six hub rows go through shared memory once per warp (one store and one load each)."""
+    if not info["pull_ok"] or info["kernel"] == 0:
+        return None
+    T = info["pull_threads"]
+    pslots = int((kn.schedule_table("pull_slot_rxn") >= 0).sum())
+    second = int((kn.schedule_table("pull_slot_f2") != 4 * T + 3).sum()) if info["pull_slots2"] else 0
+    nslots = int(kn.schedule_table("pull_n_nslots").sum())
+    warps = info["threads"] // 32
+    return ybytes * (4 * info["n_species"] + pslots + second + nslots + 2 * 6 * warps)
 
 
 # FP64 / shared-memory peaks: measured on this pool's B200 with
@@ -108,11 +128,15 @@ def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU, name: st
     rank r integrates the contiguous shard r (no data-path collective)."""
     from gen import perturbed_co_start, zone_profile
     from gen.configs import network
-    from paper_1409_5826_b200.shard import zone_shard
 
     net = network(name)
     total = zones_per_gpu * world
-    lo, hi = zone_shard(total, rank, world)
+    if world == 1:  # (the reference arm comes through here: it must not load the product library)
+        lo, hi = 0, total
+    else:
+        from paper_1409_5826_b200.shard import zone_shard
+
+        lo, hi = zone_shard(total, rank, world)
     T9, rho = zone_profile(total, PROFILE_SEED)
     Y0 = perturbed_co_start(net, total, seed=1000 + PROFILE_SEED)
     return net, T9[lo:hi].copy(), rho[lo:hi].copy(), Y0[lo:hi].copy()
@@ -144,6 +168,20 @@ def cpu_baseline(net, T9, rho, Y0, target_s=15.0):
             "sample": f"first {n} of {len(T9)} zones of the same workload, {steps} sub-steps, "
                       f"{best:.2f} s, gcc -O2 -ffp-contract=off, OpenMP dynamic over zones",
             "zone_substeps_per_s": steps / best}
+
+
+def cpu_baseline_1core(net, T9, rho, Y0, zones=64):
+    """BASELINE.md CPU-baseline plan (i): the oracle on ONE host core, first `zones` zones."""
+    from oracle import Oracle
+
+    o = Oracle(net)
+    t0 = time.perf_counter()
+    out = o.integrate(T9[:zones], rho[:zones], Y0[:zones], T_HYDRO, n_threads=1)
+    el = time.perf_counter() - t0
+    steps = int(out["n_steps"].sum())
+    return {"value": zones / el, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {zones} zones of the same workload, {steps} sub-steps, {el:.2f} s, one thread",
+            "zone_substeps_per_s": steps / el}
 
 
 def run_reference(args):
@@ -247,31 +285,97 @@ def run_ours(args):
     substeps = int(n_steps.sum().item())
     assert int(status.max().item()) == 0, "a zone reported a status bit"
 
-    # ---- e2e: same call through the host-buffer entry point, copies inside --
-    Yp = torch.from_numpy(Y0h.copy()).pin_memory()
+    # ---- e2e: the same step through the host-buffer entry point ------------------
+    # pinned HOST buffers in, results back in pinned HOST buffers, everything inside the timed
+    # region.  Default: zero-copy (the zone kernel reads and writes the mapped host buffers
+    # itself).  Also timed: the staged path (cudaMemcpyAsync through device scratch).
     Ysrc = torch.from_numpy(Y0h.copy())
+    Yp = torch.from_numpy(Y0h.copy()).pin_memory()
     T9p, rhop = torch.from_numpy(T9h.copy()).pin_memory(), torch.from_numpy(rhoh.copy()).pin_memory()
     dtp = torch.zeros(z, dtype=torch.float64).pin_memory()
     stp = torch.zeros(z, dtype=torch.int32).pin_memory()
     sts = torch.zeros(z, dtype=torch.int32).pin_memory()
-    e2e_steps = max(1, min(args.steps, 3))
-    e2e_s = 0.0
-    for it in range(1 + e2e_steps):
-        Yp.copy_(Ysrc)
-        dtp.zero_()
-        barrier()
-        t1 = time.perf_counter()
-        kn.net_integrate_host(z, T9p.numpy(), rhop.numpy(), Yp.numpy(), T_HYDRO, dtp.numpy(),
-                              stp.numpy(), sts.numpy())
-        if it > 0:
-            e2e_s += time.perf_counter() - t1
+    e2e_steps = max(1, min(args.steps, 5))
+
+    def time_host_path(net_obj):
+        total = 0.0
+        for it in range(1 + e2e_steps):
+            Yp.copy_(Ysrc)
+            dtp.zero_()
+            flush.zero_()
+            barrier()
+            t1 = time.perf_counter()
+            net_obj.net_integrate_host(z, T9p.numpy(), rhop.numpy(), Yp.numpy(), T_HYDRO, dtp.numpy(),
+                                       stp.numpy(), sts.numpy())
+            if it > 0:
+                total += time.perf_counter() - t1
+        assert int(sts.max()) == 0 and int(stp.sum()) == substeps
+        return total
+
+    e2e_s = time_host_path(kn)
+    kn_staged = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel, host_chunk=-z))
+    staged_s = time_host_path(kn_staged)
     h2d = z * (N * ybytes + 8 + 8 + 8)
     d2h = z * (N * ybytes + 8 + 4 + 4)
+    steps_host = n_steps.cpu().numpy()
+
+    # ---- secondary points: config 3 and config 5 ---------------
+    extra = {}
+    if world == 1 and not args.no_extra and args.network == "hub150" and args.precision == 64:
+        from gen import build_config
+
+        def dev_t(a, dtype=torch.float64):
+            return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(dev)
+
+        c3 = build_config(3)
+        z3 = c3["zones"]
+        T3, r3, Y3 = dev_t(c3["T9"]), dev_t(c3["rho"]), dev_t(c3["Y0"])
+        Yw, dtw = torch.empty_like(Y3), torch.zeros(z3, dtype=torch.float64, device=dev)
+        st3 = torch.zeros(z3, dtype=torch.int32, device=dev)
+        best3, sub3 = None, 0
+        for it in range(3):
+            Yw.copy_(Y3)
+            dtw.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            sub3 = 0
+            e0.record(stream)
+            for _ in range(c3["calls"]):
+                kn.net_integrate(z3, T3, r3, Yw, c3["t_hydro"], dtw, st3, None, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best3 = ms if best3 is None else min(best3, ms)
+        extra["config3"] = {"what": "configs[2]: 128 zones x 10 consecutive hydro steps, dt carried (best of 3)",
+                            "ms_per_10_calls": best3, "zone_networks_per_s": z3 * c3["calls"] / (best3 * 1e-3)}
+        c5 = build_config(5)
+        k5 = K.Net(c5["network"])
+        z5 = c5["zones"]
+        T5, r5, Y5 = dev_t(c5["T9"]), dev_t(c5["rho"]), dev_t(c5["Y0"])
+        Yw, dtw = torch.empty_like(Y5), torch.zeros(z5, dtype=torch.float64, device=dev)
+        st5 = torch.zeros(z5, dtype=torch.int32, device=dev)
+        best5 = None
+        for it in range(3):
+            Yw.copy_(Y5)
+            dtw.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            k5.net_integrate(z5, T5, r5, Yw, c5["t_hydro"], dtw, st5, None, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best5 = ms if best5 is None else min(best5, ms)
+        sub5 = int(st5.sum().item())
+        extra["config5"] = {"what": "configs[4]: hub365 (365sp/4400rx), 4096 zones, one hydro step (best of 3)",
+                            "ms": best5, "zone_networks_per_s": z5 / (best5 * 1e-3), "sub_steps": sub5,
+                            "ns_per_zone_substep": best5 * 1e6 / sub5,
+                            "kernel": k5.schedule_info()["kernel"], "threads_per_zone": k5.schedule_info()["threads"]}
 
     # ---- max over ranks ---------------------------------------------------
     from paper_1409_5826_b200.shard import reduce_job
 
-    (total_ms, e2e_s), (substeps_all,) = reduce_job([total_ms, e2e_s], [substeps], device=dev)
+    best_ms, median_ms = float(np.min(kernel_ms)), float(np.median(kernel_ms))
+    (total_ms, e2e_s, staged_s, best_ms, median_ms), (substeps_all,) = reduce_job(
+        [total_ms, e2e_s, staged_s, best_ms, median_ms], [substeps], device=dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -280,52 +384,79 @@ def run_ours(args):
     ms_per_step = total_ms / args.steps
     value = z * world / (ms_per_step * 1e-3)
     e2e_value = z * world / (e2e_s / e2e_steps)
+    staged_value = z * world / (staged_s / e2e_steps)
     flops, smem_b = algorithmic_work(net, info["n_entries"])
+    pull_b = pull_design_smem_bytes(kn, info, ybytes)
     fp64_peak, smem_peak, peak_src = load_peaks()
     per_launch_substeps = substeps  # rank 0's launch
     k_ms = float(np.mean(kernel_ms))
     fp64_ach = flops * per_launch_substeps / (k_ms * 1e-3) / 1e12
-    smem_ach = smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12
-    # dram__bytes_read.sum + dram__bytes_write.sum of one 16384-zone launch, from the
-    # ncu --set full capture summarised in profiles/r01e_pull2_kernel.md (20.46 MB read + 3.8 KB written)
-    traffic = DRAM_BYTES_PER_LAUNCH if z == ZONES_PER_GPU else None
+    default_run = (z == ZONES_PER_GPU and args.precision == 64 and args.kernel == 0 and args.network == "hub150")
+    traffic = DRAM_BYTES_PER_LAUNCH if default_run else None
+    dtype = "f64" if args.precision == 64 else "f32"
+    kname = ({0: "zone_kernel", 1: "zone_kernel_pull", 2: "zone_kernel_pull2"}[info["kernel"]]
+             + f"<{'double' if args.precision == 64 else 'float'}, adaptive>")
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC if args.precision == 64 else METRIC.replace("fp64", "fp32 study"),
+        "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+        "scaling": "weak", "vs_baseline": None, "dtype": dtype,
         "data": "synthetic",
         "config": {
-            "workload": "configs[3]: synthetic 150sp/1604rx hub network (seed 1409), 16384 zones per GPU, "
-                        "T9~U[1,10], log10 rho~U[7,9.5] (seed 4), lognormal-perturbed C/O start, "
-                        "one hydro step of 1e-6 s, adaptive dt",
+            "workload": f"configs[3]: synthetic 150sp/{net.n_reactions}rx hub network ({args.network}, seed 1409), "
+                        "16384 zones per GPU, T9~U[1,10], log10 rho~U[7,9.5] (seed 4), lognormal-perturbed "
+                        "C/O start, one hydro step of 1e-6 s, adaptive dt",
             "zones_per_gpu": z, "sub_steps_per_step": substeps_all,
             "mean_sub_steps_per_zone": substeps_all / (z * world),
+            "sub_steps_per_zone": {"min": int(steps_host.min()), "median": float(np.median(steps_host)),
+                                   "p99": float(np.percentile(steps_host, 99)), "max": int(steps_host.max())},
             "l2": "256 MB buffer written between timed iterations (L2 flush)",
             "parallelism": f"zones sharded contiguously over {world} GPU(s), no collective",
             "threads_per_zone": info["threads"], "zones_per_sm": info["zones_per_sm"],
         },
+        "ms_per_step_best": best_ms, "ms_per_step_median": median_ms,
+        "value_best": z * world / (best_ms * 1e-3), "value_median": z * world / (median_ms * 1e-3),
         "zone_substeps_per_s": substeps_all / (ms_per_step * 1e-3),
         "wall_s_timed_region": wall,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e2e_steps, "api": "net_integrate_host (pinned host buffers)"},
-        "gpu_launches": 2 * args.steps,  # per step: the launch-order kernel and the zone kernel
+                "steps": e2e_steps,
+                "api": "net_integrate_host on pinned host buffers: zero-copy -- the zone kernel reads each "
+                       "zone's inputs from, and writes its results to, the mapped host buffers over the link, "
+                       "inside the timed region; no staging copy",
+                "staged": {"value": staged_value,
+                           "api": "the same call with params.host_chunk < 0: cudaMemcpyAsync H2D, launch, "
+                                  "cudaMemcpyAsync D2H through device scratch"}},
+        # per step: memset + histogram + scatter of the launch order (2 kernels) and the zone kernel
+        "gpu_launches": 3 * args.steps,
         "roofline": {
-            "bound": "alu",
-            "kernel": {0: "zone_kernel", 1: "zone_kernel_pull", 2: "zone_kernel_pull2"}[info["kernel"]]
-                      + f"<{'double' if args.precision == 64 else 'float'}, adaptive>", "achieved": fp64_ach,
-            "peak": fp64_peak, "unit": "TFLOP/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
-            "what": f"{flops} algorithmic FP64 ops per zone-substep x {per_launch_substeps} zone-substeps "
-                    f"per launch / {k_ms:.2f} ms; peak = FP64 non-FMA issue rate, {peak_src}",
+            "bound": "alu", "kernel": kname, "achieved": fp64_ach,
+            "peak": fp64_peak, "unit": "Tinstr/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
+            "what": f"{flops} algorithmic FP64 instructions (FMA = 1) per zone-substep x {per_launch_substeps} "
+                    f"zone-substeps per launch / {k_ms:.2f} ms; peak = FP64 issue rate, {peak_src}; "
+                    f"traffic = dram bytes of one launch from the ncu capture in {DRAM_BYTES_SOURCE}"
+                    + ("" if default_run else " (not this configuration: null)"),
         },
-        "roofline_smem": {
-            "bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "TB/s",
-            "frac": smem_ach / smem_peak,
-            "what": f"{smem_b} algorithmic shared-memory bytes per zone-substep; peak {peak_src}",
+        "roofline_smem_direct": {
+            "bound": "smem", "achieved": smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12, "peak": smem_peak,
+            "unit": "TB/s", "frac": smem_b * per_launch_substeps / (k_ms * 1e-3) / 1e12 / smem_peak,
+            "what": f"context only: {smem_b} shared-memory bytes per zone-substep of the DIRECT (flux-array) "
+                    f"design of SURVEY 8(d), which this kernel does not execute; peak {peak_src}",
         },
     }
+    if pull_b is not None:
+        ach = pull_b * per_launch_substeps / (k_ms * 1e-3) / 1e12
+        out["roofline_smem"] = {
+            "bound": "smem", "achieved": ach, "peak": smem_peak, "unit": "TB/s", "frac": ach / smem_peak,
+            "what": f"{pull_b} shared-memory bytes per zone-substep that the pull design must move (4 publishes per "
+                    f"species, one word per P-slot, second factor and N-slot, the hub-row hand-over), counted "
+                    f"from the compiled schedule; peak {peak_src}",
+        }
+    if extra:
+        out["extra"] = extra
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(net, T9h, rhoh, Y0h)
+        out["cpu_baseline_1core"] = cpu_baseline_1core(net, T9h, rhoh, Y0h)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -390,6 +521,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the secondary config 3 / config 5 points")
     ap.add_argument("--zones", type=int, default=ZONES_PER_GPU,
                     help="zones per GPU (profiling only; the metric is quoted at the default)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],

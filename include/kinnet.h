@@ -22,13 +22,22 @@
  *     failure.
  *   - "host" / "device" below says where a pointer must live.  The caller owns
  *     every array it passes.  net_create copies the host tables; the net_t owns
- *     its device copies.  net_integrate* are asynchronous on `cuda_stream` (a
- *     cudaStream_t cast to void*, NULL = default stream) and never synchronise;
- *     the only allocation is net_integrate's launch-order scratch (4 bytes per
- *     zone, owned by the net_t, grown when a call brings more zones than any
- *     before).  One net_t serves one stream at a time: calls on the same net_t
- *     from different streams must be ordered by the caller.  net_integrate_host is the synchronous end-to-end
- *     variant taking host buffers.
+ *     its device copies and its fixed workspaces.  net_integrate* / net_rates / net_rhs
+ *     are asynchronous on `cuda_stream` (a cudaStream_t cast to void*, NULL = default
+ *     stream); they allocate nothing, never synchronise, and are legal under stream
+ *     capture (every operation they enqueue is a kernel launch or a memset node).
+ *   - One net_t may be driven from several streams (and host threads) at once.  The only
+ *     per-call device state is the launch-order workspace of net_integrate (4 bytes per
+ *     zone + 8 KB): the net_t holds 8 of them ("lanes", 65536 zones each after
+ *     net_create, grown by net_reserve), one per stream that calls with >= 1024 zones.
+ *     A call that finds no lane (a ninth stream, or more zones than reserved) still runs
+ *     and returns the same results bit for bit; it only launches the zones in caller
+ *     order instead of hottest first.  A captured call keeps the lane of the stream it
+ *     was captured on: graphs that may replay concurrently must be captured on
+ *     different streams.
+ *   - A net_t belongs to the CUDA device that was current in net_create; calls with
+ *     another device current fail with NET_EINVAL.
+ *   - net_integrate_host / net_integrate_host_async take HOST buffers (end to end).
  *   - Y is zone-major [zones * n_species], molar abundances Y_i = X_i / A_i
  *     (Eq. (2) with X the mass fraction); double when the net was
  *     created with precision 64, float with precision 32 (the paper's
@@ -72,6 +81,9 @@ typedef struct {
                             the two-species kernel also takes reactions with two),
                             else the generic flux-array kernel; 1 = always the generic kernel;
                             2 = the one-species pull kernel when the network qualifies (A/B tests) */
+    int host_chunk;      /* net_integrate_host*: zones per chunk of the staged path; 0 = default
+                            max(16384, zones/16); < 0 = always stage through device scratch, in
+                            chunks of -host_chunk zones, even when the buffers are pinned       */
 } net_params_t;
 
 /* Fill *p with the defaults listed above. */
@@ -127,6 +139,7 @@ int net_integrate(net_t *net, int zones, const double *T9, const double *rho, vo
  * binding-energy table supplied by the caller (units: those of B per mole of species, per
  * gram of matter -- e.g. B in MeV gives MeV mol/g; multiply by N_A to get MeV/g).
  *   net_set_binding_energy  B host [n_species]; copied; may be called again to replace it
+ *                           (synchronises the device first: a launch in flight may read the table)
  *   net_integrate_energy    net_integrate plus energy device [zones] out (NULL = net_integrate);
  *                           fails with NET_EINVAL if no table has been set
  */
@@ -140,11 +153,36 @@ int net_integrate_fixed(net_t *net, int zones, const double *T9, const double *r
                         double dt_fixed, long long n_steps, void *cuda_stream);
 
 /*
- * End-to-end variant: every array is a HOST buffer (pinned for full copy
- * speed).  Copies inputs to net-owned device scratch, integrates, copies the
- * results back and synchronises before returning (the 154-in / 152-out float
- * exchange of PAPER.md L106-110, batched).  Scratch grows on demand.
+ * Grow every launch-order lane to hold max_zones zones (see "Conventions").  Synchronises the
+ * device and reallocates: call it at set-up time, never inside a capture or with launches
+ * in flight on other host threads.  Shrinks nothing.
  */
+int net_reserve(net_t *net, int max_zones);
+
+/*
+ * End-to-end variants: every array is a HOST buffer -- the 154-in / 152-out float exchange of
+ * PAPER.md L106-110, batched (the link and the CPU while the GPU
+ * integrates).
+ *   - Pinned (page-locked) buffers, e.g. cudaHostAlloc / torch pin_memory: ZERO-COPY.  One
+ *     launch over the whole batch; each zone's CTA reads its T9, rho, dt and abundances from the
+ *     mapped host buffers when it starts and writes abundances, dt, steps and status back when
+ *     it ends, so every transfer overlaps the integration of the other zones and the global
+ *     hottest-first order is kept.  No device scratch.
+ *   - Any other host memory: staged through device scratch owned by the net_t (grown on
+ *     demand: that call then synchronises the internal streams and allocates), in chunks of
+ *     params.host_chunk zones over three internal streams, so that the upload of one chunk, the
+ *     kernels of the previous one and the download of the one before overlap; the launch order
+ *     then applies within a chunk.
+ *   net_integrate_host_async  enqueues everything and returns; the host buffers must stay
+ *                             valid and untouched until net_wait returns.  One batch in
+ *                             flight per net_t.
+ *   net_wait                  blocks until the batch enqueued last is back in the host buffers
+ *   net_integrate_host        = net_integrate_host_async + net_wait
+ * Results are bit for bit those of net_integrate on the same zones, on either path.
+ */
+int net_integrate_host_async(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                             double t_hydro, double *dt, int *n_steps, int *status);
+int net_wait(net_t *net);
 int net_integrate_host(net_t *net, int zones, const double *T9, const double *rho, void *Y,
                        double t_hydro, double *dt, int *n_steps, int *status);
 

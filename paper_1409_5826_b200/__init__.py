@@ -22,7 +22,8 @@ NET_STATUS_MAX_STEPS, NET_STATUS_NONFINITE = 1, 2
 
 EXPORTS = (
     "net_default_params", "net_create", "net_create_host", "net_destroy", "net_integrate",
-    "net_integrate_fixed", "net_integrate_host", "net_set_binding_energy", "net_integrate_energy", "net_rates", "net_rhs", "net_schedule_info",
+    "net_integrate_fixed", "net_integrate_host", "net_integrate_host_async", "net_wait", "net_reserve",
+    "net_set_binding_energy", "net_integrate_energy", "net_rates", "net_rhs", "net_schedule_info",
     "net_schedule_table", "net_last_error",
 )
 
@@ -31,7 +32,7 @@ class net_params_t(C.Structure):
     _fields_ = [
         ("kappa", C.c_double), ("eps_y", C.c_double), ("y_floor", C.c_double),
         ("growth", C.c_double), ("max_steps", C.c_longlong), ("precision", C.c_int),
-        ("kernel", C.c_int),
+        ("kernel", C.c_int), ("host_chunk", C.c_int),
     ]
 
 
@@ -67,6 +68,9 @@ def _load() -> C.CDLL:
     lib.net_integrate_energy.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp, vp]
     lib.net_integrate_fixed.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, C.c_longlong, vp]
     lib.net_integrate_host.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp]
+    lib.net_integrate_host_async.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp]
+    lib.net_wait.argtypes = [vp]
+    lib.net_reserve.argtypes = [vp, C.c_int]
     lib.net_rates.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     lib.net_rhs.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp]
     lib.net_schedule_info.argtypes = [vp, C.POINTER(net_schedule_info_t)]
@@ -97,16 +101,17 @@ class NetParams:
     max_steps: int = 10_000_000
     precision: int = 64
     kernel: int = 0  # 0 = automatic, 1 = generic kernel only, 2 = one-species pull kernel
+    host_chunk: int = 0  # staged host path: zones per chunk; < 0 = never zero-copy
 
     def to_c(self) -> net_params_t:
         return net_params_t(self.kappa, self.eps_y, self.y_floor, self.growth, self.max_steps,
-                            self.precision, self.kernel)
+                            self.precision, self.kernel, self.host_chunk)
 
 
 def net_default_params() -> NetParams:
     p = net_params_t()
     _check(lib.net_default_params(C.byref(p)))
-    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel)
+    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel, p.host_chunk)
 
 
 def _ptr(t):
@@ -197,6 +202,16 @@ class Net:
     def net_integrate_host(self, zones, T9, rho, Y, t_hydro, dt=None, n_steps=None, status=None):
         _check(lib.net_integrate_host(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y),
                                       float(t_hydro), _ptr(dt), _ptr(n_steps), _ptr(status)))
+
+    def net_integrate_host_async(self, zones, T9, rho, Y, t_hydro, dt=None, n_steps=None, status=None):
+        _check(lib.net_integrate_host_async(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y),
+                                            float(t_hydro), _ptr(dt), _ptr(n_steps), _ptr(status)))
+
+    def net_wait(self):
+        _check(lib.net_wait(self._h))
+
+    def net_reserve(self, max_zones):
+        _check(lib.net_reserve(self._h, int(max_zones)))
 
     def net_rates(self, zones, T9, rho, R, stream=None):
         _check(lib.net_rates(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(R), _stream(stream)))

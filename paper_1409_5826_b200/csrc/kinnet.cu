@@ -22,6 +22,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -78,6 +79,7 @@ struct KParams {
     // zones
     const double* T9;
     const double* rho;
+    const int* order;  // [zones] launch order (zone of CTA b), NULL = identity
     void* Y;
     double* dt;
     int* n_steps;
@@ -110,7 +112,7 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int T = p.T, N = p.N, W = p.W, rs = p.rs, slots = rs * T, nbs = p.nbs;
-    const int z = blockIdx.x;
+    const int z = p.order ? p.order[blockIdx.x] : blockIdx.x;
 
     double* redmin = reinterpret_cast<double*>(smem_raw);            // [32] per-warp dt minima
     double* ybig = redmin + 32;                                      // [kMaxBig] start-of-step Y of big species
@@ -316,28 +318,49 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
 // hands out CTAs in index order, so in caller order the long zones that happen to start
 // late run alone on their SMs at the end.  Longest-processing-time-first on the T9 proxy
 // removes that tail (PAPER.md L200 leaves the load balance of unequal networks open).  A
-// counting sort on T9 quantised to 1/64 (one CTA, shared-memory histogram); the order
+// counting sort on T9 quantised to 1/64: a histogram kernel and a scatter kernel, both over
+// as many CTAs as the batch needs, on a 2 x 1024-int workspace zeroed by a memset node in
+// front of them (three stream operations, all legal under stream capture).  The order
 // inside a bucket is whatever the atomics give -- it only moves WHEN a zone runs, never
 // what it computes.
 constexpr int kOrderBuckets = 1024;
 constexpr int kOrderMinZones = 1024;
-__global__ void __launch_bounds__(1024) zone_order_kernel(const double* T9, int zones, int* order) {
-    __shared__ int hist[kOrderBuckets];
-    __shared__ int warp_tot[32];
-    const int tid = threadIdx.x;
-    hist[tid] = 0;
+constexpr int kOrderThreads = 256;
+constexpr int kOrderZonesPerCta = 4096;
+
+__device__ __forceinline__ int order_bucket(double t9) {
+    // descending temperature -> ascending bucket; NaN and <= 0 last
+    const double k = t9 * 64.0;
+    const int b = (k > 0.0) ? (k < 1023.0 ? static_cast<int>(k) : 1023) : 0;
+    return kOrderBuckets - 1 - b;
+}
+
+__global__ void __launch_bounds__(kOrderThreads) zone_hist_kernel(const double* T9, int zones, int* hist) {
+    __shared__ int h[kOrderBuckets];
+    for (int i = threadIdx.x; i < kOrderBuckets; i += kOrderThreads) h[i] = 0;
     __syncthreads();
-    auto bucket = [](double t9) {  // descending temperature -> ascending bucket; NaN and <= 0 last
-        const double k = t9 * 64.0;
-        int b = (k > 0.0) ? (k < 1023.0 ? static_cast<int>(k) : 1023) : 0;
-        return kOrderBuckets - 1 - b;
-    };
-    for (int z = tid; z < zones; z += 1024) atomicAdd(&hist[bucket(T9[z])], 1);
+    const int lo = blockIdx.x * kOrderZonesPerCta, hi = min(zones, lo + kOrderZonesPerCta);
+    for (int z = lo + threadIdx.x; z < hi; z += kOrderThreads) atomicAdd(&h[order_bucket(T9[z])], 1);
     __syncthreads();
-    // exclusive scan of the 1024 counts: warp scan + scan of the 32 warp totals
-    const int lane = tid & 31, warp = tid >> 5;
-    const int mine = hist[tid];
-    int incl = mine;
+    for (int i = threadIdx.x; i < kOrderBuckets; i += kOrderThreads)
+        if (h[i]) atomicAdd(&hist[i], h[i]);
+}
+
+// Every CTA scans the 1024 counts for itself (cheaper than a fourth launch), then places its
+// slice of the zones: position = start of the bucket + a ticket from the bucket's cursor.
+__global__ void __launch_bounds__(kOrderThreads) zone_scatter_kernel(const double* T9, int zones, const int* hist,
+                                                                    int* cursor, int* order) {
+    __shared__ int start[kOrderBuckets];
+    __shared__ int warp_tot[kOrderThreads / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int PER = kOrderBuckets / kOrderThreads;  // consecutive buckets per thread
+    int c[PER], run = 0;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+        c[q] = hist[tid * PER + q];
+        run += c[q];
+    }
+    int incl = run;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const int up = __shfl_up_sync(0xffffffffu, incl, o);
@@ -345,19 +368,19 @@ __global__ void __launch_bounds__(1024) zone_order_kernel(const double* T9, int 
     }
     if (lane == 31) warp_tot[warp] = incl;
     __syncthreads();
-    if (warp == 0) {
-        int w = warp_tot[lane];
+    int base = incl - run;
+    for (int w = 0; w < warp; ++w) base += warp_tot[w];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int up = __shfl_up_sync(0xffffffffu, w, o);
-            if (lane >= o) w += up;
-        }
-        warp_tot[lane] = w - warp_tot[lane];  // exclusive
+    for (int q = 0; q < PER; ++q) {
+        start[tid * PER + q] = base;
+        base += c[q];
     }
     __syncthreads();
-    hist[tid] = warp_tot[warp] + incl - mine;
-    __syncthreads();
-    for (int z = tid; z < zones; z += 1024) order[atomicAdd(&hist[bucket(T9[z])], 1)] = z;
+    const int lo = blockIdx.x * kOrderZonesPerCta, hi = min(zones, lo + kOrderZonesPerCta);
+    for (int z = lo + tid; z < hi; z += kOrderThreads) {
+        const int b = order_bucket(T9[z]);
+        order[start[b] + atomicAdd(&cursor[b], 1)] = z;
+    }
 }
 
 struct DeviceTables {
@@ -384,6 +407,15 @@ struct DeviceTables {
 
 }  // namespace
 
+// Launch-order workspaces ("lanes"): one per stream that has a sorted launch in flight on
+// this net_t.  [0, 1024) bucket counts, [1024, 2048) bucket cursors, then the order itself.
+constexpr int kLanes = 8;
+constexpr int kLaneHeader = 2 * kOrderBuckets;
+constexpr int kDefaultReserve = 65536;  // zones per lane allocated by net_create
+constexpr int kHostStreams = 3;         // internal streams of net_integrate_host_async
+constexpr int kHostMinChunk = 16384;    // zones; a staged chunk is max(this, zones / kHostMaxChunks)
+constexpr int kHostMaxChunks = 16;
+
 struct net {
     Schedule S;
     kinnet::PullSchedule PS;
@@ -395,10 +427,14 @@ struct net {
     int device = -1;
     int zones_per_sm = 0;
     DeviceTables D;
-    int* d_order = nullptr;  // launch order scratch of net_integrate, grown on demand
-    int order_cap = 0;
-    // scratch of net_integrate_host
-    cudaStream_t host_stream = nullptr;
+    // launch-order lanes (net_create / net_reserve allocate; net_integrate only picks one)
+    std::mutex mu;
+    int lane_cap = 0;
+    int* lane_buf[kLanes] = {};
+    cudaStream_t lane_stream[kLanes] = {};
+    bool lane_used[kLanes] = {};
+    // device scratch and streams of net_integrate_host_async
+    cudaStream_t host_stream[kHostStreams] = {};
     int scratch_zones = 0;
     double *sT9 = nullptr, *srho = nullptr, *sdt = nullptr;
     void* sY = nullptr;
@@ -463,15 +499,23 @@ size_t net_smem(const net* n) {
     return n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
 }
 
+constexpr size_t kMaxSmem = 227 * 1024;
+constexpr size_t kRatesSmem = 64 * sizeof(double);  // MODE kRates touches only the fixed header
+
+size_t generic_smem(const net* n) {
+    return n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
+}
+
 int prepare_kernels(net* n) {
-    const size_t smem = n->P.precision == 32 ? smem_bytes<float>(n->S) : smem_bytes<double>(n->S);
-    kernel_fn fns[4] = {pick_kernel<kAdaptive>(n), pick_kernel<kFixed>(n), pick_kernel<kRhs>(n),
-                        pick_kernel<kRates>(n)};
-    for (kernel_fn f : fns) {
-        const size_t need = (f == fns[3]) ? smem_bytes<double>(n->S) : smem;
-        CUDA_TRY(cudaFuncSetAttribute(reinterpret_cast<const void*>(f),
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      static_cast<int>(need)));
+    // the generic kernels are prepared only where they can be launched: a network on the pull
+    // path may have a flux array that does not fit (net_rates needs none of it)
+    const size_t smem = generic_smem(n);
+    if (smem <= kMaxSmem) {
+        kernel_fn fns[3] = {pick_kernel<kAdaptive>(n), pick_kernel<kFixed>(n), pick_kernel<kRhs>(n)};
+        for (kernel_fn f : fns)
+            CUDA_TRY(cudaFuncSetAttribute(reinterpret_cast<const void*>(f),
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          static_cast<int>(smem)));
     }
     int nb = 0;
     if (use_pull_kernel(n)) {
@@ -484,9 +528,65 @@ int prepare_kernels(net* n) {
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, pull_block(n), pull_smem(n)));
     } else {
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-            &nb, reinterpret_cast<const void*>(fns[0]), n->S.T, smem));
+            &nb, reinterpret_cast<const void*>(pick_kernel<kAdaptive>(n)), n->S.T, smem));
     }
     n->zones_per_sm = nb;
+    return NET_OK;
+}
+
+int alloc_lanes(net* n, int cap) {
+    for (int l = 0; l < kLanes; ++l) {
+        if (n->lane_buf[l]) cudaFree(n->lane_buf[l]);
+        n->lane_buf[l] = nullptr;
+    }
+    n->lane_cap = 0;
+    for (int l = 0; l < kLanes; ++l)
+        CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->lane_buf[l]),
+                            sizeof(int) * (static_cast<size_t>(kLaneHeader) + cap)));
+    n->lane_cap = cap;
+    return NET_OK;
+}
+
+// The lane of this stream, or of no stream yet; NULL when the batch is larger than the lanes
+// or every lane belongs to another stream (the launch then runs in caller order).
+int* pick_lane(net* n, cudaStream_t stream, int zones) {
+    if (zones > n->lane_cap) return nullptr;
+    std::lock_guard<std::mutex> lock(n->mu);
+    for (int l = 0; l < kLanes; ++l)
+        if (n->lane_used[l] && n->lane_stream[l] == stream) return n->lane_buf[l];
+    for (int l = 0; l < kLanes; ++l)
+        if (!n->lane_used[l]) {
+            n->lane_used[l] = true;
+            n->lane_stream[l] = stream;
+            return n->lane_buf[l];
+        }
+    return nullptr;
+}
+
+// Enqueue the counting sort of the zones by falling T9; returns the order (device) or NULL.
+int enqueue_order(net* n, int zones, const double* T9, cudaStream_t stream, const int** order) {
+    *order = nullptr;
+    if (zones < kOrderMinZones) return NET_OK;  // fewer zones than a couple of waves
+    int* lane = pick_lane(n, stream, zones);
+    if (!lane) return NET_OK;
+    const int ctas = (zones + kOrderZonesPerCta - 1) / kOrderZonesPerCta;
+    CUDA_TRY(cudaMemsetAsync(lane, 0, sizeof(int) * kLaneHeader, stream));
+    zone_hist_kernel<<<ctas, kOrderThreads, 0, stream>>>(T9, zones, lane);
+    zone_scatter_kernel<<<ctas, kOrderThreads, 0, stream>>>(T9, zones, lane, lane + kOrderBuckets,
+                                                           lane + kLaneHeader);
+    CUDA_TRY(cudaGetLastError());
+    *order = lane + kLaneHeader;
+    return NET_OK;
+}
+
+// Entry-point checks shared by everything that launches.
+int check_net(const net* n) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != n->device)
+        return fail(NET_EINVAL, "the net_t lives on device " + std::to_string(n->device) +
+                                    " but the calling thread's current device is " + std::to_string(dev));
     return NET_OK;
 }
 
@@ -591,12 +691,13 @@ void fill_params(const net* n, KParams& k) {
 
 template <int MODE>
 int launch(net* n, int zones, KParams& k, void* stream) {
-    if (!n) return fail(NET_EINVAL, "null net");
-    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    if (int rc = check_net(n)) return rc;
     if (zones < 0) return fail(NET_EINVAL, "zones < 0");
     if (zones == 0) return NET_OK;
     if (!k.T9 || !k.rho) return fail(NET_EINVAL, "null T9/rho");
-    const size_t smem = (MODE == kRates) ? smem_bytes<double>(n->S) : net_smem(n);
+    const size_t smem = (MODE == kRates) ? kRatesSmem : generic_smem(n);
+    if (smem > kMaxSmem)
+        return fail(NET_EINVAL, "the generic kernel's flux array does not fit one CTA's shared memory");
     kernel_fn f = pick_kernel<MODE>(n);
     f<<<zones, n->S.T, smem, static_cast<cudaStream_t>(stream)>>>(k);
     CUDA_TRY(cudaGetLastError());
@@ -663,7 +764,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
         n->PS.ok = false;  // only the two-species kernel is instantiated with N-slots
         n->PS.why = "reactions with two non-hub reactants need the two-species-per-thread kernel";
     }
-    if (net_smem(n) > 227 * 1024) {
+    if (net_smem(n) > kMaxSmem) {
         delete n;
         return fail(NET_EINVAL, "network too large for one CTA's shared memory");
     }
@@ -686,6 +787,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
             n->has_device = true;
             rc = prepare_kernels(n);
         }
+        if (rc == NET_OK) rc = alloc_lanes(n, kDefaultReserve);
         if (rc != NET_OK) {
             std::string keep = g_last_error;
             net_destroy(n);
@@ -695,6 +797,17 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
     }
     *out = n;
     return NET_OK;
+}
+
+// Device alias of a pinned (page-locked, mapped) host buffer, or NULL for anything else.
+void* mapped_alias(const void* host) {
+    if (!host) return nullptr;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
 }
 
 }  // namespace
@@ -710,6 +823,7 @@ int net_default_params(net_params_t* p) {
     p->max_steps = 10000000LL;
     p->precision = 64;
     p->kernel = 0;
+    p->host_chunk = 0;
     return NET_OK;
 }
 
@@ -737,18 +851,30 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.p_slot_rxn); cudaFree(n->D.p_f1); cudaFree(n->D.p_f2);
         cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent); cudaFree(n->D.bind);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
-        cudaFree(n->ssteps); cudaFree(n->sstatus); cudaFree(n->d_order);
-        if (n->host_stream) cudaStreamDestroy(n->host_stream);
+        cudaFree(n->ssteps); cudaFree(n->sstatus);
+        for (int l = 0; l < kLanes; ++l) cudaFree(n->lane_buf[l]);
+        for (cudaStream_t s : n->host_stream)
+            if (s) cudaStreamDestroy(s);
     }
     delete n;
 }
 
+int net_reserve(net_t* n, int max_zones) {
+    if (int rc = check_net(n)) return rc;
+    if (max_zones < 0) return fail(NET_EINVAL, "max_zones < 0");
+    if (max_zones <= n->lane_cap) return NET_OK;
+    CUDA_TRY(cudaDeviceSynchronize());  // nothing in flight may still read the old workspaces
+    std::lock_guard<std::mutex> lock(n->mu);
+    return alloc_lanes(n, max_zones);
+}
+
 int net_set_binding_energy(net_t* n, const double* B) {
-    if (!n || !B) return fail(NET_EINVAL, "null argument");
-    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+    if (int rc = check_net(n)) return rc;
+    if (!B) return fail(NET_EINVAL, "null argument");
     for (int i = 0; i < n->S.N; ++i)
         if (!std::isfinite(B[i])) return fail(NET_EINVAL, "non-finite binding energy");
     if (!n->D.bind) CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->D.bind), sizeof(double) * n->S.N));
+    CUDA_TRY(cudaDeviceSynchronize());  // a launch in flight may still read the old table
     CUDA_TRY(cudaMemcpy(n->D.bind, B, sizeof(double) * n->S.N, cudaMemcpyHostToDevice));
     return NET_OK;
 }
@@ -761,33 +887,24 @@ int net_integrate(net_t* n, int zones, const double* T9, const double* rho, void
 int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                          double t_hydro, double* dt, int* n_steps, int* status, double* energy,
                          void* stream) {
-    if (!n) return fail(NET_EINVAL, "null net");
+    if (int rc = check_net(n)) return rc;
     if (energy && !n->D.bind)
         return fail(NET_EINVAL, "energy asked for before net_set_binding_energy");
-    if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
+    if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+    if (zones == 0) return NET_OK;
+    if (!Y) return fail(NET_EINVAL, "null Y");
+    if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
     if (!std::isfinite(t_hydro)) return fail(NET_EINVAL, "t_hydro is not finite");
-    if (n->has_device && use_pull_kernel(n)) {
-        if (zones < 0) return fail(NET_EINVAL, "zones < 0");
-        if (zones == 0) return NET_OK;
-        if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
+    const int* order = nullptr;
+    if (int rc = enqueue_order(n, zones, T9, static_cast<cudaStream_t>(stream), &order)) return rc;
+    if (use_pull_kernel(n)) {
         KPull q;
         fill_pull(n, q);
         q.mode = kAdaptive;
         q.T9 = T9; q.rho = rho; q.Y = Y; q.dt = dt; q.n_steps = n_steps; q.status = status;
         q.t_hydro = t_hydro;
         q.bind = n->D.bind; q.energy = energy;
-        if (zones >= kOrderMinZones) {  // more zones than a couple of waves: hottest first
-            if (zones > n->order_cap) {
-                cudaFree(n->d_order);
-                n->d_order = nullptr;
-                n->order_cap = 0;
-                CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->d_order), sizeof(int) * zones));
-                n->order_cap = zones;
-            }
-            zone_order_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(stream)>>>(T9, zones, n->d_order);
-            CUDA_TRY(cudaGetLastError());
-            q.order = n->d_order;
-        }
+        q.order = order;
         return launch_pull(n, zones, q, stream);
     }
     KParams k;
@@ -795,15 +912,16 @@ int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rh
     k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
     k.t_hydro = t_hydro;
     k.bind = n->D.bind; k.energy = energy;
+    k.order = order;
     return launch<kAdaptive>(n, zones, k, stream);
 }
 
 int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                         double dt_fixed, long long n_steps, void* stream) {
-    if (!n) return fail(NET_EINVAL, "null net");
+    if (int rc = check_net(n)) return rc;
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
     if (n_steps < 0 || n_steps > 2000000000LL) return fail(NET_EINVAL, "n_steps out of range [0, 2e9]");
-    if (n->has_device && use_pull_kernel(n)) {
+    if (use_pull_kernel(n)) {
         if (zones < 0) return fail(NET_EINVAL, "zones < 0");
         if (zones == 0) return NET_OK;
         if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
@@ -822,7 +940,7 @@ int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho
 }
 
 int net_rates(net_t* n, int zones, const double* T9, const double* rho, double* R, void* stream) {
-    if (!n) return fail(NET_EINVAL, "null net");
+    if (int rc = check_net(n)) return rc;
     if (zones > 0 && !R) return fail(NET_EINVAL, "null R");
     KParams k;
     fill_params(n, k);
@@ -832,9 +950,9 @@ int net_rates(net_t* n, int zones, const double* T9, const double* rho, double* 
 
 int net_rhs(net_t* n, int zones, const double* T9, const double* rho, const void* Y, void* Fplus,
             void* Fminus, void* stream) {
-    if (!n) return fail(NET_EINVAL, "null net");
+    if (int rc = check_net(n)) return rc;
     if (zones > 0 && (!Y || !Fplus || !Fminus)) return fail(NET_EINVAL, "null Y/Fplus/Fminus");
-    if (n->has_device && use_pull_kernel(n)) {
+    if (use_pull_kernel(n)) {
         if (zones < 0) return fail(NET_EINVAL, "zones < 0");
         if (zones == 0) return NET_OK;
         if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
@@ -850,16 +968,38 @@ int net_rhs(net_t* n, int zones, const double* T9, const double* rho, const void
     return launch<kRhs>(n, zones, k, stream);
 }
 
-int net_integrate_host(net_t* n, int zones, const double* T9, const double* rho, void* Y,
-                       double t_hydro, double* dt, int* n_steps, int* status) {
-    if (!n) return fail(NET_EINVAL, "null net");
-    if (!n->has_device) return fail(NET_ECUDA, "net has no device copy (net_create_host)");
+// Host-buffer path (what crosses the link per network, and
+// what the CPU and the link do while the GPU integrates).
+//   * Pinned buffers: ZERO-COPY.  The zone kernel itself reads a zone's T9, rho, dt and
+//     abundances from the mapped host buffers when the zone starts (S6 in) and writes them back
+//     when it ends (S6 out): one launch over the whole batch in the global hottest-first order,
+//     every transfer overlapped with the integration of the other zones, no staging copy.
+//   * Anything else (pageable memory): staged through net-owned device scratch in chunks over
+//     three internal streams (upload of chunk c, kernels of c-1 and download of c-2 overlap;
+//     the launch order then applies within a chunk).
+int net_integrate_host_async(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                             double t_hydro, double* dt, int* n_steps, int* status) {
+    if (int rc = check_net(n)) return rc;
     if (zones < 0) return fail(NET_EINVAL, "zones < 0");
     if (zones == 0) return NET_OK;
     if (!T9 || !rho || !Y) return fail(NET_EINVAL, "null T9/rho/Y");
+    for (cudaStream_t& s : n->host_stream)
+        if (!s) CUDA_TRY(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    if (n->P.host_chunk >= 0) {  // < 0 forces the staged path
+        void* aT9 = mapped_alias(T9);
+        void* arho = mapped_alias(rho);
+        void* aY = mapped_alias(Y);
+        void* adt = mapped_alias(dt);
+        void* asteps = mapped_alias(n_steps);
+        void* astatus = mapped_alias(status);
+        if (aT9 && arho && aY && (adt || !dt) && (asteps || !n_steps) && (astatus || !status))
+            return net_integrate(n, zones, static_cast<const double*>(aT9), static_cast<const double*>(arho),
+                                 aY, t_hydro, static_cast<double*>(adt), static_cast<int*>(asteps),
+                                 static_cast<int*>(astatus), n->host_stream[0]);
+    }
     const size_t ysz = (n->P.precision == 32 ? sizeof(float) : sizeof(double)) * (size_t)n->S.N;
-    if (!n->host_stream) CUDA_TRY(cudaStreamCreateWithFlags(&n->host_stream, cudaStreamNonBlocking));
     if (zones > n->scratch_zones) {
+        for (cudaStream_t s : n->host_stream) CUDA_TRY(cudaStreamSynchronize(s));
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
         cudaFree(n->ssteps); cudaFree(n->sstatus);
         n->sT9 = n->srho = n->sdt = nullptr; n->sY = nullptr; n->ssteps = n->sstatus = nullptr;
@@ -872,23 +1012,44 @@ int net_integrate_host(net_t* n, int zones, const double* T9, const double* rho,
         CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->sstatus), sizeof(int) * zones));
         n->scratch_zones = zones;
     }
-    cudaStream_t s = n->host_stream;
-    CUDA_TRY(cudaMemcpyAsync(n->sT9, T9, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(cudaMemcpyAsync(n->srho, rho, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(cudaMemcpyAsync(n->sY, Y, ysz * zones, cudaMemcpyHostToDevice, s));
-    if (dt) CUDA_TRY(cudaMemcpyAsync(n->sdt, dt, sizeof(double) * zones, cudaMemcpyHostToDevice, s));
-    else CUDA_TRY(cudaMemsetAsync(n->sdt, 0, sizeof(double) * zones, s));
-    int rc = net_integrate(n, zones, n->sT9, n->srho, n->sY, t_hydro, n->sdt, n->ssteps,
-                           n->sstatus, s);
-    if (rc != NET_OK) return rc;
-    CUDA_TRY(cudaMemcpyAsync(Y, n->sY, ysz * zones, cudaMemcpyDeviceToHost, s));
-    if (dt) CUDA_TRY(cudaMemcpyAsync(dt, n->sdt, sizeof(double) * zones, cudaMemcpyDeviceToHost, s));
-    if (n_steps)
-        CUDA_TRY(cudaMemcpyAsync(n_steps, n->ssteps, sizeof(int) * zones, cudaMemcpyDeviceToHost, s));
-    if (status)
-        CUDA_TRY(cudaMemcpyAsync(status, n->sstatus, sizeof(int) * zones, cudaMemcpyDeviceToHost, s));
-    CUDA_TRY(cudaStreamSynchronize(s));
+    const int chunk = n->P.host_chunk != 0
+                          ? std::abs(n->P.host_chunk)
+                          : std::max(kHostMinChunk, (zones + kHostMaxChunks - 1) / kHostMaxChunks);
+    int c = 0;
+    for (int lo = 0; lo < zones; lo += chunk, ++c) {
+        const int m = std::min(chunk, zones - lo);
+        cudaStream_t s = n->host_stream[c % kHostStreams];
+        char* Yh = static_cast<char*>(Y) + ysz * lo;
+        char* Yd = static_cast<char*>(n->sY) + ysz * lo;
+        CUDA_TRY(cudaMemcpyAsync(n->sT9 + lo, T9 + lo, sizeof(double) * m, cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemcpyAsync(n->srho + lo, rho + lo, sizeof(double) * m, cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemcpyAsync(Yd, Yh, ysz * m, cudaMemcpyHostToDevice, s));
+        if (dt) CUDA_TRY(cudaMemcpyAsync(n->sdt + lo, dt + lo, sizeof(double) * m, cudaMemcpyHostToDevice, s));
+        else CUDA_TRY(cudaMemsetAsync(n->sdt + lo, 0, sizeof(double) * m, s));
+        if (int rc = net_integrate(n, m, n->sT9 + lo, n->srho + lo, Yd, t_hydro, n->sdt + lo,
+                                   n->ssteps + lo, n->sstatus + lo, s))
+            return rc;
+        CUDA_TRY(cudaMemcpyAsync(Yh, Yd, ysz * m, cudaMemcpyDeviceToHost, s));
+        if (dt) CUDA_TRY(cudaMemcpyAsync(dt + lo, n->sdt + lo, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
+        if (n_steps)
+            CUDA_TRY(cudaMemcpyAsync(n_steps + lo, n->ssteps + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
+        if (status)
+            CUDA_TRY(cudaMemcpyAsync(status + lo, n->sstatus + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
+    }
     return NET_OK;
+}
+
+int net_wait(net_t* n) {
+    if (int rc = check_net(n)) return rc;
+    for (cudaStream_t s : n->host_stream)
+        if (s) CUDA_TRY(cudaStreamSynchronize(s));
+    return NET_OK;
+}
+
+int net_integrate_host(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                       double t_hydro, double* dt, int* n_steps, int* status) {
+    if (int rc = net_integrate_host_async(n, zones, T9, rho, Y, t_hydro, dt, n_steps, status)) return rc;
+    return net_wait(n);
 }
 
 int net_schedule_info(const net_t* n, net_schedule_info_t* info) {

@@ -412,13 +412,14 @@ def test_bitwise_run_to_run_determinism(hub150):
     assert (a["n_steps"] == b["n_steps"]).all() and (a["dt"] == b["dt"]).all()
 
 
-def test_launch_order_changes_nothing_but_the_schedule(hub150):
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_launch_order_changes_nothing_but_the_schedule(hub150, kernel):
     """From 1024 zones up net_integrate launches the hottest zones first (a counting sort
-    with atomics).  The order decides WHEN a zone runs, never what it computes: 2048 zones in
-    one call (sorted) are bit for bit the same 2048 zones in four calls of 512 (caller order),
-    and two sorted runs agree bit for bit."""
+    with atomics), on the pull kernels and on the generic one.  The order decides WHEN a zone
+    runs, never what it computes: 2048 zones in one call (sorted) are bit for bit the same
+    2048 zones in four calls of 512 (caller order), and two sorted runs agree bit for bit."""
     c = build_config(4, zones=2048)
-    kn = K.Net(hub150)
+    kn = K.Net(hub150, K.NetParams(kernel=kernel))
     whole = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     again = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     parts = [gpu_integrate(kn, c["T9"][lo:lo + 512], c["rho"][lo:lo + 512], c["Y0"][lo:lo + 512], c["t_hydro"])
@@ -429,21 +430,121 @@ def test_launch_order_changes_nothing_but_the_schedule(hub150):
     assert whole["n_steps"].max() > 20 * whole["n_steps"].min()  # the spread the order is there for
 
 
-def test_host_entry_point_matches_device_path(hub150):
-    c = build_config(3)
+def _state(c, z):
+    return (dev(c["T9"]), dev(c["rho"]), dev(c["Y0"]), torch.zeros(z, dtype=torch.float64, device=DEV),
+            torch.zeros(z, dtype=torch.int32, device=DEV), torch.zeros(z, dtype=torch.int32, device=DEV))
+
+
+def test_net_integrate_under_stream_capture(hub150):
+    """include/kinnet.h: net_integrate allocates nothing and never synchronises, so two
+    consecutive hydro steps (dt carried) can be captured into one CUDA graph; the replay is bit
+    for bit the eager result.  2048 zones: the sorted launch (memset + two order kernels + the
+    zone kernel per call)."""
+    z = 2048
+    c = build_config(4, zones=z)
     kn = K.Net(hub150)
+    T9, rho, Y, dt, steps, status = _state(c, z)
+    for _ in range(2):  # eager reference
+        kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status)
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (Y, dt, steps, status)]
+    Y0 = dev(c["Y0"])
+    g = torch.cuda.CUDAGraph()
+    Y.copy_(Y0)
+    dt.zero_()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        for _ in range(2):
+            kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status)  # stream = the capturing one
+    for _ in range(2):  # replay twice from the same start
+        Y.copy_(Y0)
+        dt.zero_()
+        steps.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        for got, ref in zip((Y, dt, steps, status), want):
+            assert torch.equal(got, ref)
+    assert int(steps.sum()) > 0
+
+
+def test_one_net_two_streams(hub150):
+    """One net_t driven from two streams at once on disjoint zone ranges (each range large
+    enough for the sorted launch, so each stream holds its own launch-order lane) returns what
+    a single-stream call over all zones returns, bit for bit."""
+    z = 4096
+    c = build_config(4, zones=z)
+    kn = K.Net(hub150)
+    T9, rho, Y, dt, steps, status = _state(c, z)
+    kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status)
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (Y, dt, steps, status)]
+    T9, rho, Y, dt, steps, status = _state(c, z)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    h = z // 2
+    for rep in range(3):  # interleaved submissions, both streams busy together
+        for s, lo in ((s1, 0), (s2, h)):
+            sl = slice(lo, lo + h)
+            if rep == 0:
+                kn.net_integrate(h, T9[sl], rho[sl], Y[sl], c["t_hydro"], dt[sl], steps[sl], status[sl], s)
+    torch.cuda.synchronize()
+    for got, ref in zip((Y, dt, steps, status), want):
+        assert torch.equal(got, ref)
+
+
+def test_net_reserve_and_oversized_batches(g16):
+    """More zones than the launch-order lanes hold (65536 after net_create): the call runs in
+    caller order and returns the same bits as after net_reserve (sorted)."""
+    z = 70_000
+    rng = np.random.default_rng(70)
+    T9, rho = rng.uniform(1, 10, z), 10 ** rng.uniform(7, 9.5, z)
+    Y0 = np.repeat(build_config(1)["Y0"], z, axis=0)
+    kn = K.Net(g16)
+    a = gpu_integrate(kn, T9, rho, Y0, 1e-9)
+    kn.net_reserve(z)
+    b = gpu_integrate(kn, T9, rho, Y0, 1e-9)
+    for key in ("Y", "dt", "n_steps", "status"):
+        assert np.array_equal(a[key], b[key]), key
+    assert (a["status"] == 0).all() and a["n_steps"].min() >= 1
+
+
+@pytest.mark.parametrize("zones,host_chunk", [(128, 0), (5000, 0), (5000, -2048), (3000, -1024)])
+def test_host_entry_points_match_device_path(hub150, zones, host_chunk):
+    """net_integrate_host (and the async pair) against net_integrate on the same zones, bit for
+    bit.  host_chunk = 0 with pinned buffers is the zero-copy path (the kernel reads and writes
+    the host buffers itself); host_chunk < 0 forces the staged path: 5000 zones travel as chunks
+    of 2048 + 2048 + 904 through the three internal streams, each with its own launch order."""
+    c = build_config(4, zones=zones)
+    kn = K.Net(hub150, K.NetParams(host_chunk=host_chunk))
     a = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     z = c["zones"]
-    Y = torch.from_numpy(c["Y0"].copy()).pin_memory()
-    T9 = torch.from_numpy(c["T9"].copy()).pin_memory()
-    rho = torch.from_numpy(c["rho"].copy()).pin_memory()
-    dt = torch.zeros(z, dtype=torch.float64).pin_memory()
-    steps = torch.zeros(z, dtype=torch.int32).pin_memory()
-    status = torch.zeros(z, dtype=torch.int32).pin_memory()
+
+    def pinned():
+        return (torch.from_numpy(c["T9"].copy()).pin_memory(), torch.from_numpy(c["rho"].copy()).pin_memory(),
+                torch.from_numpy(c["Y0"].copy()).pin_memory(), torch.zeros(z, dtype=torch.float64).pin_memory(),
+                torch.zeros(z, dtype=torch.int32).pin_memory(), torch.full((z,), -1, dtype=torch.int32).pin_memory())
+
+    T9, rho, Y, dt, steps, status = pinned()
     kn.net_integrate_host(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"], dt.numpy(),
                           steps.numpy(), status.numpy())
     assert (Y.numpy() == a["Y"]).all() and (steps.numpy() == a["n_steps"]).all()
-    assert (dt.numpy() == a["dt"]).all()
+    assert (dt.numpy() == a["dt"]).all() and (status.numpy() == 0).all()
+    # asynchronous: the call returns, the host does something else, net_wait brings the results
+    T9, rho, Y, dt, steps, status = pinned()
+    kn.net_integrate_host_async(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"], dt.numpy(),
+                                steps.numpy(), status.numpy())
+    busy = float(np.linalg.norm(np.random.default_rng(0).standard_normal((300, 300)) @ np.eye(300)))
+    kn.net_wait()
+    assert busy > 0 and (Y.numpy() == a["Y"]).all() and (steps.numpy() == a["n_steps"]).all()
+    assert (dt.numpy() == a["dt"]).all() and (status.numpy() == 0).all()
+    # optional outputs may be NULL
+    T9, rho, Y, dt, steps, status = pinned()
+    kn.net_integrate_host(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"])
+    assert (Y.numpy() == a["Y"]).all()
+    # pageable memory always takes the staged path
+    Yp, dtp = c["Y0"].copy(), np.zeros(z)
+    kn.net_integrate_host(z, c["T9"].copy(), c["rho"].copy(), Yp, c["t_hydro"], dtp)
+    assert (Yp == a["Y"]).all() and (dtp == a["dt"]).all()
 
 
 def test_fp32_variant_report(hub150, capsys):
