@@ -25,6 +25,7 @@ class _Params(C.Structure):
         ("y_floor", C.c_double),
         ("growth", C.c_double),
         ("max_steps", C.c_longlong),
+        ("method", C.c_int),
     ]
 
 
@@ -35,6 +36,7 @@ class OracleParams:
     y_floor: float = 1e-10
     growth: float = 2.0
     max_steps: int = 10_000_000
+    method: int = 0  # 0 = asymptotic (the paper's method), 1 = QSS variant
 
 
 _lib = None
@@ -90,7 +92,7 @@ class Oracle:
             np.ascontiguousarray(net.coef, np.float64).reshape(-1),
         ]
         p = params or OracleParams()
-        cp = _Params(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps)
+        cp = _Params(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.method)
         A, nr, re, npd, pr, co = self._keep
         self._h = lib.oracle_create(self.N, _ip(A), self.M, _ip(nr), _ip(re), _ip(npd), _ip(pr),
                                     _dp(co), C.byref(cp))

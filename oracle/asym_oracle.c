@@ -18,6 +18,13 @@
  *   O7 update       k dt >= kappa -> Eq. (3), else forward Euler; Jacobi
  *                                                   P:L61-69 Eq. (3); S:Q4-Q6,Q8
  *   O8/O9 advance, outputs
+ *   method = 1      the QSS variant of O7 named as future work in P:L217-219.  The paper
+ *                   gives no formula (its ref. [5] is not in the container): DESIGN.md
+ *                   reading Q20 takes the predictor of the published alpha-QSS scheme,
+ *                   y' = y + dt (F+ - k y)/(1 + alpha k dt) with the Pade alpha, for every
+ *                   species, behind the same fluxes, sums and dt controller.  Pinned by
+ *                   hand-worked per-step factors, the exact e^{-k dt} it approximates, the
+ *                   two-species fixed point, the Euler limit and RK4 on a tiny network.
  *
  * Precision: double throughout.  precision == 32 is the paper's single-
  * precision study (S:Q13): Y, f, F+, F-, k and the update in float;
@@ -60,6 +67,8 @@ typedef struct {
     double y_floor;      /* abundance floor inside the dt controller, S:Q7       */
     double growth;       /* dt growth cap per step, S:Q7                         */
     long long max_steps; /* per call; status bit 1 when hit                      */
+    int method;          /* 0 = asymptotic / forward Euler (the paper's method);
+                            1 = explicit quasi-steady-state variant, P:L217-219     */
 } oracle_params;
 
 typedef struct {
@@ -86,6 +95,7 @@ void oracle_default_params(oracle_params *p) {
     p->y_floor = 1e-10;
     p->growth = 2.0;
     p->max_steps = 10000000LL;
+    p->method = 0;
 }
 
 static double ln_factorial(int m) {

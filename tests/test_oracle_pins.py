@@ -572,3 +572,95 @@ def test_arbiter_controller_contract_and_agreement_with_fp64(g16, hub150):
     b = oh.integrate(4.0, 1e8, Y0, 1e-8, precision=80)
     m = a["Y"] * hub150.A > 1e-12
     assert a["n_steps"][0] == b["n_steps"][0] and np.abs(a["Y"][m] / b["Y"][m] - 1).max() < 1e-9
+
+
+# ------------------------------------------------ QSS variant (reading Q20)
+QSS = dict(method=1)
+
+
+@pytest.mark.parametrize("a,num,den", [(1.0, 252, 685), (2.0, 21, 155)])
+def test_qss_single_decay_hand_worked_factor(a, num, den):
+    """A -> B, F+_A = 0: per step Y_A *= (1 + (alpha - 1) a)/(1 + alpha a), a = k dt.
+    By hand: alpha(1) = (1+11+60+180)/(1+12+60+360) = 252/433 -> factor (252/433)/(685/433)
+    = 252/685; alpha(2) = (8+44+120+180)/(8+48+120+360) = 352/536 = 44/67 -> factor
+    (1 - 46/67)/(1 + 88/67) = 21/155.  B receives what A loses (F+_B = F-_A, k_B = 0)."""
+    for precision in (64, 80):
+        o = Oracle(decay_net(1.0), OracleParams(**QSS))
+        n, Y0 = 10, 0.75
+        out = o.integrate_fixed(1.0, 1.0, [Y0, 0.0], a, n, precision=precision)
+        assert out["Y"][0, 0] == pytest.approx(Y0 * (num / den) ** n, rel=1e-13)
+        # B: k_B = 0 -> plain Euler on F+_B = k Y_A(old): Y_B = a Y0 sum_j f^j
+        f = num / den
+        assert out["Y"][0, 1] == pytest.approx(a * Y0 * (1 - f**n) / (1 - f), rel=1e-13)
+
+
+@pytest.mark.parametrize("a,tol", [(1e-3, 1e-12), (0.1, 2e-12), (0.5, 1e-7), (1.0, 1.1e-5), (2.0, 1.2e-3)])
+def test_qss_tracks_the_exact_exponential(a, tol):
+    """With the exact weight the quasi-steady-state step reproduces Y0 e^{-k dt} for constant k
+    and F+ = 0; the Pade alpha is within 4e-6 of it at k dt = 1 and 1.5e-4 at k dt = 2
+    (absolute, per step).  Forward Euler at k dt = 0.5 is off by 0.1."""
+    o = Oracle(decay_net(1.0), OracleParams(**QSS))
+    Y = o.integrate_fixed(1.0, 1.0, [1.0, 0.0], a, 1)["Y"][0, 0]
+    assert abs(Y - np.exp(-a)) < tol * max(1.0, 1.0) and Y != 1 - a
+
+
+def test_qss_euler_limit_and_stiff_limit():
+    """alpha -> 1/2 as k dt -> 0: the step is y (1 - a/2)/(1 + a/2) = y (1 - a + a^2/2 - ...),
+    forward Euler to first order: after n = 100 steps at a = 1e-4 the ratio to the Euler closed
+    form (1 - a)^n is 1 + n a^2/2 = 1 + 5e-7.  alpha -> 1 as k dt -> infinity: with a source,
+    y' -> y + (F+ - k y)/k = F+/k, the steady state, as Eq. (3) does."""
+    o = Oracle(decay_net(1.0), OracleParams(**QSS))
+    a, n = 1e-4, 100
+    Y = o.integrate_fixed(1.0, 1.0, [1.0, 0.0], a, n)["Y"][0, 0]
+    assert Y / (1 - a) ** n - 1 == pytest.approx(n * a * a / 2, rel=2e-2)
+    kf, kr = 3.0e9, 1.0e9
+    o2 = Oracle(make_toy([1, 1], [((0,), (1,)), ((1,), (0,))], [kf, kr]), OracleParams(**QSS))
+    Y = o2.integrate_fixed(1.0, 1.0, [0.9, 0.1], 1.0, 1)["Y"][0]
+    assert Y[0] == pytest.approx(kr * 0.1 / kf, rel=1e-7)  # F+_A / k_A from the old Y_B
+
+
+@pytest.mark.parametrize("dt", [1e-3, 0.5, 10.0, 1e3])
+def test_qss_two_species_equilibrium_ratio(dt):
+    """F+ = k y at Y_A/Y_B = k_r/k_f whatever alpha is: an exact fixed point at any dt (started
+    there, the state does not move).  The error mode contracts for moderate dt; at k dt ~ 1e3
+    the Jacobi predictor hands each species the other's steady state and the mode decays only
+    like 1 - O(1/(k dt)^2) per step, so there only boundedness and positivity are asserted."""
+    kf, kr = 3.0, 1.0
+    o = Oracle(make_toy([1, 1], [((0,), (1,)), ((1,), (0,))], [kf, kr]), OracleParams(**QSS))
+    Y = o.integrate_fixed(1.0, 1.0, [[0.25, 0.75]], dt, 1000)["Y"]
+    assert Y[0, 0] == pytest.approx(0.25, rel=1e-13) and Y[0, 1] == pytest.approx(0.75, rel=1e-13)
+    Y = np.array([[0.9, 0.1]])
+    for _ in range(60):
+        Y = o.integrate_fixed(1.0, 1.0, Y, dt, 1000)["Y"]
+    if dt <= 10.0:
+        assert Y[0, 0] / Y[0, 1] == pytest.approx(kr / kf, rel=1e-12)
+    else:
+        assert (Y > 0).all() and Y.sum() < 10.0
+
+
+def test_qss_brute_force_tiny_network_and_positivity(hub150):
+    """The variant as an approximation of Eq. (1): RK4 on the tiny network, error O(eps_Y) and
+    shrinking with it; on hub150 it stays non-negative and finite, and it is a different
+    integrator from the asymptotic one (results differ) behind the same controller."""
+    net = tiny_net()
+    Y0 = np.array([0.5, 0.3, 0.1, 0.0, 0.0, 0.0])
+    Y0 /= (Y0 * net.A).sum()
+    t_end = 0.8
+    R = Oracle(net).rates(1.0, 1.0)
+    ref = rk4(net, R, Y0.copy(), t_end, 8_000)
+    errs = []
+    for eps in (0.04, 0.01, 0.0025):
+        out = Oracle(net, OracleParams(eps_y=eps, **QSS)).integrate(1.0, 1.0, Y0, t_end)
+        X, Xr = out["Y"][0] * net.A, ref * net.A
+        m = Xr > 1e-6
+        errs.append(np.abs(X[m] / Xr[m] - 1).max())
+    assert errs[0] < 4e-2 and errs[1] < 0.45 * errs[0] and errs[2] < 0.45 * errs[1]
+    rng = np.random.default_rng(6)
+    z = 6
+    T9, rho = rng.uniform(1, 10, z), 10 ** rng.uniform(7, 9.5, z)
+    Y0 = np.zeros((z, 150))
+    Y0[:, 3], Y0[:, 15] = 0.5 / 12, 0.5 / 16
+    q = Oracle(hub150, OracleParams(**QSS)).integrate(T9, rho, Y0, 1e-7)
+    a = Oracle(hub150).integrate(T9, rho, Y0, 1e-7)
+    assert (q["Y"] >= 0).all() and np.isfinite(q["Y"]).all() and (q["status"] == 0).all()
+    assert q["n_asym"].sum() > 0 and not np.allclose(q["Y"], a["Y"], rtol=1e-6, atol=1e-30)
