@@ -62,7 +62,7 @@ def pull_design_smem_bytes(kn, info, ybytes):
 
 
 # FP64 / shared-memory peaks: measured on this pool's B200 with
-# `python -m paper_1409_5826_b200.peaks` (profiles/r01_peaks.md); fallback =
+# `python bench_peaks.py` (profiles/peaks.json); fallback =
 # unit counts x clocks.max.sm from the guides (64 FP64 lanes and 128 B of shared
 # memory per clock per SM, 148 SMs, 1965 MHz).
 NOMINAL_FP64_TINSTR = 148 * 64 * 1.965e9 / 1e12
@@ -152,13 +152,13 @@ def cpu_sample_size(o, T9, rho, Y0, cores, target_s):
     return int(max(probe, min(len(T9), rate * target_s)))
 
 
-def cpu_baseline(net, T9, rho, Y0, target_s=15.0):
+def cpu_baseline(net, T9, rho, Y0, target_s=15.0, method=0):
     """The oracle as it stands on the host cores, on a bounded prefix sample
     (about target_s seconds of CPU work)."""
-    from oracle import Oracle, max_threads
+    from oracle import Oracle, OracleParams, max_threads
 
     cores = max_threads()
-    o = Oracle(net)
+    o = Oracle(net, OracleParams(method=method))
     n = cpu_sample_size(o, T9, rho, Y0, cores, target_s)
     t0 = time.perf_counter()
     out = o.integrate(T9[:n], rho[:n], Y0[:n], T_HYDRO, n_threads=cores)
@@ -170,11 +170,11 @@ def cpu_baseline(net, T9, rho, Y0, target_s=15.0):
             "zone_substeps_per_s": steps / best}
 
 
-def cpu_baseline_1core(net, T9, rho, Y0, zones=64):
+def cpu_baseline_1core(net, T9, rho, Y0, zones=64, method=0):
     """BASELINE.md CPU-baseline plan (i): the oracle on ONE host core, first `zones` zones."""
-    from oracle import Oracle
+    from oracle import Oracle, OracleParams
 
-    o = Oracle(net)
+    o = Oracle(net, OracleParams(method=method))
     t0 = time.perf_counter()
     out = o.integrate(T9[:zones], rho[:zones], Y0[:zones], T_HYDRO, n_threads=1)
     el = time.perf_counter() - t0
@@ -236,7 +236,8 @@ def run_ours(args):
 
     net, T9h, rhoh, Y0h = workload(rank, world, args.zones, args.network)
     z, N = Y0h.shape
-    kn = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel))
+    method = {"asymptotic": 0, "qss": 1}[args.method]
+    kn = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel, method=method))
     info = kn.schedule_info()
     ynp = np.float64 if args.precision == 64 else np.float32
     ybytes = 8 if args.precision == 64 else 4
@@ -313,7 +314,7 @@ def run_ours(args):
         return total
 
     e2e_s = time_host_path(kn)
-    kn_staged = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel, host_chunk=-z))
+    kn_staged = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel, host_chunk=-z, method=method))
     staged_s = time_host_path(kn_staged)
     h2d = z * (N * ybytes + 8 + 8 + 8)
     d2h = z * (N * ybytes + 8 + 4 + 4)
@@ -321,7 +322,7 @@ def run_ours(args):
 
     # ---- secondary points: config 3 and config 5 ---------------
     extra = {}
-    if world == 1 and not args.no_extra and args.network == "hub150" and args.precision == 64:
+    if world == 1 and not args.no_extra and args.network == "hub150" and args.precision == 64 and method == 0:
         from gen import build_config
 
         def dev_t(a, dtype=torch.float64):
@@ -391,7 +392,8 @@ def run_ours(args):
     per_launch_substeps = substeps  # rank 0's launch
     k_ms = float(np.mean(kernel_ms))
     fp64_ach = flops * per_launch_substeps / (k_ms * 1e-3) / 1e12
-    default_run = (z == ZONES_PER_GPU and args.precision == 64 and args.kernel == 0 and args.network == "hub150")
+    default_run = (z == ZONES_PER_GPU and args.precision == 64 and args.kernel == 0 and args.network == "hub150"
+                   and method == 0)
     traffic = DRAM_BYTES_PER_LAUNCH if default_run else None
     dtype = "f64" if args.precision == 64 else "f32"
     kname = ({0: "zone_kernel", 1: "zone_kernel_pull", 2: "zone_kernel_pull2"}[info["kernel"]]
@@ -405,7 +407,8 @@ def run_ours(args):
         "config": {
             "workload": f"configs[3]: synthetic 150sp/{net.n_reactions}rx hub network ({args.network}, seed 1409), "
                         "16384 zones per GPU, T9~U[1,10], log10 rho~U[7,9.5] (seed 4), lognormal-perturbed "
-                        "C/O start, one hydro step of 1e-6 s, adaptive dt",
+                        "C/O start, one hydro step of 1e-6 s, adaptive dt"
+                        + ("" if method == 0 else "; QSS variant of the update (net_params_t.method = 1)"),
             "zones_per_gpu": z, "sub_steps_per_step": substeps_all,
             "mean_sub_steps_per_zone": substeps_all / (z * world),
             "sub_steps_per_zone": {"min": int(steps_host.min()), "median": float(np.median(steps_host)),
@@ -455,8 +458,8 @@ def run_ours(args):
     if extra:
         out["extra"] = extra
     if world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(net, T9h, rhoh, Y0h)
-        out["cpu_baseline_1core"] = cpu_baseline_1core(net, T9h, rhoh, Y0h)
+        out["cpu_baseline"] = cpu_baseline(net, T9h, rhoh, Y0h, method=method)
+        out["cpu_baseline_1core"] = cpu_baseline_1core(net, T9h, rhoh, Y0h, method=method)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -532,6 +535,9 @@ def main():
     ap.add_argument("--network", default="hub150", choices=["hub150", "hub150hh"],
                     help="hub150 = the metric's network; hub150hh = the same plus 16 heavy + heavy reactions "
                          "and their inverses (the fast path must survive them, DESIGN.md 4.8)")
+    ap.add_argument("--method", default="asymptotic", choices=["asymptotic", "qss"],
+                    help="qss = the explicit quasi-steady-state variant of the update (PAPER.md L217-219, "
+                         "DESIGN.md reading Q20); the metric is quoted on the paper's asymptotic method")
     ap.add_argument("--sweep", choices=["zones", "size"],
                     help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
                          "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")

@@ -1,8 +1,8 @@
-// peaks.cu -- micro-benchmarks for the two roofline denominators of the zone
+// bench_peaks.cu -- micro-benchmarks for the two roofline denominators of the zone
 // kernel that MEASURED_PEAKS.json does not hold: plain (non-tensor) FP64 issue
 // rate and shared-memory bandwidth, chip-wide on the device it runs on.
-// Prints one JSON line.  Built by paper_1409_5826_b200/build.py into
-// kinnet_peaks; run with `python -m paper_1409_5826_b200.peaks`.
+// Prints one JSON line.  Built and run by bench_peaks.py (beside bench.py, whose roofline
+// denominators it measures); not part of the library.
 #include <cuda_runtime.h>
 
 #include <cstdio>

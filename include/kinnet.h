@@ -84,6 +84,11 @@ typedef struct {
     int host_chunk;      /* net_integrate_host*: zones per chunk of the staged path; 0 = default
                             max(16384, zones/16); < 0 = always stage through device scratch, in
                             chunks of -host_chunk zones, even when the buffers are pinned       */
+    int method;          /* 0 = the paper's method: Eq. (3) where k dt >= kappa, forward Euler below;
+                            1 = explicit quasi-steady-state variant (named as the
+                            next step; formula = DESIGN.md reading Q20): every species takes
+                            y' = y + dt (F+ - k y) / (1 + alpha(k dt) k dt) with the Pade alpha,
+                            behind the same rates, fluxes, sums and dt controller                */
 } net_params_t;
 
 /* Fill *p with the defaults listed above. */

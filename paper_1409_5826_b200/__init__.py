@@ -32,7 +32,7 @@ class net_params_t(C.Structure):
     _fields_ = [
         ("kappa", C.c_double), ("eps_y", C.c_double), ("y_floor", C.c_double),
         ("growth", C.c_double), ("max_steps", C.c_longlong), ("precision", C.c_int),
-        ("kernel", C.c_int), ("host_chunk", C.c_int),
+        ("kernel", C.c_int), ("host_chunk", C.c_int), ("method", C.c_int),
     ]
 
 
@@ -102,16 +102,17 @@ class NetParams:
     precision: int = 64
     kernel: int = 0  # 0 = automatic, 1 = generic kernel only, 2 = one-species pull kernel
     host_chunk: int = 0  # staged host path: zones per chunk; < 0 = never zero-copy
+    method: int = 0  # 0 = asymptotic (the paper's method), 1 = QSS variant
 
     def to_c(self) -> net_params_t:
         return net_params_t(self.kappa, self.eps_y, self.y_floor, self.growth, self.max_steps,
-                            self.precision, self.kernel, self.host_chunk)
+                            self.precision, self.kernel, self.host_chunk, self.method)
 
 
 def net_default_params() -> NetParams:
     p = net_params_t()
     _check(lib.net_default_params(C.byref(p)))
-    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel, p.host_chunk)
+    return NetParams(p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel, p.host_chunk, p.method)
 
 
 def _ptr(t):

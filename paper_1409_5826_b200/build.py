@@ -17,8 +17,7 @@ LIB = os.path.join(HERE, "libkinnet.so")
 HEADERS = [os.path.join(CSRC, h) for h in ("schedule.h", "zone_pull.cuh", "zone_pull2.cuh", "device_util.cuh")] + [
     os.path.join(HERE, "..", "include", "kinnet.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-NVCC_FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2,-Wall",
-              *os.environ.get("KINNET_DEFS", "").split()]  # e.g. KINNET_DEFS="-DKINNET_MINB160=4" for A/B builds
+NVCC_FLAGS = [*ARCH, "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-O2,-Wall"]
 
 # (object name, source, extra defines)
 UNITS = [
@@ -43,20 +42,6 @@ def nvcc() -> str:
     if not os.path.exists(exe):
         raise RuntimeError("nvcc not found: the CUDA extension cannot be built")
     return exe
-
-
-PEAKS_SRC = os.path.join(CSRC, "peaks.cu")
-PEAKS_BIN = os.path.join(HERE, "kinnet_peaks")
-
-
-def build_peaks(force: bool = False) -> str:
-    """Micro-benchmark binary for the FP64 / shared-memory roofline denominators."""
-    if force or not os.path.exists(PEAKS_BIN) or os.path.getmtime(PEAKS_BIN) < os.path.getmtime(PEAKS_SRC):
-        tmp = PEAKS_BIN + f".tmp{os.getpid()}"
-        subprocess.check_call([nvcc(), *ARCH, "-O3", "-lineinfo", "-std=c++17", "-cudart", "static",
-                               PEAKS_SRC, "-o", tmp])
-        os.replace(tmp, PEAKS_BIN)
-    return PEAKS_BIN
 
 
 def _compile(unit, force: bool, verbose: bool) -> tuple[str, bool]:
@@ -93,4 +78,3 @@ if __name__ == "__main__":
     import sys
 
     print(build(force=True, verbose="-v" in sys.argv))
-    print(build_peaks(force=True))

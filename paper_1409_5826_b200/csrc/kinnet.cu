@@ -94,6 +94,7 @@ struct KParams {
     // integrator parameters
     double kappa, eps_y, y_floor, growth;
     long long max_steps;
+    int method;  // 0 = asymptotic / Euler, 1 = QSS variant
 };
 
 
@@ -278,7 +279,11 @@ __global__ void __launch_bounds__(TB) zone_kernel(const KParams p) {
             const real h = static_cast<real>(dts);
             const real k = (y > 0) ? Fm / y : static_cast<real>(0);
             const real kdt = k * h;
-            if (kdt >= kappa)
+            if (p.method == 1) {  // QSS variant (reading Q20)
+                const real num = ((kdt + static_cast<real>(11)) * kdt + static_cast<real>(60)) * kdt + static_cast<real>(180);
+                const real den = ((kdt + static_cast<real>(12)) * kdt + static_cast<real>(60)) * kdt + static_cast<real>(360);
+                y = y + h * (Fp - Fm) / (static_cast<real>(1) + num / den * kdt);
+            } else if (kdt >= kappa)
                 y = (y + h * Fp) / (static_cast<real>(1) + kdt);
             else
                 y = y + h * (Fp - Fm);
@@ -467,16 +472,16 @@ int pull_block(const net* n) { return n->pull2 ? n->PS.T / 2 : n->PS.T; }
 pull_fn pick_pull(const net* n, bool adaptive) {
     if (n->pull2) {
         if (adaptive)
-            return n->P.precision == 32 ? kinnet::pull2_kernel_f32_adaptive(n->PS)
-                                        : kinnet::pull2_kernel_f64_adaptive(n->PS);
-        return n->P.precision == 32 ? kinnet::pull2_kernel_f32_fixed(n->PS)
-                                    : kinnet::pull2_kernel_f64_fixed(n->PS);
+            return n->P.precision == 32 ? kinnet::pull2_kernel_f32_adaptive(n->PS, n->P.method)
+                                        : kinnet::pull2_kernel_f64_adaptive(n->PS, n->P.method);
+        return n->P.precision == 32 ? kinnet::pull2_kernel_f32_fixed(n->PS, n->P.method)
+                                    : kinnet::pull2_kernel_f64_fixed(n->PS, n->P.method);
     }
     if (adaptive)
-        return n->P.precision == 32 ? kinnet::pull_kernel_f32_adaptive(n->PS)
-                                    : kinnet::pull_kernel_f64_adaptive(n->PS);
-    return n->P.precision == 32 ? kinnet::pull_kernel_f32_fixed(n->PS)
-                                : kinnet::pull_kernel_f64_fixed(n->PS);
+        return n->P.precision == 32 ? kinnet::pull_kernel_f32_adaptive(n->PS, n->P.method)
+                                    : kinnet::pull_kernel_f64_adaptive(n->PS, n->P.method);
+    return n->P.precision == 32 ? kinnet::pull_kernel_f32_fixed(n->PS, n->P.method)
+                                : kinnet::pull_kernel_f64_fixed(n->PS, n->P.method);
 }
 
 size_t pull_smem(const net* n) {
@@ -605,6 +610,7 @@ void fill_pull(const net* n, KPull& k) {
     k.agg_ent = n->D.p_agg_ent;
     k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
     k.growth = n->P.growth; k.max_steps = static_cast<int>(n->P.max_steps);
+    k.method = n->P.method;
 }
 
 int launch_pull(net* n, int zones, KPull& k, void* stream) {
@@ -687,6 +693,7 @@ void fill_params(const net* n, KParams& k) {
     k.big_slot = n->D.big_slot;
     k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
     k.growth = n->P.growth; k.max_steps = n->P.max_steps;
+    k.method = n->P.method;
 }
 
 template <int MODE>
@@ -717,6 +724,10 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
     if (n->P.precision != 64 && n->P.precision != 32) {
         delete n;
         return fail(NET_EINVAL, "precision must be 64 or 32");
+    }
+    if (n->P.method != 0 && n->P.method != 1) {
+        delete n;
+        return fail(NET_EINVAL, "method must be 0 (asymptotic) or 1 (QSS)");
     }
     if (!(n->P.kappa > 0) || !(n->P.eps_y > 0) || !(n->P.y_floor > 0) || !(n->P.growth > 1) ||
         n->P.max_steps < 1 || n->P.max_steps > 2000000000LL) {
@@ -824,6 +835,7 @@ int net_default_params(net_params_t* p) {
     p->precision = 64;
     p->kernel = 0;
     p->host_chunk = 0;
+    p->method = 0;
     return NET_OK;
 }
 

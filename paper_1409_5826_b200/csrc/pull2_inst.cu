@@ -10,7 +10,7 @@
 
 namespace kinnet {
 
-pull_fn PULL_FN(const PullSchedule& P) { return pick_pull2<PULL_REAL, PULL_ADAPT != 0>(P); }
+pull_fn PULL_FN(const PullSchedule& P, int method) { return pick_pull2<PULL_REAL, PULL_ADAPT != 0>(P, method); }
 
 #if PULL_ADAPT != 0 && defined(PULL2_DEFINE_SUPPORTED)
 bool pull2_supported(const PullSchedule& P, int* spill) {

@@ -11,6 +11,6 @@
 
 namespace kinnet {
 
-pull_fn PULL_FN(const PullSchedule& P) { return pick_pull_real<PULL_REAL, PULL_ADAPT != 0>(P); }
+pull_fn PULL_FN(const PullSchedule& P, int method) { return pick_pull_real<PULL_REAL, PULL_ADAPT != 0>(P, method); }
 
 }  // namespace kinnet

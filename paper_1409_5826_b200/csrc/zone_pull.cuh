@@ -42,16 +42,9 @@ constexpr int kJ2C = kinnet::kPullMaxSlots2;
 // only the warp with the longest rows reaches them (the species are dealt to threads by
 // falling in-degree), and every thread gets the registers back.  Measured on configs[3]
 // (zone-networks/s): 0 -> 161.7k, 4 -> 172.7k, 8 -> 165.0k, 12 -> 171.2k, 16 -> 173.1k.
-#ifndef KINNET_SPILL_SLOTS
-#define KINNET_SPILL_SLOTS 4
-#endif
-constexpr int kPullSpillSlots = KINNET_SPILL_SLOTS;
-
-// resident CTAs per SM the 160-thread instantiation is compiled for (register budget
-// 65536 / (160 * MINB)); build.py may override it for A/B runs
-#ifndef KINNET_MINB160
-#define KINNET_MINB160 3
-#endif
+constexpr int kPullSpillSlots = 4;
+// (the 160-thread instantiation is compiled for 3 resident CTAs per SM, 4 with fp32 state:
+// register budget 65536 / (160 * MINB); 4 with fp64 state spills: 152.6k against 172.5k)
 
 struct KPull {
     int N, M, nbs;
@@ -79,6 +72,7 @@ struct KPull {
     double t_hydro, dt_fixed;
     double kappa, eps_y, y_floor, growth;
     int n_fixed, max_steps;
+    int method;               // 0 = asymptotic / Euler, 1 = QSS variant (net_params_t.method)
 };
 
 
@@ -86,20 +80,17 @@ typedef void (*pull_fn)(const KPull);
 
 template <typename real>
 __host__ __device__ inline size_t pull_smem_bytes(int T, int W, int M) {
-#ifndef KINNET_PAD_SMEM
-#define KINNET_PAD_SMEM 0  // occupancy experiments: extra bytes that lower the CTAs per SM
-#endif
     return 32 * sizeof(double) +
            sizeof(real) * (static_cast<size_t>(W) * 8 + 4 * T + 4 + kPullSpillSlots * T) +
-           sizeof(double) * static_cast<size_t>(M) + KINNET_PAD_SMEM;
+           sizeof(double) * static_cast<size_t>(M);
 }
 
 // Kernel for a compiled pull schedule; one definition per (state type, adaptive/fixed)
 // pair, each in its own translation unit (pull_inst.cu).
-pull_fn pull_kernel_f64_adaptive(const PullSchedule& P);
-pull_fn pull_kernel_f64_fixed(const PullSchedule& P);
-pull_fn pull_kernel_f32_adaptive(const PullSchedule& P);
-pull_fn pull_kernel_f32_fixed(const PullSchedule& P);
+pull_fn pull_kernel_f64_adaptive(const PullSchedule& P, int method);
+pull_fn pull_kernel_f64_fixed(const PullSchedule& P, int method);
+pull_fn pull_kernel_f32_adaptive(const PullSchedule& P, int method);
+pull_fn pull_kernel_f32_fixed(const PullSchedule& P, int method);
 
 #ifdef KINNET_PULL_INSTANTIATE
 
@@ -157,12 +148,22 @@ __device__ __forceinline__ real lds_at(uint32_t a) {
 }
 
 
+// QSS variant (reading Q20): alpha(a) k with a = k dt, the weight of
+// the loss term in  y' = y + dt (F+ - k y)/(1 + alpha a) = y + (F+ - k y)/(q + alpha k),  q = 1/dt.
+template <typename real>
+__device__ __forceinline__ real qss_alpha_k(real k, real h) {
+    const real a = k * h;
+    const real num = fma(fma(a + static_cast<real>(11), a, static_cast<real>(60)), a, static_cast<real>(180));
+    const real den = fma(fma(a + static_cast<real>(12), a, static_cast<real>(60)), a, static_cast<real>(360));
+    return num * rcp_pos(den) * k;
+}
+
 template <typename real>
 __device__ __forceinline__ real abs_of(real a) {
     return a < 0 ? -a : a;
 }
 
-template <typename real, int TB, int MINB, int CP, int J2, bool ADAPT>
+template <typename real, int TB, int MINB, int CP, int J2, bool ADAPT, bool QSS>
 __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     static_assert(CP % 4 == 0 && CP <= kinnet::kPullMaxSlots, "slot capacity");
     static_assert(J2 % 4 == 0 && J2 <= kJ2C, "second-factor slot capacity");
@@ -262,6 +263,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
     const real y_floor = static_cast<real>(p.y_floor);
     const double growth = p.growth, t_hydro = p.t_hydro;
     const bool rhs_only = p.mode == kRhs;
+    constexpr bool qss = QSS;  // net_params_t.method = 1, an instantiation (see zone_pull2.cuh)
 
     // The controller runs on q = 1/dt: the candidates become
     // |F+ - F-| / (eps max(y, floor)), their reciprocal factor is formed while the
@@ -507,6 +509,7 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             const real ya = fma(y, qr, Fp) * rcp_pos(qr + k);
             const real ye = fma(h, change, y);
             yn = (y > 0 && k * h >= kappa_) ? ya : ye;
+            if (qss) yn = fma(change, rcp_pos(qr + qss_alpha_k(y > 0 ? k : static_cast<real>(0), h)), y);  // uniform
         }
         {  // hub species, on lanes 0..nbs-1 of every warp: Y (Y q + F+) / (Y q + F-)
             const bool pos = yme > Tiny<real>::v();
@@ -514,6 +517,10 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
             const real ya = fma(yme, qr, hFp) * (yme * rcp_pos(pos ? den : static_cast<real>(1)));
             const real ye = fma(h, hFp - hFm, yme);
             real hn = (pos && h * hFm >= kappa_ * yme) ? ya : ye;
+            if (qss) {
+                const real kh = pos ? hFm * rcp_pos(pos ? yme : static_cast<real>(1)) : static_cast<real>(0);
+                hn = fma(hFp - hFm, rcp_pos(qr + qss_alpha_k(kh, h)), yme);
+            }
             if (lane >= nbs) hn = 0;  // a missing hub reads as abundance 0
             yh0 = __shfl_sync(0xffffffffu, hn, 0);  // unconditional: the three go out back to back
             yh1 = __shfl_sync(0xffffffffu, hn, 1);
@@ -548,31 +555,33 @@ __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {
 // pull kernel: block-size classes with the residency the register file allows
 // (65536 / (TB * MINB) registers per thread) x P-slot capacity classes
 
-template <typename real, int CP, int J2, bool ADAPT>
+template <typename real, int CP, int J2, bool ADAPT, bool QSS>
 pull_fn pick_pull_block(int T) {
     switch (T) {
-        case 32: return zone_kernel_pull<real, 32, 12, CP, J2, ADAPT>;
-        case 64: return zone_kernel_pull<real, 64, 6, CP, J2, ADAPT>;
-        case 160: return zone_kernel_pull<real, 160, sizeof(real) == 8 ? KINNET_MINB160 : KINNET_MINB160 + 1, CP, J2, ADAPT>;  // fp32 state halves the rate registers
-        case 256: return zone_kernel_pull<real, 256, 2, CP, J2, ADAPT>;
-        case 384: return zone_kernel_pull<real, 384, 1, CP, J2, ADAPT>;
-        default: return zone_kernel_pull<real, 512, 1, CP, J2, ADAPT>;
+        case 32: return zone_kernel_pull<real, 32, 12, CP, J2, ADAPT, QSS>;
+        case 64: return zone_kernel_pull<real, 64, 6, CP, J2, ADAPT, QSS>;
+        case 160: return zone_kernel_pull<real, 160, sizeof(real) == 8 ? 3 : 4, CP, J2, ADAPT, QSS>;  // fp32 state halves the rate registers
+        case 256: return zone_kernel_pull<real, 256, 2, CP, J2, ADAPT, QSS>;
+        case 384: return zone_kernel_pull<real, 384, 1, CP, J2, ADAPT, QSS>;
+        default: return zone_kernel_pull<real, 512, 1, CP, J2, ADAPT, QSS>;
     }
 }
 
-template <typename real, int J2, bool ADAPT>
+template <typename real, int J2, bool ADAPT, bool QSS>
 pull_fn pick_pull_slots(const kinnet::PullSchedule& P) {
-    if (P.slots <= 12) return pick_pull_block<real, 12, J2, ADAPT>(P.T);
-    if (P.slots <= 20) return pick_pull_block<real, 20, J2, ADAPT>(P.T);
-    return pick_pull_block<real, 24, J2, ADAPT>(P.T);
+    if (P.slots <= 12) return pick_pull_block<real, 12, J2, ADAPT, QSS>(P.T);
+    if (P.slots <= 20) return pick_pull_block<real, 20, J2, ADAPT, QSS>(P.T);
+    return pick_pull_block<real, 24, J2, ADAPT, QSS>(P.T);
 }
 
 // P-slot capacity classes x second-factor capacity classes (the packed offsets of
-// the unused capacity would only hold registers)
+// the unused capacity would only hold registers); the QSS variant is instantiated for the
+// larger second-factor class only
 template <typename real, bool ADAPT>
-pull_fn pick_pull_real(const kinnet::PullSchedule& P) {
-    if (P.slots2 <= 4) return pick_pull_slots<real, 4, ADAPT>(P);
-    return pick_pull_slots<real, 8, ADAPT>(P);
+pull_fn pick_pull_real(const kinnet::PullSchedule& P, int method = 0) {
+    if (method == 1) return pick_pull_slots<real, 8, ADAPT, true>(P);
+    if (P.slots2 <= 4) return pick_pull_slots<real, 4, ADAPT, false>(P);
+    return pick_pull_slots<real, 8, ADAPT, false>(P);
 }
 
 #endif  // KINNET_PULL_INSTANTIATE

@@ -28,10 +28,11 @@ __host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill) {  
            sizeof(double) * static_cast<size_t>(M);
 }
 
-pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P);
-pull_fn pull2_kernel_f64_fixed(const PullSchedule& P);
-pull_fn pull2_kernel_f32_adaptive(const PullSchedule& P);
-pull_fn pull2_kernel_f32_fixed(const PullSchedule& P);
+// method = net_params_t.method (1 = the QSS instantiations)
+pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P, int method);
+pull_fn pull2_kernel_f64_fixed(const PullSchedule& P, int method);
+pull_fn pull2_kernel_f32_adaptive(const PullSchedule& P, int method);
+pull_fn pull2_kernel_f32_fixed(const PullSchedule& P, int method);
 // slots of the two sides of a schedule compiled for virtual threads; false when no
 // instantiation covers it (the caller then compiles the one-species schedule)
 bool pull2_supported(const PullSchedule& P, int* spill);
@@ -92,7 +93,9 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 // NS = 4 compiles the N-slots in (networks with heavy + heavy reactions, schedule.h): four more
 // gathers per side into k, skipped by the warps none of whose species has one, and the hub
 // owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
-template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT>
+// QSS compiles the quasi-steady-state variant of the update in (net_params_t.method = 1); a
+// run-time switch costs the default kernel 6 % (registers), so it is an instantiation.
+template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS>
 __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
@@ -227,6 +230,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     const real yfl_eps = eps_y * y_floor;
     const double growth = p.growth, t_hydro = p.t_hydro;
     const bool rhs_only = p.mode == kRhs;
+    constexpr bool qss = QSS;
 
     double t = 0.0, q_prev = 0.0, dt_out = 0.0;
     int steps = 0;
@@ -490,6 +494,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             const real ea = fma(h, cha, ya), eb = fma(h, chb, yb);
             yna = (ya > 0 && ka * h >= kappa) ? aa : ea;
             ynb = (yb > 0 && kb * h >= kappa) ? ab : eb;
+            if (qss) {  // uniform: the QSS variant, one formula for every species
+                yna = fma(cha, rcp_pos(qr + qss_alpha_k(ya > 0 ? ka : static_cast<real>(0), h)), ya);
+                ynb = fma(chb, rcp_pos(qr + qss_alpha_k(yb > 0 ? kb : static_cast<real>(0), h)), yb);
+            }
         }
         {  // hub species, on lanes 0..nbs-1 of every warp: Y (Y q + F+) / (Y q + F-)
             const bool pos = yme > Tiny<real>::v();
@@ -497,6 +505,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             const real as = fma(yme, qr, hFp) * (yme * rcp_pos(pos ? den : static_cast<real>(1)));
             const real es = fma(h, hFp - hFm, yme);
             real hn = (pos && h * hFm >= kappa * yme) ? as : es;
+            if (qss) {
+                const real kh = pos ? hFm * rcp_pos(pos ? yme : static_cast<real>(1)) : static_cast<real>(0);
+                hn = fma(hFp - hFm, rcp_pos(qr + qss_alpha_k(kh, h)), yme);
+            }
             if (lane >= nbs) hn = 0;  // a missing hub reads as abundance 0
             yh0 = __shfl_sync(0xffffffffu, hn, 0);
             yh1 = __shfl_sync(0xffffffffu, hn, 1);
@@ -554,30 +566,36 @@ inline bool pull2_sides(const PullSchedule& P, int& slots_a, int& slots_b, int& 
 inline int pull2_cap_a(int slots_a) { return slots_a <= 20 ? 20 : 24; }
 
 template <typename real, int TB, int CPA, bool ADAPT>
-pull_fn pick_pull2_j2(int s2, int ns) {
-    // networks with N-slots have two-factor P-slots anyway: one second-factor class for them
-    if (ns > 0)
-        return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, kPullNSlots, ADAPT>;
-    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 4, 0, ADAPT>;
-    return zone_kernel_pull2<real, TB, CPA, CPA - kPull2RegA, kPull2CapB, kPull2SpillB, 8, 0, ADAPT>;
+pull_fn pick_pull2_j2(int s2, int ns, bool qss) {
+    // networks with N-slots have two-factor P-slots anyway: one second-factor class for them;
+    // the QSS variant is instantiated for the larger second-factor class only
+    constexpr int SA = CPA - kPull2RegA, CB = kPull2CapB, SB = kPull2SpillB, NS = kPullNSlots;
+    if (qss) {
+        if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, true>;
+        return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, true>;
+    }
+    if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, false>;
+    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false>;
+    return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false>;
 }
 template <typename real, int TB, bool ADAPT>
-pull_fn pick_pull2_cap(int sa, int s2, int ns) {
-    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2, ns);
-    return pick_pull2_j2<real, TB, 24, ADAPT>(s2, ns);
+pull_fn pick_pull2_cap(int sa, int s2, int ns, bool qss) {
+    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2, ns, qss);
+    return pick_pull2_j2<real, TB, 24, ADAPT>(s2, ns, qss);
 }
 template <typename real, bool ADAPT>
-pull_fn pick_pull2(const PullSchedule& P) {
+pull_fn pick_pull2(const PullSchedule& P, int method = 0) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2)) return nullptr;
     if (sa > 24 || sb > kPull2CapB || s2 > kJ2C) return nullptr;
+    const bool qss = method == 1;
     switch (P.T / 2) {
-        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2, P.nslots);
-        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2, P.nslots);
-        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2, P.nslots);
-        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2, P.nslots);
-        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2, P.nslots);
-        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2, P.nslots);
+        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2, P.nslots, qss);
+        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2, P.nslots, qss);
+        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2, P.nslots, qss);
+        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2, P.nslots, qss);
+        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2, P.nslots, qss);
+        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2, P.nslots, qss);
         default: return nullptr;
     }
 }

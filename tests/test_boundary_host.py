@@ -26,8 +26,8 @@ def test_library_exports_every_declared_symbol():
 
 def test_default_params():
     p = K.net_default_params()
-    assert (p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel, p.host_chunk) == (
-        1.0, 0.05, 1e-10, 2.0, 10_000_000, 64, 0, 0)
+    assert (p.kappa, p.eps_y, p.y_floor, p.growth, p.max_steps, p.precision, p.kernel, p.host_chunk,
+            p.method) == (1.0, 0.05, 1e-10, 2.0, 10_000_000, 64, 0, 0, 0)
 
 
 def test_integrate_without_device_copy_fails_loudly(g16):
