@@ -19,13 +19,43 @@ namespace kinnet {
 // once per sub-step, conflict-free, they would otherwise hold 36 registers of the 168
 // that let four CTAs share an SM (16 K registers per scheduler: 3 warps of <= 168).
 constexpr int kPull2SmemCoefs = 9;
+// Spilled slot rates per thread that tensor memory takes (the rest stay in shared memory): with
+// the 18 G coefficients that is 60 of the 64 columns a CTA may hold when five share an SM.
+constexpr int kPull2TmemRates = 12;
 
+// spill = slot rates of both sides kept out of registers.  tmem: they and the G coefficients
+// live in tensor memory instead of shared memory (pull2_uses_tmem).
 template <typename real>
-__host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill) {  // spill = slot rates of both sides kept in shared memory
-    return 32 * sizeof(double) +
-           sizeof(real) * (static_cast<size_t>(TB / 32) * 8 + 8 * TB + 4 + static_cast<size_t>(spill) * TB +
-                           static_cast<size_t>(kPull2SmemCoefs) * 2 * TB) +
+__host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill, bool tmem, bool ksmem) {
+    // with tensor memory holding G and the spilled rates, the K coefficients move from registers
+    // to shared memory: 128 registers instead of 168 = a fifth resident CTA per SM
+    const size_t coef = tmem ? static_cast<size_t>(ksmem ? kPullCoefs - kPull2SmemCoefs : 0) * 2 * TB +
+                                   static_cast<size_t>(spill > kPull2TmemRates ? spill - kPull2TmemRates : 0) * TB
+                             : static_cast<size_t>(spill) * TB + static_cast<size_t>(kPull2SmemCoefs) * 2 * TB;
+    return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(TB / 32) * 8 + 8 * TB + 4 + coef) +
            sizeof(double) * static_cast<size_t>(M);
+}
+
+// Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) as a LANE-PRIVATE store for what
+// a thread re-reads every sub-step and never changes during the call: the G coefficients and the
+// slot rates that do not fit the registers.  tcgen05.ld reaches a warp's own 32 lanes at ~12
+// cycles and does not touch the shared-memory pipe, which is this kernel's busiest unit
+// (measured: a saturated LDS stream loses nothing to a concurrent tcgen05.ld stream).  Block
+// sizes from 96 threads up (at most four CTAs per SM, so the columns always fit); smaller
+// networks keep everything in shared memory.
+inline bool pull2_uses_tmem(int TB) { return TB >= 96; }
+// ... and then, for networks without N-slots, the K coefficients live in shared memory: 128
+// registers instead of 168, a fifth resident 96-thread CTA per SM (217k -> 235k zone-networks/s on
+// configs[3]).  With N-slots the 128-register build spills and loses (180.8k against 186.7k).
+inline bool pull2_k_in_smem(int TB, int nslots) { return pull2_uses_tmem(TB) && nslots == 0; }
+// tensor-memory columns one CTA allocates (power of two >= 32): per thread the 18 G coefficients
+// and up to kPull2TmemRates spilled rates, 4-byte words, one column group per four warps
+inline int pull2_tmem_cols(int TB, int spill, int real_bytes) {
+    const int rows = 2 * kPull2SmemCoefs + (spill < kPull2TmemRates ? spill : kPull2TmemRates);
+    const int need = (real_bytes / 4) * rows * ((TB / 32 + 3) / 4);
+    int cols = 32;
+    while (cols < need) cols *= 2;
+    return cols;
 }
 
 // method = net_params_t.method (1 = the QSS instantiations)
@@ -39,6 +69,92 @@ bool pull2_supported(const PullSchedule& P, int* spill);
 
 #ifdef KINNET_PULL_INSTANTIATE
 
+// ---- tcgen05.ld / st on the calling warp's own lanes (32x32b: lane i <-> thread i of the warp)
+#define KINNET_TM_LD(N, OUTS, ...)                                                                   \
+    __device__ __forceinline__ void tm_ld(uint32_t (&r)[N], uint32_t a) {                           \
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x" #N ".b32 {" OUTS "}, [%" #N "];" : __VA_ARGS__ : "r"(a)); \
+    }                                                                                               \
+    /* the wait names the registers so that no use of them can be scheduled above it */            \
+    __device__ __forceinline__ void tm_wait(uint32_t (&r)[N]) {                                     \
+        asm volatile("tcgen05.wait::ld.sync.aligned;" : KINNET_TM_INOUT##N(r)::"memory");           \
+    }                                                                                               \
+    __device__ __forceinline__ void tm_touch(uint32_t (&r)[N]) { asm volatile("" : KINNET_TM_INOUT##N(r)); }
+#define KINNET_TM_INOUT1(r) "+r"(r[0])
+#define KINNET_TM_INOUT2(r) KINNET_TM_INOUT1(r), "+r"(r[1])
+#define KINNET_TM_INOUT4(r) KINNET_TM_INOUT2(r), "+r"(r[2]), "+r"(r[3])
+#define KINNET_TM_INOUT8(r) KINNET_TM_INOUT4(r), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7])
+#define KINNET_TM_INOUT16(r)                                                                         \
+    KINNET_TM_INOUT8(r), "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+KINNET_TM_LD(1, "%0", "=r"(r[0]))
+KINNET_TM_LD(2, "%0,%1", "=r"(r[0]), "=r"(r[1]))
+KINNET_TM_LD(4, "%0,%1,%2,%3", "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]))
+KINNET_TM_LD(8, "%0,%1,%2,%3,%4,%5,%6,%7", "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]),
+             "=r"(r[6]), "=r"(r[7]))
+KINNET_TM_LD(16, "%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15", "=r"(r[0]), "=r"(r[1]), "=r"(r[2]),
+             "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]),
+             "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]))
+#undef KINNET_TM_LD
+
+__device__ __forceinline__ void tm_st(uint32_t a, double v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(a), "r"(__double2loint(v)),
+                 "r"(__double2hiint(v))
+                 : "memory");
+}
+__device__ __forceinline__ void tm_st(uint32_t a, float v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(a), "r"(__float_as_uint(v)) : "memory");
+}
+__device__ __forceinline__ double tm_val(uint32_t lo, uint32_t hi) {
+    return __hiloint2double(static_cast<int>(hi), static_cast<int>(lo));
+}
+// the nine G coefficients of both sides of a thread: columns [0, 9 W) and [9 W, 18 W), W words per value
+__device__ __forceinline__ void tm_load_g(double (&Ga)[9], double (&Gb)[9], uint32_t a) {
+    uint32_t u[16], v[16], w[4];
+    tm_ld(u, a);
+    tm_ld(v, a + 16);
+    tm_ld(w, a + 32);
+    tm_wait(u);
+    tm_touch(v);
+    tm_touch(w);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) Ga[j] = tm_val(u[2 * j], u[2 * j + 1]);
+    Ga[8] = tm_val(v[0], v[1]);
+#pragma unroll
+    for (int j = 0; j < 7; ++j) Gb[j] = tm_val(v[2 + 2 * j], v[3 + 2 * j]);
+    Gb[7] = tm_val(w[0], w[1]);
+    Gb[8] = tm_val(w[2], w[3]);
+}
+__device__ __forceinline__ void tm_load_g(float (&Ga)[9], float (&Gb)[9], uint32_t a) {
+    uint32_t u[16], v[2];
+    tm_ld(u, a);
+    tm_ld(v, a + 16);
+    tm_wait(u);
+    tm_touch(v);
+#pragma unroll
+    for (int j = 0; j < 9; ++j) Ga[j] = __uint_as_float(u[j]);
+#pragma unroll
+    for (int j = 0; j < 7; ++j) Gb[j] = __uint_as_float(u[9 + j]);
+    Gb[7] = __uint_as_float(v[0]);
+    Gb[8] = __uint_as_float(v[1]);
+}
+// four consecutive spilled rates
+__device__ __forceinline__ void tm_load4(double (&x)[4], uint32_t a) {
+    uint32_t u[8];
+    tm_ld(u, a);
+    tm_wait(u);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) x[j] = tm_val(u[2 * j], u[2 * j + 1]);
+}
+__device__ __forceinline__ void tm_load4(float (&x)[4], uint32_t a) {
+    uint32_t u[4];
+    tm_ld(u, a);
+    tm_wait(u);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) x[j] = __uint_as_float(u[j]);
+}
+__host__ __device__ constexpr uint32_t tm_alloc_cols(uint32_t need) {
+    return need <= 32 ? 32 : need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
+}
+
 // One side (one species) of a thread: everything that is loop invariant.
 template <typename real, int CP, int CPR, int J2, int NS>
 struct PullSide {
@@ -50,13 +166,11 @@ struct PullSide {
 };
 
 // k = F-/y and the six hub-row shares of one species (see zone_pull.cuh)
-template <typename real, int TV>
-__device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPull2SmemCoefs], uint32_t s_G,
-                                               real y, real p1, real p2, real p3, real yh0, real yh1,
-                                               real yh2, real& k, real (&share)[6]) {
-    real G[kPull2SmemCoefs];
-#pragma unroll
-    for (int j = 0; j < kPull2SmemCoefs; ++j) G[j] = lds_at<real>(s_G + j * TV * sizeof(real));
+template <typename real>
+__device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPull2SmemCoefs],
+                                               const real (&G)[kPull2SmemCoefs], real y, real p1, real p2,
+                                               real p3, real yh0, real yh1, real yh2, real& k,
+                                               real (&share)[6]) {
     real e0 = fma(C[4], yh0, C[1]);
     e0 = fma(C[5], yh1, e0);
     e0 = fma(C[6], yh2, e0);
@@ -95,8 +209,9 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 // owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
 // QSS compiles the quasi-steady-state variant of the update in (net_params_t.method = 1); a
 // run-time switch costs the default kernel 6 % (registers), so it is an instantiation.
-template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS>
-__global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
+// TM: G coefficients and spilled slot rates in tensor memory instead of shared memory.
+template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS, bool TM>
+__global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
@@ -113,9 +228,18 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     double* redq = reinterpret_cast<double*>(smem_raw);       // [32] per-warp q maxima, [16..18] own terms
     real* red = reinterpret_cast<real*>(redq + 32);           // [NW][8] per-warp hub-row sums
     real* YP = red + NW * 8;                                  // [4][TV] published products, then 1
-    real* Rx = YP + 4 * TV + 4;                               // [SPA + SPB + 2 NS][T] spilled slot rates, N-slot rates
-    real* Gs = Rx + (SPA + SPB + 2 * NS) * T;                         // [9][TV] G0, Gx of every virtual thread
-    double* Rbuf = reinterpret_cast<double*>(Gs + kPull2SmemCoefs * TV);  // [M] rates, set-up only
+    constexpr int NRX = SPA + SPB + 2 * NS;                   // slot rates kept out of registers, per thread
+    real* Rx = YP + 4 * TV + 4;                               // [NRX - NRT][T] spilled slot rates, N-slot rates
+    constexpr int NRT = TM ? (NRX < kPull2TmemRates ? NRX : kPull2TmemRates) : 0;  // rate rows in tensor memory
+    real* Gs = Rx + (NRX - NRT) * T;                          // [9][TV] G0, Gx of every virtual thread      (not TM)
+    constexpr int NK = kPullCoefs - kPull2SmemCoefs;          // K coefficients per species
+    constexpr bool KS = TM && NS == 0;                        // K in shared memory instead of registers
+    real* Ks = Gs;                                            // [NK][TV] K of every virtual thread          (KS)
+    double* Rbuf = reinterpret_cast<double*>(Gs + (TM ? (KS ? NK * TV : 0) : kPull2SmemCoefs * TV));  // [M] rates, set-up only
+    // tensor-memory columns of a thread (TM): G of side a, G of side b, then the NRX rates
+    constexpr uint32_t RW = sizeof(real) / 4, TMC = RW * (2 * kPull2SmemCoefs + NRT);
+    constexpr uint32_t TM_ALLOC = tm_alloc_cols(TMC * ((NW + 3) / 4));
+    __shared__ uint32_t tm_slot;
     uint32_t s_redq;
     asm volatile("mov.u32 %0, %1;"
                  : "=r"(s_redq)
@@ -125,8 +249,15 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     const uint32_t s_Rx = s_YP + (4 * TV + 4) * SZ + tid * SZ;
     const uint32_t s_own = s_redq + 16 * 8;   // [3] own-consumption terms of the hub owners
     const uint32_t s_ownp = s_redq + 20 * 8;  // [3] their own P-slot sums (NS > 0)
-    const uint32_t s_G = s_YP + (4 * TV + 4 + (SPA + SPB + 2 * NS) * T) * SZ;
+    const uint32_t s_G = s_YP + (4 * TV + 4 + (NRX - NRT) * T) * SZ;
     if (s_YP + (4 * TV + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
+    if (TM && warp == 0) {  // one warp allocates this CTA's columns; the address arrives through shared memory
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         static_cast<uint32_t>(__cvta_generic_to_shared(&tm_slot))),
+                     "n"(TM_ALLOC)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
 
     PullSide<real, CPA, CPRA, J2, NS> A;
     PullSide<real, CPB, CPRB, J2, NS> B;
@@ -171,7 +302,19 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         }
     }
     if (tid < 4) YP[4 * TV + tid] = static_cast<real>(1);
+    if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    uint32_t tm_base = 0;  // this thread's lane quarter and first column
+    if (TM) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tm_base = *reinterpret_cast<volatile uint32_t*>(&tm_slot) + (static_cast<uint32_t>(warp & 3) << 21) +
+                  static_cast<uint32_t>(warp >> 2) * TMC;
+    }
+    // spilled rate `row` (0 .. NRX) of this thread: shared memory, or tensor memory
+    auto put_rate = [&](int row, real r) {
+        if (row < NRT) tm_st(tm_base + RW * (2 * kPull2SmemCoefs + row), r);
+        else Rx[(row - NRT) * T + tid] = r;
+    };
 
     auto slot_rate = [&](int e, int v) -> real {
         const int32_t w = p.slot_rxn[e * TV + v];
@@ -182,20 +325,20 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     for (int e = 0; e < CPA; ++e) {
         const real r = slot_rate(e, va);
         if (e < CPRA) A.R[e] = r;
-        else Rx[(e - CPRA) * T + tid] = r;
+        else put_rate(e - CPRA, r);
     }
 #pragma unroll
     for (int e = 0; e < CPB; ++e) {
         const real r = slot_rate(e, vb);
         if (e < CPRB) B.R[e] = r;
-        else Rx[(SPA + e - CPRB) * T + tid] = r;
+        else put_rate(SPA + e - CPRB, r);
     }
 #pragma unroll
     for (int e = 0; e < NS; ++e) {
-        Rx[(SPA + SPB + e) * T + tid] = slot_rate(kPullMaxSlots + e, va);
-        Rx[(SPA + SPB + NS + e) * T + tid] = slot_rate(kPullMaxSlots + e, vb);
+        put_rate(SPA + SPB + e, slot_rate(kPullMaxSlots + e, va));
+        put_rate(SPA + SPB + NS + e, slot_rate(kPullMaxSlots + e, vb));
     }
-    auto rate_sums = [&](real (&C)[kPullCoefs - kPull2SmemCoefs], int v) {
+    auto rate_sums = [&](real (&C)[kPullCoefs - kPull2SmemCoefs], int v, int side) {
         int q = p.agg_ptr[v];
 #pragma unroll
         for (int s = 0; s < kPullCoefs; ++s) {
@@ -206,11 +349,21 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
                 acc += static_cast<double>(w >> 24) * Rbuf[w & 0xffffff];
             }
             if (s < kPullCoefs - kPull2SmemCoefs) C[s] = static_cast<real>(acc);
+            else if (TM) tm_st(tm_base + RW * (side * kPull2SmemCoefs + s - (kPullCoefs - kPull2SmemCoefs)), static_cast<real>(acc));
             else Gs[(s - (kPullCoefs - kPull2SmemCoefs)) * TV + v] = static_cast<real>(acc);
         }
     };
-    rate_sums(A.C, va);
-    rate_sums(B.C, vb);
+    rate_sums(A.C, va, 0);
+    rate_sums(B.C, vb, 1);
+    if (TM) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    if (KS) {
+#pragma unroll
+        for (int j = 0; j < NK; ++j) {
+            Ks[j * TV + va] = A.C[j];
+            Ks[j * TV + vb] = B.C[j];
+        }
+    }
+    const uint32_t s_K = s_G;  // Ks sits where Gs would
 
     // ---- S6: zone state in ---------------------------------------------------------
     real* Yg = reinterpret_cast<real*>(p.Y) + (size_t)z * N;
@@ -264,9 +417,29 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         // ---- rate sums: k = F-/y (Eq. (1)) and the hub-row shares, added over the two ----------
         real ka, kb, share[6];
         {
-            real sb[6];
-            pull_rate_sums<real, TV>(A.C, s_G + va * SZ, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
-            pull_rate_sums<real, TV>(B.C, s_G + vb * SZ, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+            real sb[6], Ga[kPull2SmemCoefs], Gb[kPull2SmemCoefs];
+            if (TM) {
+                tm_load_g(Ga, Gb, tm_base);
+            } else {
+#pragma unroll
+                for (int j = 0; j < kPull2SmemCoefs; ++j) {
+                    Ga[j] = lds_at<real>(s_G + (j * TV + va) * SZ);
+                    Gb[j] = lds_at<real>(s_G + (j * TV + vb) * SZ);
+                }
+            }
+            if (KS) {
+                real Ka[NK], Kb[NK];
+#pragma unroll
+                for (int j = 0; j < NK; ++j) {
+                    Ka[j] = lds_at<real>(s_K + (j * TV + va) * SZ);
+                    Kb[j] = lds_at<real>(s_K + (j * TV + vb) * SZ);
+                }
+                pull_rate_sums<real>(Ka, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
+                pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+            } else {
+                pull_rate_sums<real>(A.C, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
+                pull_rate_sums<real>(B.C, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+            }
 #pragma unroll
             for (int i = 0; i < 6; ++i) share[i] += sb[i];
         }
@@ -303,7 +476,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             x3 *= lds_at<real>(hi16(v1));                                                  \
         }                                                                                  \
     }
-#define KINNET_XOFF(e) (static_cast<uint32_t>((e) >= CPRA ? (e) - CPRA : 0) * T * SZ)
 #define KINNET_FMAS_A(g)                                                        \
     if ((g) == 0) {                                                             \
         sa0 = A.R[0] * a0;                                                      \
@@ -316,12 +488,13 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         sa2 = fma(A.R[(4 * (g) + 2) % CPRA], a2, sa2);                          \
         sa3 = fma(A.R[(4 * (g) + 3) % CPRA], a3, sa3);                          \
     } else if (4 * (g) < CPA && 4 * (g) < A.wn) {                               \
-        sa0 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g))), a0, sa0);          \
-        sa1 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 1)), a1, sa1);      \
-        sa2 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 2)), a2, sa2);      \
-        sa3 = fma(lds_at<real>(s_Rx + KINNET_XOFF(4 * (g) + 3)), a3, sa3);      \
+        real xr[4];                                                             \
+        rates4(xr, (4 * (g) >= CPRA ? 4 * (g) - CPRA : 0));                     \
+        sa0 = fma(xr[0], a0, sa0);                                              \
+        sa1 = fma(xr[1], a1, sa1);                                              \
+        sa2 = fma(xr[2], a2, sa2);                                              \
+        sa3 = fma(xr[3], a3, sa3);                                              \
     }
-#define KINNET_XOFFB(e) (static_cast<uint32_t>(SPA + ((e) >= CPRB ? (e) - CPRB : 0)) * T * SZ)
 #define KINNET_FMAS_B(g)                                                        \
     if (4 * (g) < CPRB && ((g) == 0 || 4 * (g) < B.wn)) {                       \
         sb0 = fma(B.R[(4 * (g)) % CPRB], b0, sb0);                              \
@@ -329,10 +502,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
         sb2 = fma(B.R[(4 * (g) + 2) % CPRB], b2, sb2);                          \
         sb3 = fma(B.R[(4 * (g) + 3) % CPRB], b3, sb3);                          \
     } else if (4 * (g) < CPB && 4 * (g) < B.wn) {                               \
-        sb0 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g))), b0, sb0);         \
-        sb1 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 1)), b1, sb1);     \
-        sb2 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 2)), b2, sb2);     \
-        sb3 = fma(lds_at<real>(s_Rx + KINNET_XOFFB(4 * (g) + 3)), b3, sb3);     \
+        real xr[4];                                                             \
+        rates4(xr, SPA + (4 * (g) >= CPRB ? 4 * (g) - CPRB : 0));               \
+        sb0 = fma(xr[0], b0, sb0);                                              \
+        sb1 = fma(xr[1], b1, sb1);                                              \
+        sb2 = fma(xr[2], b2, sb2);                                              \
+        sb3 = fma(xr[3], b3, sb3);                                              \
     }
 #define KINNET_STAGE(g)                               \
     KINNET_LOADS(A, CPA, g, a0, a1, a2, a3)           \
@@ -341,6 +516,15 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     KINNET_FMAS_A(g)   \
     KINNET_FMAS_B(g)
             static_assert(CPRA >= 4 && CPRB >= 4, "group 0 reads its rates from registers");
+            // four consecutive spilled rates of this thread, rows row .. row + 3
+            auto rates4 = [&](real (&x)[4], int row) {
+                if (row < NRT) {
+                    tm_load4(x, tm_base + RW * (2 * kPull2SmemCoefs + row));
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) x[j] = lds_at<real>(s_Rx + (row - NRT + j) * T * SZ);
+                }
+            };
             const bool up16 = lane & 16, up8 = lane & 8, up4 = lane & 4;
             // level 16 of the butterfly (rows 0..2 = F+ shares of the hubs, 3..5 = F- shares)
             real r0 = __shfl_xor_sync(0xffffffffu, up16 ? share[0] : share[3], 16);
@@ -376,8 +560,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
 #undef KINNET_FMAS_A
 #undef KINNET_FMAS_B
 #undef KINNET_LOADS
-#undef KINNET_XOFF
-#undef KINNET_XOFFB
             // lanes 0, 8, 4, 16, 24, 20 hold the warp totals of rows 0, 1, 2, 3, 4, 5
             const int row = 3 * (lane >> 4) + ((lane & 4) ? 2 : ((lane >> 3) & 1));
             if ((lane & 3) == 0 && (lane & 12) != 12) sts(s_red + (warp * 8 + row) * SZ, tot);
@@ -385,24 +567,29 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             Fpb = (sb0 + sb1) + (sb2 + sb3);
         }
         if (NS > 0) {  // N-slots: k += sum nu R Y_partner, F- of the reactants of heavy + heavy reactions
-            constexpr uint32_t NA = (SPA + SPB) * T * SZ, NB = (SPA + SPB + NS) * T * SZ, ROW = T * SZ;
+            auto nrates4 = [&](real (&x)[4], int row) {
+                if (row < NRT) {
+                    tm_load4(x, tm_base + RW * (2 * kPull2SmemCoefs + row));
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) x[j] = lds_at<real>(s_Rx + (row - NRT + j) * T * SZ);
+                }
+            };
             if (A.wnn > 0) {  // warp-uniform: the schedule keeps these species in one warp
                 const uint32_t w0 = A.f1[CPA / 2], w1 = A.f1[(CPA + NS) / 2 - 1];
                 const real n0 = lds_at<real>(lo16(w0)), n1 = lds_at<real>(hi16(w0));
                 const real n2 = lds_at<real>(lo16(w1)), n3 = lds_at<real>(hi16(w1));
-                const real u0 = lds_at<real>(s_Rx + NA) * n0, u1 = lds_at<real>(s_Rx + NA + ROW) * n1;
-                const real u2 = fma(lds_at<real>(s_Rx + NA + 2 * ROW), n2, u0);
-                const real u3 = fma(lds_at<real>(s_Rx + NA + 3 * ROW), n3, u1);
-                ka += u2 + u3;
+                real x[4];
+                nrates4(x, SPA + SPB);
+                ka += fma(x[2], n2, x[0] * n0) + fma(x[3], n3, x[1] * n1);
             }
             if (B.wnn > 0) {
                 const uint32_t w0 = B.f1[CPB / 2], w1 = B.f1[(CPB + NS) / 2 - 1];
                 const real n0 = lds_at<real>(lo16(w0)), n1 = lds_at<real>(hi16(w0));
                 const real n2 = lds_at<real>(lo16(w1)), n3 = lds_at<real>(hi16(w1));
-                const real u0 = lds_at<real>(s_Rx + NB) * n0, u1 = lds_at<real>(s_Rx + NB + ROW) * n1;
-                const real u2 = fma(lds_at<real>(s_Rx + NB + 2 * ROW), n2, u0);
-                const real u3 = fma(lds_at<real>(s_Rx + NB + 3 * ROW), n3, u1);
-                kb += u2 + u3;
+                real x[4];
+                nrates4(x, SPA + SPB + NS);
+                kb += fma(x[2], n2, x[0] * n0) + fma(x[3], n3, x[1] * n1);
             }
             // a hub made by heavy + heavy reactions gathers those fluxes on its own thread
             if (hub_owner) sts(s_ownp + tid * SZ, Fpa);
@@ -459,6 +646,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
             if (B.own >= 0) {
                 Fpo[B.own] = Fpb;
                 Fmo[B.own] = kb * yb;
+            }
+            if (TM) {  // give the columns back (every warp is past its last tcgen05.ld)
+                __syncthreads();
+                if (warp == 0)
+                    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base & 0xffffu), "n"(TM_ALLOC));
             }
             return;
         }
@@ -530,6 +722,8 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 ? 480 : 384) / TB)
     const int bad = ((A.own >= 0) && !isfinite(static_cast<double>(ya))) ||
                     ((B.own >= 0) && !isfinite(static_cast<double>(yb)));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
+    if (TM && warp == 0)  // every warp is past its last tcgen05.ld: give the columns back
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base & 0xffffu), "n"(TM_ALLOC));
     if (p.energy) {  // uniform; Yg still holds the start-of-call abundances
         double e = 0.0;
         if (A.own >= 0) e = p.bind[A.own] * (static_cast<double>(ya) - static_cast<double>(Yg[A.own]));
@@ -570,13 +764,14 @@ pull_fn pick_pull2_j2(int s2, int ns, bool qss) {
     // networks with N-slots have two-factor P-slots anyway: one second-factor class for them;
     // the QSS variant is instantiated for the larger second-factor class only
     constexpr int SA = CPA - kPull2RegA, CB = kPull2CapB, SB = kPull2SpillB, NS = kPullNSlots;
+    constexpr bool TM = TB >= 96;  // = pull2_uses_tmem(TB)
     if (qss) {
-        if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, true>;
-        return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, true>;
+        if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, true, TM>;
+        return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, true, TM>;
     }
-    if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, false>;
-    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false>;
-    return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false>;
+    if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, false, TM>;
+    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false, TM>;
+    return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false, TM>;
 }
 template <typename real, int TB, bool ADAPT>
 pull_fn pick_pull2_cap(int sa, int s2, int ns, bool qss) {
