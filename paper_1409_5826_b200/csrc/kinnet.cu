@@ -484,15 +484,13 @@ pull_fn pick_pull(const net* n, bool adaptive) {
                                 : kinnet::pull_kernel_f64_fixed(n->PS, n->P.method);
 }
 
+int pull2_store_of(const net* n) { return kinnet::pull2_store(n->PS.T / 2, n->PS.nslots); }
+
 size_t pull_smem(const net* n) {
     if (n->pull2)
         return n->P.precision == 32
-                   ? kinnet::pull2_smem_bytes<float>(n->PS.T / 2, n->S.M, n->pull2_spill,
-                                                     kinnet::pull2_uses_tmem(n->PS.T / 2),
-                                                     kinnet::pull2_k_in_smem(n->PS.T / 2, n->PS.nslots))
-                   : kinnet::pull2_smem_bytes<double>(n->PS.T / 2, n->S.M, n->pull2_spill,
-                                                      kinnet::pull2_uses_tmem(n->PS.T / 2),
-                                                      kinnet::pull2_k_in_smem(n->PS.T / 2, n->PS.nslots));
+                   ? kinnet::pull2_smem_bytes<float>(n->PS.T / 2, n->S.M, n->pull2_spill, pull2_store_of(n))
+                   : kinnet::pull2_smem_bytes<double>(n->PS.T / 2, n->S.M, n->pull2_spill, pull2_store_of(n));
     return n->P.precision == 32 ? pull_smem_bytes<float>(n->PS.T, n->PS.W, n->S.M)
                                 : pull_smem_bytes<double>(n->PS.T, n->PS.W, n->S.M);
 }
@@ -535,7 +533,7 @@ int prepare_kernels(net* n) {
         CUDA_TRY(cudaFuncSetAttribute(f2, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       static_cast<int>(pull_smem(n))));
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, pull_block(n), pull_smem(n)));
-        if (n->pull2 && kinnet::pull2_uses_tmem(pull_block(n))) {
+        if (n->pull2 && pull2_store_of(n) != kinnet::kStoreSmem) {
             // the occupancy calculator answers 1 for a kernel that allocates tensor memory; the
             // residency is the smallest of the register, shared-memory and tensor-memory limits
             cudaFuncAttributes fa;
@@ -543,8 +541,8 @@ int prepare_kernels(net* n) {
             const int warps = pull_block(n) / 32, regs = (fa.numRegs + 7) / 8 * 8;
             const int by_regs = 4 * (16384 / (32 * regs)) / warps;
             const int by_smem = static_cast<int>((228 * 1024) / (pull_smem(n) + fa.sharedSizeBytes + 1024));
-            const int by_tmem = 512 / kinnet::pull2_tmem_cols(pull_block(n), n->pull2_spill,
-                                                              n->P.precision == 32 ? 4 : 8);
+            const int by_tmem = 512 / kinnet::pull2_tmem_cols(pull2_store_of(n), pull_block(n),
+                                                              n->P.precision == 32 ? 4 : 8, n->pull2_spill);
             nb = std::min(by_regs, std::min(by_smem, by_tmem));
         }
     } else {

@@ -146,6 +146,23 @@ __device__ __forceinline__ real lds_at(uint32_t a) {
     lds(v, a);
     return v;
 }
+// the same under a predicate (0 where it is false): a predicated LDS, no branch
+template <typename real>
+__device__ __forceinline__ real lds_if(bool on, uint32_t a);
+template <>
+__device__ __forceinline__ double lds_if<double>(bool on, uint32_t a) {
+    double v = 0.0;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q ld.shared.f64 %0, [%1]; }"
+                 : "+d"(v) : "r"(a), "r"(static_cast<uint32_t>(on)) : "memory");
+    return v;
+}
+template <>
+__device__ __forceinline__ float lds_if<float>(bool on, uint32_t a) {
+    float v = 0.0f;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %2, 0; @q ld.shared.f32 %0, [%1]; }"
+                 : "+f"(v) : "r"(a), "r"(static_cast<uint32_t>(on)) : "memory");
+    return v;
+}
 
 
 // QSS variant (reading Q20): alpha(a) k with a = k dt, the weight of
@@ -158,10 +175,9 @@ __device__ __forceinline__ real qss_alpha_k(real k, real h) {
     return num * rcp_pos(den) * k;
 }
 
-template <typename real>
-__device__ __forceinline__ real abs_of(real a) {
-    return a < 0 ? -a : a;
-}
+// |a| as an operand modifier of the multiply that follows (a select costs four instructions in fp64)
+__device__ __forceinline__ double abs_of(double a) { return fabs(a); }
+__device__ __forceinline__ float abs_of(float a) { return fabsf(a); }
 
 template <typename real, int TB, int MINB, int CP, int J2, bool ADAPT, bool QSS>
 __global__ void __launch_bounds__(TB, MINB) zone_kernel_pull(const KPull p) {

@@ -19,43 +19,57 @@ namespace kinnet {
 // once per sub-step, conflict-free, they would otherwise hold 36 registers of the 168
 // that let four CTAs share an SM (16 K registers per scheduler: 3 warps of <= 168).
 constexpr int kPull2SmemCoefs = 9;
-// Spilled slot rates per thread that tensor memory takes (the rest stay in shared memory): with
-// the 18 G coefficients that is 60 of the 64 columns a CTA may hold when five share an SM.
-constexpr int kPull2TmemRates = 12;
 
-// spill = slot rates of both sides kept out of registers.  tmem: they and the G coefficients
-// live in tensor memory instead of shared memory (pull2_uses_tmem).
-template <typename real>
-__host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill, bool tmem, bool ksmem) {
-    // with tensor memory holding G and the spilled rates, the K coefficients move from registers
-    // to shared memory: 128 registers instead of 168 = a fifth resident CTA per SM
-    const size_t coef = tmem ? static_cast<size_t>(ksmem ? kPullCoefs - kPull2SmemCoefs : 0) * 2 * TB +
-                                   static_cast<size_t>(spill > kPull2TmemRates ? spill - kPull2TmemRates : 0) * TB
-                             : static_cast<size_t>(spill) * TB + static_cast<size_t>(kPull2SmemCoefs) * 2 * TB;
-    return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(TB / 32) * 8 + 8 * TB + 4 + coef) +
-           sizeof(double) * static_cast<size_t>(M);
+// Where a thread keeps what it re-reads every sub-step (the loop-invariant coefficients):
+//   kStoreSmem    G and the spilled slot rates in shared memory, K in registers (block sizes < 96: up to
+//                 12 CTAs per SM are too many for the tensor-memory columns)
+//   kStoreTmem    G and up to 12 spilled rates in tensor memory, K in registers (168 registers, four
+//                 96-thread CTAs per SM): the instantiations with N-slots, which spill at 128 registers
+//   kStoreTmemKs  the same with K in shared memory (128 registers): 160-thread blocks, three per SM,
+//                 whose two lane groups leave each thread 64 columns
+//   kStoreTmemK   K, G and 8 or 12 spilled rates in tensor memory (128 registers, five 96-thread CTAs per SM)
+enum Pull2Store { kStoreSmem = 0, kStoreTmem = 1, kStoreTmemKs = 2, kStoreTmemK = 3 };
+__host__ __device__ constexpr int pull2_store(int TB, int nslots) {
+    return TB < 96 ? kStoreSmem : nslots > 0 ? kStoreTmem : TB == 160 ? kStoreTmemKs : kStoreTmemK;
 }
-
-// Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) as a LANE-PRIVATE store for what
-// a thread re-reads every sub-step and never changes during the call: the G coefficients and the
-// slot rates that do not fit the registers.  tcgen05.ld reaches a warp's own 32 lanes at ~12
-// cycles and does not touch the shared-memory pipe, which is this kernel's busiest unit
-// (measured: a saturated LDS stream loses nothing to a concurrent tcgen05.ld stream).  Block
-// sizes from 96 threads up (at most four CTAs per SM, so the columns always fit); smaller
-// networks keep everything in shared memory.
-inline bool pull2_uses_tmem(int TB) { return TB >= 96; }
-// ... and then, for networks without N-slots, the K coefficients live in shared memory: 128
-// registers instead of 168, a fifth resident 96-thread CTA per SM (217k -> 235k zone-networks/s on
-// configs[3]).  With N-slots the 128-register build spills and loses (180.8k against 186.7k).
-inline bool pull2_k_in_smem(int TB, int nslots) { return pull2_uses_tmem(TB) && nslots == 0; }
-// tensor-memory columns one CTA allocates (power of two >= 32): per thread the 18 G coefficients
-// and up to kPull2TmemRates spilled rates, 4-byte words, one column group per four warps
-inline int pull2_tmem_cols(int TB, int spill, int real_bytes) {
-    const int rows = 2 * kPull2SmemCoefs + (spill < kPull2TmemRates ? spill : kPull2TmemRates);
-    const int need = (real_bytes / 4) * rows * ((TB / 32 + 3) / 4);
+// Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) as a LANE-PRIVATE store: tcgen05.ld
+// reaches a warp's own 32 lanes in ~12 cycles and does not touch the shared-memory pipe, which is this
+// kernel's busiest unit (measured: a saturated LDS stream loses nothing to a concurrent tcgen05.ld
+// stream).  Layout of a thread's columns under kStoreTmemK, in values of `real` (chunks of 8 values, one
+// tcgen05.ld each, so that a 96-thread CTA can hold its 96 columns as three 32-column allocations --
+// 5 x 96 <= 512 where the power-of-two 128 would allow four CTAs only):
+//   [ 0.. 8)  K of side a: C0 C1 C4 C5 C6 C2 C7 C3     [ 8..16)  C8 C9, then G0 G3 G1 G5 G2 G7 of side a
+//   [16..32)  the same of side b                      [32..38)  G4 G6 G8 of side a, of side b; [38..40) unused
+//   [40..)    spilled slot rates
+constexpr int kPull2TmemRateBase = 40;
+// spilled slot rates per thread that tensor memory takes (the rest stay in shared memory)
+__host__ __device__ constexpr int pull2_tmem_rates(int store, int TB, int real_bytes, int spill) {
+    const int cap = store == kStoreSmem ? 0 : (store == kStoreTmemK && TB == 96 && real_bytes == 8) ? 8 : 12;
+    return spill < cap ? spill : cap;
+}
+// columns per thread (32-bit words), and what one CTA allocates
+__host__ __device__ constexpr int pull2_tmem_words(int store, int TB, int real_bytes, int spill) {
+    const int nrt = pull2_tmem_rates(store, TB, real_bytes, spill);
+    return (real_bytes / 4) * (store == kStoreTmemK ? kPull2TmemRateBase + nrt : 2 * kPull2SmemCoefs + nrt);
+}
+__host__ __device__ constexpr int pull2_tmem_cols(int store, int TB, int real_bytes, int spill) {
+    const int need = pull2_tmem_words(store, TB, real_bytes, spill) * ((TB / 32 + 3) / 4);
+    if (need > 64 && need <= 96) return 96;  // three allocations of 32
     int cols = 32;
     while (cols < need) cols *= 2;
     return cols;
+}
+
+// spill = slot rates of both sides kept out of registers
+template <typename real>
+__host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill, int store) {
+    const int nrt = pull2_tmem_rates(store, TB, static_cast<int>(sizeof(real)), spill);
+    const size_t coef = static_cast<size_t>(spill - nrt) * TB +
+                        (store == kStoreSmem     ? static_cast<size_t>(kPull2SmemCoefs) * 2 * TB
+                         : store == kStoreTmemKs ? static_cast<size_t>(kPullCoefs - kPull2SmemCoefs) * 2 * TB
+                                                 : 0);
+    return 32 * sizeof(double) + sizeof(real) * (static_cast<size_t>(TB / 32) * 8 + 8 * TB + 4 + coef) +
+           sizeof(double) * static_cast<size_t>(M);
 }
 
 // method = net_params_t.method (1 = the QSS instantiations)
@@ -151,8 +165,20 @@ __device__ __forceinline__ void tm_load4(float (&x)[4], uint32_t a) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) x[j] = __uint_as_float(u[j]);
 }
-__host__ __device__ constexpr uint32_t tm_alloc_cols(uint32_t need) {
-    return need <= 32 ? 32 : need <= 64 ? 64 : need <= 128 ? 128 : need <= 256 ? 256 : 512;
+// eight consecutive values
+__device__ __forceinline__ void tm_load8(double (&x)[8], uint32_t a) {
+    uint32_t u[16];
+    tm_ld(u, a);
+    tm_wait(u);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = tm_val(u[2 * j], u[2 * j + 1]);
+}
+__device__ __forceinline__ void tm_load8(float (&x)[8], uint32_t a) {
+    uint32_t u[8];
+    tm_ld(u, a);
+    tm_wait(u);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = __uint_as_float(u[j]);
 }
 
 // One side (one species) of a thread: everything that is loop invariant.
@@ -209,10 +235,13 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 // owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
 // QSS compiles the quasi-steady-state variant of the update in (net_params_t.method = 1); a
 // run-time switch costs the default kernel 6 % (registers), so it is an instantiation.
-// TM: G coefficients and spilled slot rates in tensor memory instead of shared memory.
-template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS, bool TM>
-__global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 480 : 384) / TB)
+// ST: where the coefficients live (Pull2Store; = pull2_store(TB, NS)).
+template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS, int ST>
+__global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
+    static_assert(ST == pull2_store(TB, NS), "store mode");
+    constexpr bool TM = ST != kStoreSmem;   // tensor memory in use
+    constexpr bool KT = ST == kStoreTmemK;  // ... for K too
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
     static_assert(NS == 0 || NS == kPullNSlots, "N-slot capacity");
@@ -230,16 +259,20 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
     real* YP = red + NW * 8;                                  // [4][TV] published products, then 1
     constexpr int NRX = SPA + SPB + 2 * NS;                   // slot rates kept out of registers, per thread
     real* Rx = YP + 4 * TV + 4;                               // [NRX - NRT][T] spilled slot rates, N-slot rates
-    constexpr int NRT = TM ? (NRX < kPull2TmemRates ? NRX : kPull2TmemRates) : 0;  // rate rows in tensor memory
+    constexpr int NRT = pull2_tmem_rates(ST, TB, sizeof(real), NRX);  // rate rows in tensor memory
     real* Gs = Rx + (NRX - NRT) * T;                          // [9][TV] G0, Gx of every virtual thread      (not TM)
     constexpr int NK = kPullCoefs - kPull2SmemCoefs;          // K coefficients per species
-    constexpr bool KS = TM && NS == 0;                        // K in shared memory instead of registers
+    constexpr bool KS = ST == kStoreTmemKs;                   // K in shared memory instead of registers
     real* Ks = Gs;                                            // [NK][TV] K of every virtual thread          (KS)
     double* Rbuf = reinterpret_cast<double*>(Gs + (TM ? (KS ? NK * TV : 0) : kPull2SmemCoefs * TV));  // [M] rates, set-up only
-    // tensor-memory columns of a thread (TM): G of side a, G of side b, then the NRX rates
-    constexpr uint32_t RW = sizeof(real) / 4, TMC = RW * (2 * kPull2SmemCoefs + NRT);
-    constexpr uint32_t TM_ALLOC = tm_alloc_cols(TMC * ((NW + 3) / 4));
-    __shared__ uint32_t tm_slot;
+    // tensor-memory columns of a thread (TM): G of side a, G of side b, then the NRT rates; KT: see
+    // pull2_store.  TM_BLK: columns per allocation (a 96-column CTA holds three of 32)
+    constexpr uint32_t RW = sizeof(real) / 4, TMC = pull2_tmem_words(ST, TB, sizeof(real), NRX);
+    constexpr uint32_t TM_COLS = pull2_tmem_cols(ST, TB, sizeof(real), NRX);
+    constexpr uint32_t TM_NBLK = TM_COLS == 96 ? 3 : 1, TM_BLK = TM_COLS / TM_NBLK;
+    constexpr uint32_t TM_RATE0 = RW * (KT ? kPull2TmemRateBase : 2 * kPull2SmemCoefs);  // first rate column
+    static_assert(TM_NBLK == 1 || NW <= 4, "split allocations: one lane group");
+    __shared__ uint32_t tm_slot[3];
     uint32_t s_redq;
     asm volatile("mov.u32 %0, %1;"
                  : "=r"(s_redq)
@@ -251,11 +284,13 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
     const uint32_t s_ownp = s_redq + 20 * 8;  // [3] their own P-slot sums (NS > 0)
     const uint32_t s_G = s_YP + (4 * TV + 4 + (NRX - NRT) * T) * SZ;
     if (s_YP + (4 * TV + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
-    if (TM && warp == 0) {  // one warp allocates this CTA's columns; the address arrives through shared memory
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
-                         static_cast<uint32_t>(__cvta_generic_to_shared(&tm_slot))),
-                     "n"(TM_ALLOC)
-                     : "memory");
+    if (TM && warp == 0) {  // one warp allocates this CTA's columns; the addresses arrive through shared memory
+#pragma unroll
+        for (uint32_t b = 0; b < TM_NBLK; ++b)
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                             static_cast<uint32_t>(__cvta_generic_to_shared(&tm_slot[b]))),
+                         "n"(TM_BLK)
+                         : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
 
@@ -304,15 +339,24 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
     if (tid < 4) YP[4 * TV + tid] = static_cast<real>(1);
     if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    uint32_t tm_base = 0;  // this thread's lane quarter and first column
+    uint32_t tm_blk[TM_NBLK] = {};  // this thread's lane quarter and first column, per allocation
     if (TM) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        tm_base = *reinterpret_cast<volatile uint32_t*>(&tm_slot) + (static_cast<uint32_t>(warp & 3) << 21) +
-                  static_cast<uint32_t>(warp >> 2) * TMC;
+#pragma unroll
+        for (uint32_t b = 0; b < TM_NBLK; ++b)
+            tm_blk[b] = *reinterpret_cast<volatile uint32_t*>(&tm_slot[b]) + (static_cast<uint32_t>(warp & 3) << 21) +
+                        static_cast<uint32_t>(warp >> 2) * TMC;
     }
+    // tensor-memory address of this thread's column c (compile-time c; no access straddles allocations)
+    auto tm_at = [&](uint32_t c) -> uint32_t { return tm_blk[TM_NBLK == 1 ? 0 : c / TM_BLK] + (TM_NBLK == 1 ? c : c % TM_BLK); };
+    auto tm_free = [&]() {  // by the allocating warp (warp 0: lane quarter 0, lane group 0)
+#pragma unroll
+        for (uint32_t b = 0; b < TM_NBLK; ++b)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_blk[b] & 0xffffu), "n"(TM_BLK));
+    };
     // spilled rate `row` (0 .. NRX) of this thread: shared memory, or tensor memory
     auto put_rate = [&](int row, real r) {
-        if (row < NRT) tm_st(tm_base + RW * (2 * kPull2SmemCoefs + row), r);
+        if (row < NRT) tm_st(tm_at(TM_RATE0 + RW * row), r);
         else Rx[(row - NRT) * T + tid] = r;
     };
 
@@ -348,8 +392,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
                 const int32_t w = p.agg_ent[(size_t)q * TV + v];
                 acc += static_cast<double>(w >> 24) * Rbuf[w & 0xffffff];
             }
-            if (s < kPullCoefs - kPull2SmemCoefs) C[s] = static_cast<real>(acc);
-            else if (TM) tm_st(tm_base + RW * (side * kPull2SmemCoefs + s - (kPullCoefs - kPull2SmemCoefs)), static_cast<real>(acc));
+            if (KT) {  // value positions of a side: pull2_store; side b's K/G chunk pair follows side a's
+                constexpr int pos[kPullCoefs] = {0, 1, 5, 7, 2, 3, 4, 6, 8, 9, 10, 12, 14, 11, 32, 13, 33, 15, 34};
+                tm_st(tm_at(RW * (pos[s] < 32 ? pos[s] + 16 * side : pos[s] + 3 * side)), static_cast<real>(acc));
+            } else if (s < kPullCoefs - kPull2SmemCoefs) C[s] = static_cast<real>(acc);
+            else if (TM) tm_st(tm_at(RW * (side * kPull2SmemCoefs + s - (kPullCoefs - kPull2SmemCoefs))), static_cast<real>(acc));
             else Gs[(s - (kPullCoefs - kPull2SmemCoefs)) * TV + v] = static_cast<real>(acc);
         }
     };
@@ -401,6 +448,9 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
     const double ginv = 1.0 / growth;
     const double q_fixed = ADAPT ? 0.0 : 1.0 / p.dt_fixed;
 
+    // the hub abundance this lane updates in finalize (lane h: hub h), carried beside yh0..2: selecting
+    // it from the three warp-uniform values costs a divergent branch per sub-step
+    real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : (lane == 2 ? yh2 : static_cast<real>(0)));
     while (run) {
         // ---- publish y x {1, hubs}, both species -------------------------------------------
         const real pa1 = ya * yh0, pa2 = ya * yh1, pa3 = ya * yh2;
@@ -418,8 +468,23 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
         real ka, kb, share[6];
         {
             real sb[6], Ga[kPull2SmemCoefs], Gb[kPull2SmemCoefs];
-            if (TM) {
-                tm_load_g(Ga, Gb, tm_base);
+            if (KT) {
+                // five chunks of 8 values: K and most of G of side a, of side b, the three last G of both
+                real Ka[NK], Kb[NK], x[8];
+                tm_load8(x, tm_at(0));
+                Ka[0] = x[0], Ka[1] = x[1], Ka[4] = x[2], Ka[5] = x[3], Ka[6] = x[4], Ka[2] = x[5], Ka[7] = x[6], Ka[3] = x[7];
+                tm_load8(x, tm_at(8 * RW));
+                Ka[8] = x[0], Ka[9] = x[1], Ga[0] = x[2], Ga[3] = x[3], Ga[1] = x[4], Ga[5] = x[5], Ga[2] = x[6], Ga[7] = x[7];
+                tm_load8(x, tm_at(16 * RW));
+                Kb[0] = x[0], Kb[1] = x[1], Kb[4] = x[2], Kb[5] = x[3], Kb[6] = x[4], Kb[2] = x[5], Kb[7] = x[6], Kb[3] = x[7];
+                tm_load8(x, tm_at(24 * RW));
+                Kb[8] = x[0], Kb[9] = x[1], Gb[0] = x[2], Gb[3] = x[3], Gb[1] = x[4], Gb[5] = x[5], Gb[2] = x[6], Gb[7] = x[7];
+                tm_load8(x, tm_at(32 * RW));
+                Ga[4] = x[0], Ga[6] = x[1], Ga[8] = x[2], Gb[4] = x[3], Gb[6] = x[4], Gb[8] = x[5];
+                pull_rate_sums<real>(Ka, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
+                pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+            } else if (TM) {
+                tm_load_g(Ga, Gb, tm_at(0));
             } else {
 #pragma unroll
                 for (int j = 0; j < kPull2SmemCoefs; ++j) {
@@ -427,7 +492,8 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
                     Gb[j] = lds_at<real>(s_G + (j * TV + vb) * SZ);
                 }
             }
-            if (KS) {
+            if (KT) {
+            } else if (KS) {
                 real Ka[NK], Kb[NK];
 #pragma unroll
                 for (int j = 0; j < NK; ++j) {
@@ -442,13 +508,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
             }
 #pragma unroll
             for (int i = 0; i < 6; ++i) share[i] += sb[i];
-        }
-        real inva = 0, invb = 0;  // reciprocal factors of the dt candidates, off the critical path
-        if (ADAPT) {
-            inva = rcp_pos(ya > y_floor ? eps_y * ya : yfl_eps);
-            invb = rcp_pos(yb > y_floor ? eps_y * yb : yfl_eps);
-            if (!plain_a) inva = 0;  // hub owners are judged on their full rows in finalize
-            if (!plain_b) invb = 0;
         }
         __syncthreads();
         // own consumption of a hub owner in a hub-only reaction, read in finalize.  Stored between
@@ -470,10 +529,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
         x3 = lds_at<real>(hi16(w1));                                                       \
         if (4 * (g) < J2 && 4 * (g) < S.wn2) { /* second factors (three-body reactions) */ \
             const uint32_t v0 = S.f2[(2 * (g)) % (J2 / 2)], v1 = S.f2[(2 * (g) + 1) % (J2 / 2)]; \
-            x0 *= lds_at<real>(lo16(v0));                                                  \
-            x1 *= lds_at<real>(hi16(v0));                                                  \
-            x2 *= lds_at<real>(lo16(v1));                                                  \
-            x3 *= lds_at<real>(hi16(v1));                                                  \
+            const real z0 = lds_at<real>(lo16(v0)), z1 = lds_at<real>(hi16(v0));           \
+            const real z2 = lds_at<real>(lo16(v1)), z3 = lds_at<real>(hi16(v1));           \
+            x0 *= z0;                                                                      \
+            x1 *= z1;                                                                      \
+            x2 *= z2;                                                                      \
+            x3 *= z3;                                                                      \
         }                                                                                  \
     }
 #define KINNET_FMAS_A(g)                                                        \
@@ -519,7 +580,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
             // four consecutive spilled rates of this thread, rows row .. row + 3
             auto rates4 = [&](real (&x)[4], int row) {
                 if (row < NRT) {
-                    tm_load4(x, tm_base + RW * (2 * kPull2SmemCoefs + row));
+                    tm_load4(x, tm_at(TM_RATE0 + RW * row));
                 } else {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) x[j] = lds_at<real>(s_Rx + (row - NRT + j) * T * SZ);
@@ -569,7 +630,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
         if (NS > 0) {  // N-slots: k += sum nu R Y_partner, F- of the reactants of heavy + heavy reactions
             auto nrates4 = [&](real (&x)[4], int row) {
                 if (row < NRT) {
-                    tm_load4(x, tm_base + RW * (2 * kPull2SmemCoefs + row));
+                    tm_load4(x, tm_at(TM_RATE0 + RW * row));
                 } else {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) x[j] = lds_at<real>(s_Rx + (row - NRT + j) * T * SZ);
@@ -596,6 +657,13 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
         }
 
         // ---- S5: q candidates of the non-hub species: |F+ - F-| / (eps max(y, floor)) ------
+        real inva = 0, invb = 0;  // reciprocal factors of the dt candidates, off the critical path
+        if (ADAPT) {
+            inva = rcp_pos(ya > y_floor ? eps_y * ya : yfl_eps);
+            invb = rcp_pos(yb > y_floor ? eps_y * yb : yfl_eps);
+            if (!plain_a) inva = 0;  // hub owners are judged on their full rows in finalize
+            if (!plain_b) invb = 0;
+        }
         const real cha = fma(-ka, ya, Fpa), chb = fma(-kb, yb, Fpb);
         if (ADAPT) {
             const real qa = abs_of(cha) * inva, qb = abs_of(chb) * invb;
@@ -605,7 +673,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
         __syncthreads();
 
         // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
-        const real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : yh2);
         real invh = 0;
         double q_rem = 0.0, rem = 0.0;
         if (ADAPT) {  // these depend on nothing the barrier waited for: they run beside the loads
@@ -613,15 +680,17 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
             rem = t_hydro - t;
             q_rem = rcp_pos(rem);
         }
-        real hFp = 0, hFm = 0;
-        if (lane < nbs) {  // three active lanes: one wavefront per load instead of two
+        real hFp, hFm;
+        {   // lanes 0..nbs-1 only (one wavefront per load instead of two); predicated loads, not a
+            // branch: the divergence bookkeeping costs more than the adds the idle lanes then do on zeros
+            const bool act = lane < nbs;
             real vp[NW], vm[NW];
 #pragma unroll
             for (int w = 0; w < NW; ++w) {
-                vp[w] = lds_at<real>(s_red + (w * 8 + lane) * SZ);
-                vm[w] = lds_at<real>(s_red + (w * 8 + 3 + lane) * SZ);
+                vp[w] = lds_if<real>(act, s_red + (w * 8 + lane) * SZ);
+                vm[w] = lds_if<real>(act, s_red + (w * 8 + 3 + lane) * SZ);
             }
-            const real own_term = lds_at<real>(s_own + lane * SZ);
+            const real own_term = lds_if<real>(act, s_own + lane * SZ);
 #pragma unroll
             for (int s = 1; s < NW; s *= 2)  // fixed pairwise order over warps (log depth)
 #pragma unroll
@@ -631,7 +700,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
                 }
             hFp = vp[0];
             hFm = vm[0] + own_term;
-            if (NS > 0) hFp += lds_at<real>(s_ownp + lane * SZ);
+            if (NS > 0) hFp += lds_if<real>(act, s_ownp + lane * SZ);
         }
         if (!ADAPT && rhs_only) {
             real* Fpo = reinterpret_cast<real*>(p.Fplus) + (size_t)z * N;
@@ -650,7 +719,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
             if (TM) {  // give the columns back (every warp is past its last tcgen05.ld)
                 __syncthreads();
                 if (warp == 0)
-                    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base & 0xffffu), "n"(TM_ALLOC));
+                    tm_free();
             }
             return;
         }
@@ -705,6 +774,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
             yh0 = __shfl_sync(0xffffffffu, hn, 0);
             yh1 = __shfl_sync(0xffffffffu, hn, 1);
             yh2 = __shfl_sync(0xffffffffu, hn, 2);
+            yme = hn;
             ya = hub_owner ? hn : yna;  // hub h lives on side a of thread h: warp 0, lane h
             yb = ynb;
         }
@@ -722,8 +792,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || (TM && NS == 0) ? 48
     const int bad = ((A.own >= 0) && !isfinite(static_cast<double>(ya))) ||
                     ((B.own >= 0) && !isfinite(static_cast<double>(yb)));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
-    if (TM && warp == 0)  // every warp is past its last tcgen05.ld: give the columns back
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base & 0xffffu), "n"(TM_ALLOC));
+    if (TM && warp == 0) tm_free();  // every warp is past its last tcgen05.ld: give the columns back
     if (p.energy) {  // uniform; Yg still holds the start-of-call abundances
         double e = 0.0;
         if (A.own >= 0) e = p.bind[A.own] * (static_cast<double>(ya) - static_cast<double>(Yg[A.own]));
@@ -764,14 +833,14 @@ pull_fn pick_pull2_j2(int s2, int ns, bool qss) {
     // networks with N-slots have two-factor P-slots anyway: one second-factor class for them;
     // the QSS variant is instantiated for the larger second-factor class only
     constexpr int SA = CPA - kPull2RegA, CB = kPull2CapB, SB = kPull2SpillB, NS = kPullNSlots;
-    constexpr bool TM = TB >= 96;  // = pull2_uses_tmem(TB)
+    constexpr int S0 = pull2_store(TB, 0), SN = pull2_store(TB, NS);
     if (qss) {
-        if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, true, TM>;
-        return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, true, TM>;
+        if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, true, SN>;
+        return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, true, S0>;
     }
-    if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, false, TM>;
-    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false, TM>;
-    return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false, TM>;
+    if (ns > 0) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, NS, ADAPT, false, SN>;
+    if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false, S0>;
+    return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false, S0>;
 }
 template <typename real, int TB, bool ADAPT>
 pull_fn pick_pull2_cap(int sa, int s2, int ns, bool qss) {
