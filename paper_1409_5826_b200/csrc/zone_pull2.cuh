@@ -23,14 +23,14 @@ constexpr int kPull2SmemCoefs = 9;
 // Where a thread keeps what it re-reads every sub-step (the loop-invariant coefficients):
 //   kStoreSmem    G and the spilled slot rates in shared memory, K in registers (block sizes < 96: up to
 //                 12 CTAs per SM are too many for the tensor-memory columns)
-//   kStoreTmem    G and up to 12 spilled rates in tensor memory, K in registers (168 registers, four
-//                 96-thread CTAs per SM): the instantiations with N-slots, which spill at 128 registers
-//   kStoreTmemKs  the same with K in shared memory (128 registers): 160-thread blocks, three per SM,
-//                 whose two lane groups leave each thread 64 columns
-//   kStoreTmemK   K, G and 8 or 12 spilled rates in tensor memory (128 registers, five 96-thread CTAs per SM)
+//   kStoreTmemK   K, G and 8 or 12 spilled rates in tensor memory: 128 registers, five 96-thread CTAs per
+//                 SM.  With N-slots too (hub150hh: 221k zone-networks/s against 204k with K in 168 registers)
+//   kStoreTmemKs  160-thread blocks, three per SM, whose two lane groups leave each thread 64 columns:
+//                 G and 12 rates in tensor memory, K in shared memory (128 registers)
+//   kStoreTmem    ... and with N-slots K in registers (168 registers; the 128-register build spills)
 enum Pull2Store { kStoreSmem = 0, kStoreTmem = 1, kStoreTmemKs = 2, kStoreTmemK = 3 };
 __host__ __device__ constexpr int pull2_store(int TB, int nslots) {
-    return TB < 96 ? kStoreSmem : nslots > 0 ? kStoreTmem : TB == 160 ? kStoreTmemKs : kStoreTmemK;
+    return TB < 96 ? kStoreSmem : TB == 160 ? (nslots > 0 ? kStoreTmem : kStoreTmemKs) : kStoreTmemK;
 }
 // Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) as a LANE-PRIVATE store: tcgen05.ld
 // reaches a warp's own 32 lanes in ~12 cycles and does not touch the shared-memory pipe, which is this
