@@ -23,8 +23,8 @@ constexpr int kPull2SmemCoefs = 9;
 // Where a thread keeps what it re-reads every sub-step (the loop-invariant coefficients):
 //   kStoreSmem    G and the spilled slot rates in shared memory, K in registers (block sizes < 96: up to
 //                 12 CTAs per SM are too many for the tensor-memory columns)
-//   kStoreTmemK   K, G and 8 or 12 spilled rates in tensor memory: 128 registers, five 96-thread CTAs per
-//                 SM.  With N-slots too (hub150hh: 221k zone-networks/s against 204k with K in 168 registers)
+//   kStoreTmemK   K, G and up to 12 spilled rates in tensor memory (128 columns per lane group): no
+//                 coefficient in shared memory, none in registers beyond 20 slot rates.  With N-slots too
 //   kStoreTmemKs  160-thread blocks, three per SM, whose two lane groups leave each thread 64 columns:
 //                 G and 12 rates in tensor memory, K in shared memory (128 registers)
 //   kStoreTmem    ... and with N-slots K in registers (168 registers; the 128-register build spills)
@@ -33,18 +33,19 @@ __host__ __device__ constexpr int pull2_store(int TB, int nslots) {
     return TB < 96 ? kStoreSmem : TB == 160 ? (nslots > 0 ? kStoreTmem : kStoreTmemKs) : kStoreTmemK;
 }
 // Tensor memory (TMEM, 512 columns x 128 lanes x 32 bit per SM) as a LANE-PRIVATE store: tcgen05.ld
-// reaches a warp's own 32 lanes in ~12 cycles and does not touch the shared-memory pipe, which is this
+// reaches a warp's own 32 lanes in ~12 cycles and does not touch the shared-memory pipe, which was this
 // kernel's busiest unit (measured: a saturated LDS stream loses nothing to a concurrent tcgen05.ld
-// stream).  Layout of a thread's columns under kStoreTmemK, in values of `real` (chunks of 8 values, one
-// tcgen05.ld each, so that a 96-thread CTA can hold its 96 columns as three 32-column allocations --
-// 5 x 96 <= 512 where the power-of-two 128 would allow four CTAs only):
+// stream).  Layout of a thread's columns under kStoreTmemK, in values of `real`, chunks of 8 values = one
+// tcgen05.ld each, ordered so that every chunk completes sub-expressions of the rate sums:
 //   [ 0.. 8)  K of side a: C0 C1 C4 C5 C6 C2 C7 C3     [ 8..16)  C8 C9, then G0 G3 G1 G5 G2 G7 of side a
 //   [16..32)  the same of side b                      [32..38)  G4 G6 G8 of side a, of side b; [38..40) unused
 //   [40..)    spilled slot rates
+// The first two chunks of the NEXT sub-step are issued right after barrier B and land during the finalize.
 constexpr int kPull2TmemRateBase = 40;
 // spilled slot rates per thread that tensor memory takes (the rest stay in shared memory)
 __host__ __device__ constexpr int pull2_tmem_rates(int store, int TB, int real_bytes, int spill) {
-    const int cap = store == kStoreSmem ? 0 : (store == kStoreTmemK && TB == 96 && real_bytes == 8) ? 8 : 12;
+    (void)TB, (void)real_bytes;
+    const int cap = store == kStoreSmem ? 0 : 12;
     return spill < cap ? spill : cap;
 }
 // columns per thread (32-bit words), and what one CTA allocates
@@ -54,7 +55,6 @@ __host__ __device__ constexpr int pull2_tmem_words(int store, int TB, int real_b
 }
 __host__ __device__ constexpr int pull2_tmem_cols(int store, int TB, int real_bytes, int spill) {
     const int need = pull2_tmem_words(store, TB, real_bytes, spill) * ((TB / 32 + 3) / 4);
-    if (need > 64 && need <= 96) return 96;  // three allocations of 32
     int cols = 32;
     while (cols < need) cols *= 2;
     return cols;
@@ -165,6 +165,19 @@ __device__ __forceinline__ void tm_load4(float (&x)[4], uint32_t a) {
 #pragma unroll
     for (int j = 0; j < 4; ++j) x[j] = __uint_as_float(u[j]);
 }
+// eight values whose tcgen05.ld was issued earlier into u, v (the sub-step's first two chunks)
+__device__ __forceinline__ void tm_take8x2(double (&x)[8], double (&y)[8], uint32_t (&u)[16], uint32_t (&v)[16]) {
+    tm_wait(u);
+    tm_touch(v);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = tm_val(u[2 * j], u[2 * j + 1]), y[j] = tm_val(v[2 * j], v[2 * j + 1]);
+}
+__device__ __forceinline__ void tm_take8x2(float (&x)[8], float (&y)[8], uint32_t (&u)[8], uint32_t (&v)[8]) {
+    tm_wait(u);
+    tm_touch(v);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) x[j] = __uint_as_float(u[j]), y[j] = __uint_as_float(v[j]);
+}
 // eight consecutive values
 __device__ __forceinline__ void tm_load8(double (&x)[8], uint32_t a) {
     uint32_t u[16];
@@ -227,9 +240,13 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 }
 
 // Twelve warps per SM -- three per scheduler, whose 16 K registers then give each thread
-// 168 (ptxas derives exactly that from the launch bounds): four 96-thread CTAs, two
-// 192-thread ones.  With fp32 state the rates take half the registers: 128 registers, four
-// warps per scheduler, five 96-thread CTAs (270k -> 300k zone-networks/s on configs[3]).
+// 168 (ptxas derives exactly that from the launch bounds): four 96-thread CTAs, three 128-thread,
+// two 192-thread ones.  Five 96-thread CTAs at 128 registers run as fast on a full batch (252k
+// zone-networks/s on configs[3] either way, profiles/r02b), but the 168-register build does not spill, and
+// its sub-step is 17 % shorter in a lone CTA (0.72 us against 0.87 us): every batch that does not fill
+// the SMs gains.  160-thread blocks, whose K stays in shared memory, run three CTAs at 128 registers.
+// With fp32 state the rates take half the registers: 128 registers, four warps per scheduler, five
+// 96-thread CTAs (318k zone-networks/s on configs[3]).
 // NS = 4 compiles the N-slots in (networks with heavy + heavy reactions, schedule.h): four more
 // gathers per side into k, skipped by the warps none of whose species has one, and the hub
 // owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
@@ -237,7 +254,7 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 // run-time switch costs the default kernel 6 % (registers), so it is an instantiation.
 // ST: where the coefficients live (Pull2Store; = pull2_store(TB, NS)).
 template <typename real, int TB, int CPA, int SPA, int CPB, int SPB, int J2, int NS, bool ADAPT, bool QSS, int ST>
-__global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ? 480 : 384) / TB)
+__global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ? 480 : 384) / TB)
     zone_kernel_pull2(const KPull p) {
     static_assert(ST == pull2_store(TB, NS), "store mode");
     constexpr bool TM = ST != kStoreSmem;   // tensor memory in use
@@ -266,13 +283,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
     real* Ks = Gs;                                            // [NK][TV] K of every virtual thread          (KS)
     double* Rbuf = reinterpret_cast<double*>(Gs + (TM ? (KS ? NK * TV : 0) : kPull2SmemCoefs * TV));  // [M] rates, set-up only
     // tensor-memory columns of a thread (TM): G of side a, G of side b, then the NRT rates; KT: see
-    // pull2_store.  TM_BLK: columns per allocation (a 96-column CTA holds three of 32)
+    // pull2_store
     constexpr uint32_t RW = sizeof(real) / 4, TMC = pull2_tmem_words(ST, TB, sizeof(real), NRX);
-    constexpr uint32_t TM_COLS = pull2_tmem_cols(ST, TB, sizeof(real), NRX);
-    constexpr uint32_t TM_NBLK = TM_COLS == 96 ? 3 : 1, TM_BLK = TM_COLS / TM_NBLK;
+    constexpr uint32_t TM_COLS = pull2_tmem_cols(ST, TB, sizeof(real), NRX);  // what the CTA allocates
     constexpr uint32_t TM_RATE0 = RW * (KT ? kPull2TmemRateBase : 2 * kPull2SmemCoefs);  // first rate column
-    static_assert(TM_NBLK == 1 || NW <= 4, "split allocations: one lane group");
-    __shared__ uint32_t tm_slot[3];
+    __shared__ uint32_t tm_slot;
     uint32_t s_redq;
     asm volatile("mov.u32 %0, %1;"
                  : "=r"(s_redq)
@@ -284,13 +299,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
     const uint32_t s_ownp = s_redq + 20 * 8;  // [3] their own P-slot sums (NS > 0)
     const uint32_t s_G = s_YP + (4 * TV + 4 + (NRX - NRT) * T) * SZ;
     if (s_YP + (4 * TV + 4) * SZ > 0xffffu) __trap();  // the packed gather addresses are 16-bit
-    if (TM && warp == 0) {  // one warp allocates this CTA's columns; the addresses arrive through shared memory
-#pragma unroll
-        for (uint32_t b = 0; b < TM_NBLK; ++b)
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
-                             static_cast<uint32_t>(__cvta_generic_to_shared(&tm_slot[b]))),
-                         "n"(TM_BLK)
-                         : "memory");
+    if (TM && warp == 0) {  // one warp allocates this CTA's columns; the address arrives through shared memory
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         static_cast<uint32_t>(__cvta_generic_to_shared(&tm_slot))),
+                     "n"(TM_COLS)
+                     : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
 
@@ -339,20 +352,16 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
     if (tid < 4) YP[4 * TV + tid] = static_cast<real>(1);
     if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    uint32_t tm_blk[TM_NBLK] = {};  // this thread's lane quarter and first column, per allocation
+    uint32_t tm_base = 0;  // this thread's lane quarter and first column
     if (TM) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-        for (uint32_t b = 0; b < TM_NBLK; ++b)
-            tm_blk[b] = *reinterpret_cast<volatile uint32_t*>(&tm_slot[b]) + (static_cast<uint32_t>(warp & 3) << 21) +
-                        static_cast<uint32_t>(warp >> 2) * TMC;
+        tm_base = *reinterpret_cast<volatile uint32_t*>(&tm_slot) + (static_cast<uint32_t>(warp & 3) << 21) +
+                  static_cast<uint32_t>(warp >> 2) * TMC;
     }
-    // tensor-memory address of this thread's column c (compile-time c; no access straddles allocations)
-    auto tm_at = [&](uint32_t c) -> uint32_t { return tm_blk[TM_NBLK == 1 ? 0 : c / TM_BLK] + (TM_NBLK == 1 ? c : c % TM_BLK); };
+    // tensor-memory address of this thread's column c
+    auto tm_at = [&](uint32_t c) -> uint32_t { return tm_base + c; };
     auto tm_free = [&]() {  // by the allocating warp (warp 0: lane quarter 0, lane group 0)
-#pragma unroll
-        for (uint32_t b = 0; b < TM_NBLK; ++b)
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_blk[b] & 0xffffu), "n"(TM_BLK));
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base & 0xffffu), "n"(TM_COLS));
     };
     // spilled rate `row` (0 .. NRX) of this thread: shared memory, or tensor memory
     auto put_rate = [&](int row, real r) {
@@ -451,6 +460,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
     // the hub abundance this lane updates in finalize (lane h: hub h), carried beside yh0..2: selecting
     // it from the three warp-uniform values costs a divergent branch per sub-step
     real yme = lane == 0 ? yh0 : (lane == 1 ? yh1 : (lane == 2 ? yh2 : static_cast<real>(0)));
+    uint32_t pf0[8 * RW], pf1[8 * RW];  // K and most of G of side a, read ahead (KT)
+    if (KT) {
+        tm_ld(pf0, tm_at(0));
+        tm_ld(pf1, tm_at(8 * RW));
+    }
     while (run) {
         // ---- publish y x {1, hubs}, both species -------------------------------------------
         const real pa1 = ya * yh0, pa2 = ya * yh1, pa3 = ya * yh2;
@@ -470,10 +484,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
             real sb[6], Ga[kPull2SmemCoefs], Gb[kPull2SmemCoefs];
             if (KT) {
                 // five chunks of 8 values: K and most of G of side a, of side b, the three last G of both
-                real Ka[NK], Kb[NK], x[8];
-                tm_load8(x, tm_at(0));
+                // (the first two were issued after the last barrier B, or before the loop)
+                real Ka[NK], Kb[NK], x[8], x1[8];
+                tm_take8x2(x, x1, pf0, pf1);
                 Ka[0] = x[0], Ka[1] = x[1], Ka[4] = x[2], Ka[5] = x[3], Ka[6] = x[4], Ka[2] = x[5], Ka[7] = x[6], Ka[3] = x[7];
-                tm_load8(x, tm_at(8 * RW));
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = x1[j];
                 Ka[8] = x[0], Ka[9] = x[1], Ga[0] = x[2], Ga[3] = x[3], Ga[1] = x[4], Ga[5] = x[5], Ga[2] = x[6], Ga[7] = x[7];
                 tm_load8(x, tm_at(16 * RW));
                 Kb[0] = x[0], Kb[1] = x[1], Kb[4] = x[2], Kb[5] = x[3], Kb[6] = x[4], Kb[2] = x[5], Kb[7] = x[6], Kb[3] = x[7];
@@ -671,6 +687,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
             if (lane == 0) sts(s_redq + warp * 8, c);
         }
         __syncthreads();
+        if (KT) {  // the next sub-step's first two coefficient chunks: in flight during the finalize
+            tm_ld(pf0, tm_at(0));
+            tm_ld(pf1, tm_at(8 * RW));
+        }
 
         // ---- finalize (every warp redundantly): hub rows over warps, zone-wide dt -----------
         real invh = 0;
@@ -717,6 +737,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
                 Fmo[B.own] = kb * yb;
             }
             if (TM) {  // give the columns back (every warp is past its last tcgen05.ld)
+                if (KT) {
+                    tm_wait(pf0);
+                    tm_touch(pf1);
+                }
                 __syncthreads();
                 if (warp == 0)
                     tm_free();
@@ -789,6 +813,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST >= kStoreTmemKs ?
     if (ADAPT && steps > 0) dt_out = 1.0 / q_prev;
 
     // ---- S6: zone state out ------------------------------------------------------------------
+    if (KT) {  // the read-ahead of a sub-step that never came: land it before the barrier below
+        tm_wait(pf0);
+        tm_touch(pf1);
+    }
     const int bad = ((A.own >= 0) && !isfinite(static_cast<double>(ya))) ||
                     ((B.own >= 0) && !isfinite(static_cast<double>(yb)));
     if (__syncthreads_or(bad)) status |= NET_STATUS_NONFINITE;
