@@ -478,6 +478,10 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sts(A.s_pub + 3 * TV * SZ, pa3);
         sts(B.s_pub + 3 * TV * SZ, pb3);
 
+        // barrier A, right behind the publishes: what follows up to barrier B (rate sums, gathers, butterfly)
+        // needs no further hand-shake, so the warps' skews over it add up once, at B, instead of being
+        // waited out twice
+        __syncthreads();
         // ---- rate sums: k = F-/y (Eq. (1)) and the hub-row shares, added over the two ----------
         real ka, kb, share[6];
         {
@@ -525,7 +529,6 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
 #pragma unroll
             for (int i = 0; i < 6; ++i) share[i] += sb[i];
         }
-        __syncthreads();
         // own consumption of a hub owner in a hub-only reaction, read in finalize.  Stored between
         // the barriers: B orders it before this step's reads, the next A orders those reads
         // before the next store.
