@@ -533,6 +533,36 @@ def test_one_net_two_streams(hub150):
         assert torch.equal(got, ref)
 
 
+def test_tensor_memory_kernels_share_the_sms():
+    """Three zone kernels with different tensor-memory footprints (fp64 hub150: 128 columns per CTA,
+    fp32 hub150: 64, fp64 hub365: 256) on three streams at once, each batch large enough to fill the
+    GPU on its own: every CTA allocates its columns once and holds them to its end, so a CTA that finds
+    the SM's 512 columns taken waits for another to finish -- nothing can deadlock, and every result is
+    bit for bit the one of the same call running alone."""
+    jobs = []
+    for prec, z, cfg in ((64, 2048, 4), (32, 2048, 4), (64, 1024, 5)):
+        c = build_config(cfg, zones=z)
+        kn = K.Net(c["network"], K.NetParams(precision=prec))
+        ydt = torch.float64 if prec == 64 else torch.float32
+
+        def state(c=c, z=z, ydt=ydt):
+            return (dev(c["T9"]), dev(c["rho"]), dev(c["Y0"], ydt), torch.zeros(z, dtype=torch.float64, device=DEV),
+                    torch.zeros(z, dtype=torch.int32, device=DEV), torch.zeros(z, dtype=torch.int32, device=DEV))
+
+        st = state()
+        kn.net_integrate(z, *st[:3], c["t_hydro"], *st[3:])  # alone
+        torch.cuda.synchronize()
+        jobs.append((kn, z, c["t_hydro"], [t.clone() for t in st[2:]], state(), torch.cuda.Stream()))
+    torch.cuda.synchronize()
+    for kn, z, th, _, st, stream in jobs:  # together
+        kn.net_integrate(z, *st[:3], th, *st[3:], stream)
+    torch.cuda.synchronize()
+    for kn, z, th, want, st, _ in jobs:
+        assert int(st[5].max()) == 0
+        for got, ref in zip(st[2:], want):
+            assert torch.equal(got, ref)
+
+
 def test_net_reserve_and_oversized_batches(g16):
     """More zones than the launch-order lanes hold (65536 after net_create): the call runs in
     caller order and returns the same bits as after net_reserve (sorted)."""
