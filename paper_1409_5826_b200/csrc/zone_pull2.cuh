@@ -259,6 +259,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
     static_assert(ST == pull2_store(TB, NS), "store mode");
     constexpr bool TM = ST != kStoreSmem;   // tensor memory in use
     constexpr bool KT = ST == kStoreTmemK;  // ... for K too
+    constexpr bool BRF = TB <= 128;         // branch-free gathers (see KINNET_LOADS)
     static_assert(CPA % 4 == 0 && CPB % 4 == 0 && SPA % 4 == 0 && SPA < CPA && SPB % 4 == 0 && SPB < CPB,
                   "slot capacities");
     static_assert(NS == 0 || NS == kPullNSlots, "N-slot capacity");
@@ -539,14 +540,22 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         {
             real sa0, sa1, sa2, sa3, a0, a1, a2, a3;
             real sb0 = 0, sb1 = 0, sb2 = 0, sb3 = 0, b0, b1, b2, b3;
+// BRF: no branch inside the gathers.  Every group of four slots up to the instantiation's capacity is
+// live in every warp; the groups a warp does not use (warp-uniform trip counts wn, wn2) hold rate 0 and the
+// address of the constant 1 (one broadcast wavefront), so they add exact zeros.  Branching around them costs
+// far more than their issue slots: it cuts the sub-step into basic blocks that ptxas cannot schedule across
+// (hub150: 486 -> 448 instructions in the loop although all 20 + 12 slots of every warp are live, 255k ->
+// 265k zone-networks/s on configs[3], a lone CTA 0.72 -> 0.53 us per sub-step).  With five or six warps the
+// padding outweighs it (hub365, caps 24 + 12 against 16 + 12 in four of its six warps: 4.94 -> 5.22 ns per
+// zone-substep), so those block sizes keep the branches.
 #define KINNET_LOADS(S, CP_, g, x0, x1, x2, x3)                                            \
-    if ((4 * (g) < CP_) && ((g) == 0 || 4 * (g) < S.wn)) {                                 \
+    if ((4 * (g) < CP_) && ((g) == 0 || (BRF || 4 * (g) < S.wn))) {                                 \
         const uint32_t w0 = S.f1[(2 * (g)) % (CP_ / 2)], w1 = S.f1[(2 * (g) + 1) % (CP_ / 2)]; \
         x0 = lds_at<real>(lo16(w0));                                                       \
         x1 = lds_at<real>(hi16(w0));                                                       \
         x2 = lds_at<real>(lo16(w1));                                                       \
         x3 = lds_at<real>(hi16(w1));                                                       \
-        if (4 * (g) < J2 && 4 * (g) < S.wn2) { /* second factors (three-body reactions) */ \
+        if (4 * (g) < J2 && (BRF || 4 * (g) < S.wn2)) { /* second factors (three-body reactions) */ \
             const uint32_t v0 = S.f2[(2 * (g)) % (J2 / 2)], v1 = S.f2[(2 * (g) + 1) % (J2 / 2)]; \
             const real z0 = lds_at<real>(lo16(v0)), z1 = lds_at<real>(hi16(v0));           \
             const real z2 = lds_at<real>(lo16(v1)), z3 = lds_at<real>(hi16(v1));           \
@@ -562,12 +571,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sa1 = A.R[1] * a1;                                                      \
         sa2 = A.R[2] * a2;                                                      \
         sa3 = A.R[3] * a3;                                                      \
-    } else if (4 * (g) < CPRA && 4 * (g) < A.wn) {                              \
+    } else if (4 * (g) < CPRA && (BRF || 4 * (g) < A.wn)) {                              \
         sa0 = fma(A.R[(4 * (g)) % CPRA], a0, sa0);                              \
         sa1 = fma(A.R[(4 * (g) + 1) % CPRA], a1, sa1);                          \
         sa2 = fma(A.R[(4 * (g) + 2) % CPRA], a2, sa2);                          \
         sa3 = fma(A.R[(4 * (g) + 3) % CPRA], a3, sa3);                          \
-    } else if (4 * (g) < CPA && 4 * (g) < A.wn) {                               \
+    } else if (4 * (g) < CPA && (BRF || 4 * (g) < A.wn)) {                               \
         real xr[4];                                                             \
         rates4(xr, (4 * (g) >= CPRA ? 4 * (g) - CPRA : 0));                     \
         sa0 = fma(xr[0], a0, sa0);                                              \
@@ -576,12 +585,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sa3 = fma(xr[3], a3, sa3);                                              \
     }
 #define KINNET_FMAS_B(g)                                                        \
-    if (4 * (g) < CPRB && ((g) == 0 || 4 * (g) < B.wn)) {                       \
+    if (4 * (g) < CPRB && ((g) == 0 || (BRF || 4 * (g) < B.wn))) {                       \
         sb0 = fma(B.R[(4 * (g)) % CPRB], b0, sb0);                              \
         sb1 = fma(B.R[(4 * (g) + 1) % CPRB], b1, sb1);                          \
         sb2 = fma(B.R[(4 * (g) + 2) % CPRB], b2, sb2);                          \
         sb3 = fma(B.R[(4 * (g) + 3) % CPRB], b3, sb3);                          \
-    } else if (4 * (g) < CPB && 4 * (g) < B.wn) {                               \
+    } else if (4 * (g) < CPB && (BRF || 4 * (g) < B.wn)) {                               \
         real xr[4];                                                             \
         rates4(xr, SPA + (4 * (g) >= CPRB ? 4 * (g) - CPRB : 0));               \
         sb0 = fma(xr[0], b0, sb0);                                              \
