@@ -19,6 +19,18 @@ bool pull2_supported(const PullSchedule& P, int* spill) {
     if (spill) *spill = pull2_cap_a(sa) - kPull2RegA + kPull2SpillB + (P.nslots > 0 ? 2 * kPullNSlots : 0);
     return true;
 }
+
+bool pull2_stair_fits(const PullSchedule& P) {
+    int sa, sb, s2;
+    if (!pull2_sides(P, sa, sb, s2) || P.T / 64 < 2) return false;
+    const int nw = P.T / 64, cap_a = pull2_cap_a(sa);
+    for (int t = 0; t < P.T; ++t) {
+        const int vw = t / 32;
+        const int cap = vw < nw ? pull2_stair_a(cap_a, vw) : pull2_stair_b(kPull2CapB, nw, 2 * nw - 1 - vw);
+        if (P.n_slots[t] > cap) return false;
+    }
+    return true;
+}
 #endif
 
 }  // namespace kinnet

@@ -73,6 +73,7 @@ struct KPull {
     double kappa, eps_y, y_floor, growth;
     int n_fixed, max_steps;
     int method;               // 0 = asymptotic / Euler, 1 = QSS variant (net_params_t.method)
+    int stair;                // two-species kernel: the schedule fits the staircase of live slots (zone_pull2.cuh)
 };
 
 

@@ -11,6 +11,8 @@
 // shares of the two are added before ONE butterfly, and the redundant finalize runs
 // in NW = TB/32 warps instead of twice as many.
 #pragma once
+#include <type_traits>
+
 #include "zone_pull.cuh"
 
 namespace kinnet {
@@ -72,6 +74,17 @@ __host__ __device__ inline size_t pull2_smem_bytes(int TB, int M, int spill, int
            sizeof(double) * static_cast<size_t>(M);
 }
 
+// Staircase of live slots (branch-free block sizes): species are dealt to the virtual threads by falling
+// in-degree, so warp w's side a (virtual warp w) needs fewer slots the larger w, its side b (virtual warp
+// 2 NW - 1 - w) more.  When the compiled schedule fits under
+//   side a: max(cap_a - 4 w, 12)        side b: max(cap_b - 4 (NW - 1 - w), 4)
+// (hub150: 20 + 4, 16 + 8, 12 + 12 live slots in its three warps, against 20 + 12 in every warp), each warp
+// runs its own copy of the sub-step loop with those compile-time capacities (KPull.stair).
+__host__ __device__ constexpr int pull2_stair_a(int cap_a, int w) { return cap_a - 4 * w > 12 ? cap_a - 4 * w : 12; }
+__host__ __device__ constexpr int pull2_stair_b(int cap_b, int nw, int w) {
+    return cap_b - 4 * (nw - 1 - w) > 4 ? cap_b - 4 * (nw - 1 - w) : 4;
+}
+bool pull2_stair_fits(const PullSchedule& P);
 // method = net_params_t.method (1 = the QSS instantiations)
 pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P, int method);
 pull_fn pull2_kernel_f64_fixed(const PullSchedule& P, int method);
@@ -237,6 +250,15 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
     share[3] = p1 * m0;
     share[4] = p2 * m1;
     share[5] = p3 * m2;
+}
+
+// warp w runs f with its step of the staircase as compile-time capacities
+template <int NW, int CPA, int CPB, int W = 0, typename F>
+__device__ __forceinline__ bool stair_dispatch(int warp, F& f) {
+    if constexpr (W + 1 < NW) {
+        if (warp != W) return stair_dispatch<NW, CPA, CPB, W + 1>(warp, f);
+    }
+    return f(std::integral_constant<int, pull2_stair_a(CPA, W)>{}, std::integral_constant<int, pull2_stair_b(CPB, NW, W)>{});
 }
 
 // Twelve warps per SM -- three per scheduler, whose 16 K registers then give each thread
@@ -466,6 +488,11 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         tm_ld(pf0, tm_at(0));
         tm_ld(pf1, tm_at(8 * RW));
     }
+    // The sub-step loop, compiled for CAW / CBW live slots on side a / b of the calling warp (the
+    // instantiation's capacities, or this warp's step of the staircase).  Returns true when the kernel is done
+    // (mode kRhs).
+    auto substeps = [&](auto caw_, auto cbw_) -> bool {
+    constexpr int CAW = decltype(caw_)::value, CBW = decltype(cbw_)::value;
     while (run) {
         // ---- publish y x {1, hubs}, both species -------------------------------------------
         const real pa1 = ya * yh0, pa2 = ya * yh1, pa3 = ya * yh2;
@@ -548,8 +575,8 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
 // 265k zone-networks/s on configs[3], a lone CTA 0.72 -> 0.53 us per sub-step).  With five or six warps the
 // padding outweighs it (hub365, caps 24 + 12 against 16 + 12 in four of its six warps: 4.94 -> 5.22 ns per
 // zone-substep), so those block sizes keep the branches.
-#define KINNET_LOADS(S, CP_, g, x0, x1, x2, x3)                                            \
-    if ((4 * (g) < CP_) && ((g) == 0 || (BRF || 4 * (g) < S.wn))) {                                 \
+#define KINNET_LOADS(S, CP_, CW_, g, x0, x1, x2, x3)                                            \
+    if ((4 * (g) < CW_) && ((g) == 0 || (BRF || 4 * (g) < S.wn))) {                                 \
         const uint32_t w0 = S.f1[(2 * (g)) % (CP_ / 2)], w1 = S.f1[(2 * (g) + 1) % (CP_ / 2)]; \
         x0 = lds_at<real>(lo16(w0));                                                       \
         x1 = lds_at<real>(hi16(w0));                                                       \
@@ -571,12 +598,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sa1 = A.R[1] * a1;                                                      \
         sa2 = A.R[2] * a2;                                                      \
         sa3 = A.R[3] * a3;                                                      \
-    } else if (4 * (g) < CPRA && (BRF || 4 * (g) < A.wn)) {                              \
+    } else if (4 * (g) < CPRA && 4 * (g) < CAW && (BRF || 4 * (g) < A.wn)) {                              \
         sa0 = fma(A.R[(4 * (g)) % CPRA], a0, sa0);                              \
         sa1 = fma(A.R[(4 * (g) + 1) % CPRA], a1, sa1);                          \
         sa2 = fma(A.R[(4 * (g) + 2) % CPRA], a2, sa2);                          \
         sa3 = fma(A.R[(4 * (g) + 3) % CPRA], a3, sa3);                          \
-    } else if (4 * (g) < CPA && (BRF || 4 * (g) < A.wn)) {                               \
+    } else if (4 * (g) < CAW && (BRF || 4 * (g) < A.wn)) {                               \
         real xr[4];                                                             \
         rates4(xr, (4 * (g) >= CPRA ? 4 * (g) - CPRA : 0));                     \
         sa0 = fma(xr[0], a0, sa0);                                              \
@@ -585,12 +612,12 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sa3 = fma(xr[3], a3, sa3);                                              \
     }
 #define KINNET_FMAS_B(g)                                                        \
-    if (4 * (g) < CPRB && ((g) == 0 || (BRF || 4 * (g) < B.wn))) {                       \
+    if (4 * (g) < CPRB && 4 * (g) < CBW && ((g) == 0 || (BRF || 4 * (g) < B.wn))) {                       \
         sb0 = fma(B.R[(4 * (g)) % CPRB], b0, sb0);                              \
         sb1 = fma(B.R[(4 * (g) + 1) % CPRB], b1, sb1);                          \
         sb2 = fma(B.R[(4 * (g) + 2) % CPRB], b2, sb2);                          \
         sb3 = fma(B.R[(4 * (g) + 3) % CPRB], b3, sb3);                          \
-    } else if (4 * (g) < CPB && (BRF || 4 * (g) < B.wn)) {                               \
+    } else if (4 * (g) < CBW && (BRF || 4 * (g) < B.wn)) {                               \
         real xr[4];                                                             \
         rates4(xr, SPA + (4 * (g) >= CPRB ? 4 * (g) - CPRB : 0));               \
         sb0 = fma(xr[0], b0, sb0);                                              \
@@ -599,8 +626,8 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         sb3 = fma(xr[3], b3, sb3);                                              \
     }
 #define KINNET_STAGE(g)                               \
-    KINNET_LOADS(A, CPA, g, a0, a1, a2, a3)           \
-    KINNET_LOADS(B, CPB, g, b0, b1, b2, b3)
+    KINNET_LOADS(A, CPA, CAW, g, a0, a1, a2, a3)      \
+    KINNET_LOADS(B, CPB, CBW, g, b0, b1, b2, b3)
 #define KINNET_FMAS(g) \
     KINNET_FMAS_A(g)   \
     KINNET_FMAS_B(g)
@@ -757,7 +784,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
                 if (warp == 0)
                     tm_free();
             }
-            return;
+            return true;
         }
 
         double q, hd;
@@ -821,6 +848,17 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
             status |= NET_STATUS_MAX_STEPS;
             run = false;
         }
+    }
+    return false;
+    };
+    {
+        bool done;
+        if (BRF && NW > 1 && p.stair) {  // warp-uniform
+            done = stair_dispatch<NW, CPA, CPB>(warp, substeps);
+        } else {
+            done = substeps(std::integral_constant<int, CPA>{}, std::integral_constant<int, CPB>{});
+        }
+        if (done) return;
     }
     if (ADAPT && steps > 0) dt_out = 1.0 / q_prev;
 
