@@ -428,7 +428,7 @@ struct net {
     bool has_device = false;
     bool force_generic = false;  // params.kernel == 1: keep the table-driven kernel (A/B tests)
     bool pull2 = false;          // PS is compiled for virtual threads: two species per thread
-    bool pull2_stair = false;    // its schedule fits the staircase of live slots (zone_pull2.cuh)
+    int pull2_stair = 0;         // its schedule's staircase class (zone_pull2.cuh: pull2_stair_class)
     int pull2_spill = 0;         // side-a slot rates kept in shared memory by that kernel
     int device = -1;
     int zones_per_sm = 0;
@@ -621,7 +621,7 @@ void fill_pull(const net* n, KPull& k) {
     k.slot_rxn = n->D.p_slot_rxn;
     k.f1_pack = n->D.p_f1;
     k.f2_pack = n->D.p_f2;
-    k.stair = n->pull2 && n->pull2_stair ? 1 : 0;
+    k.stair = n->pull2 ? n->pull2_stair : 0;
     k.agg_ptr = n->D.p_agg_ptr;
     k.agg_ent = n->D.p_agg_ent;
     k.kappa = n->P.kappa; k.eps_y = n->P.eps_y; k.y_floor = n->P.y_floor;
@@ -785,7 +785,7 @@ int create_common(net_t** out, int N, const int* A, int M, const int* n_react, c
             n->PS = P2;
             n->pull2 = true;
             n->pull2_spill = spill;
-            n->pull2_stair = kinnet::pull2_stair_fits(P2);
+            n->pull2_stair = kinnet::pull2_stair_class(P2);
         }
     }
     if (n->PS.ok && n->PS.nslots > 0 && !n->pull2) {

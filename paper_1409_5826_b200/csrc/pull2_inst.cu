@@ -20,16 +20,18 @@ bool pull2_supported(const PullSchedule& P, int* spill) {
     return true;
 }
 
-bool pull2_stair_fits(const PullSchedule& P) {
+int pull2_stair_class(const PullSchedule& P) {
     int sa, sb, s2;
-    if (!pull2_sides(P, sa, sb, s2) || P.T / 64 < 2) return false;
+    if (!pull2_sides(P, sa, sb, s2) || P.T / 64 < 2) return 0;
     const int nw = P.T / 64, cap_a = pull2_cap_a(sa);
+    bool b0_empty = true;
     for (int t = 0; t < P.T; ++t) {
         const int vw = t / 32;
         const int cap = vw < nw ? pull2_stair_a(cap_a, vw) : pull2_stair_b(kPull2CapB, nw, 2 * nw - 1 - vw);
-        if (P.n_slots[t] > cap) return false;
+        if (P.n_slots[t] > cap) return 0;
+        if (vw == 2 * nw - 1 && P.owner[t] >= 0) b0_empty = false;
     }
-    return true;
+    return b0_empty ? 2 : 1;
 }
 #endif
 

@@ -84,7 +84,9 @@ __host__ __device__ constexpr int pull2_stair_a(int cap_a, int w) { return cap_a
 __host__ __device__ constexpr int pull2_stair_b(int cap_b, int nw, int w) {
     return cap_b - 4 * (nw - 1 - w) > 4 ? cap_b - 4 * (nw - 1 - w) : 4;
 }
-bool pull2_stair_fits(const PullSchedule& P);
+// KPull.stair: 0 = no fit, 1 = fits, 2 = fits and warp 0 plays no species on side b (N <= 32 (2 NW - 1)):
+// its copy of the loop then has none of that side's work (capacity 0)
+int pull2_stair_class(const PullSchedule& P);
 // method = net_params_t.method (1 = the QSS instantiations)
 pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P, int method);
 pull_fn pull2_kernel_f64_fixed(const PullSchedule& P, int method);
@@ -254,9 +256,12 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 
 // warp w runs f with its step of the staircase as compile-time capacities
 template <int NW, int CPA, int CPB, int W = 0, typename F>
-__device__ __forceinline__ bool stair_dispatch(int warp, F& f) {
+__device__ __forceinline__ bool stair_dispatch(int warp, bool b0_empty, F& f) {
     if constexpr (W + 1 < NW) {
-        if (warp != W) return stair_dispatch<NW, CPA, CPB, W + 1>(warp, f);
+        if (warp != W) return stair_dispatch<NW, CPA, CPB, W + 1>(warp, b0_empty, f);
+    }
+    if constexpr (W == 0) {
+        if (b0_empty) return f(std::integral_constant<int, pull2_stair_a(CPA, 0)>{}, std::integral_constant<int, 0>{});
     }
     return f(std::integral_constant<int, pull2_stair_a(CPA, W)>{}, std::integral_constant<int, pull2_stair_b(CPB, NW, W)>{});
 }
@@ -493,27 +498,28 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
     // (mode kRhs).
     auto substeps = [&](auto caw_, auto cbw_) -> bool {
     constexpr int CAW = decltype(caw_)::value, CBW = decltype(cbw_)::value;
+    constexpr bool HB = CBW > 0;  // this warp plays species on side b at all (else: none of that side's work)
     while (run) {
         // ---- publish y x {1, hubs}, both species -------------------------------------------
         const real pa1 = ya * yh0, pa2 = ya * yh1, pa3 = ya * yh2;
         const real pb1 = yb * yh0, pb2 = yb * yh1, pb3 = yb * yh2;
         sts(A.s_pub, ya);
-        sts(B.s_pub, yb);
+        if (HB) sts(B.s_pub, yb);
         sts(A.s_pub + TV * SZ, pa1);
-        sts(B.s_pub + TV * SZ, pb1);
+        if (HB) sts(B.s_pub + TV * SZ, pb1);
         sts(A.s_pub + 2 * TV * SZ, pa2);
-        sts(B.s_pub + 2 * TV * SZ, pb2);
+        if (HB) sts(B.s_pub + 2 * TV * SZ, pb2);
         sts(A.s_pub + 3 * TV * SZ, pa3);
-        sts(B.s_pub + 3 * TV * SZ, pb3);
+        if (HB) sts(B.s_pub + 3 * TV * SZ, pb3);
 
         // barrier A, right behind the publishes: what follows up to barrier B (rate sums, gathers, butterfly)
         // needs no further hand-shake, so the warps' skews over it add up once, at B, instead of being
         // waited out twice
         __syncthreads();
         // ---- rate sums: k = F-/y (Eq. (1)) and the hub-row shares, added over the two ----------
-        real ka, kb, share[6];
+        real ka, kb = 0, share[6];
         {
-            real sb[6], Ga[kPull2SmemCoefs], Gb[kPull2SmemCoefs];
+            real sb[6] = {}, Ga[kPull2SmemCoefs], Gb[kPull2SmemCoefs] = {};
             if (KT) {
                 // five chunks of 8 values: K and most of G of side a, of side b, the three last G of both
                 // (the first two were issued after the last barrier B, or before the loop)
@@ -523,14 +529,16 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
 #pragma unroll
                 for (int j = 0; j < 8; ++j) x[j] = x1[j];
                 Ka[8] = x[0], Ka[9] = x[1], Ga[0] = x[2], Ga[3] = x[3], Ga[1] = x[4], Ga[5] = x[5], Ga[2] = x[6], Ga[7] = x[7];
-                tm_load8(x, tm_at(16 * RW));
-                Kb[0] = x[0], Kb[1] = x[1], Kb[4] = x[2], Kb[5] = x[3], Kb[6] = x[4], Kb[2] = x[5], Kb[7] = x[6], Kb[3] = x[7];
-                tm_load8(x, tm_at(24 * RW));
-                Kb[8] = x[0], Kb[9] = x[1], Gb[0] = x[2], Gb[3] = x[3], Gb[1] = x[4], Gb[5] = x[5], Gb[2] = x[6], Gb[7] = x[7];
+                if (HB) {
+                    tm_load8(x, tm_at(16 * RW));
+                    Kb[0] = x[0], Kb[1] = x[1], Kb[4] = x[2], Kb[5] = x[3], Kb[6] = x[4], Kb[2] = x[5], Kb[7] = x[6], Kb[3] = x[7];
+                    tm_load8(x, tm_at(24 * RW));
+                    Kb[8] = x[0], Kb[9] = x[1], Gb[0] = x[2], Gb[3] = x[3], Gb[1] = x[4], Gb[5] = x[5], Gb[2] = x[6], Gb[7] = x[7];
+                }
                 tm_load8(x, tm_at(32 * RW));
                 Ga[4] = x[0], Ga[6] = x[1], Ga[8] = x[2], Gb[4] = x[3], Gb[6] = x[4], Gb[8] = x[5];
                 pull_rate_sums<real>(Ka, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
-                pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+                if (HB) pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
             } else if (TM) {
                 tm_load_g(Ga, Gb, tm_at(0));
             } else {
@@ -549,13 +557,15 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
                     Kb[j] = lds_at<real>(s_K + (j * TV + vb) * SZ);
                 }
                 pull_rate_sums<real>(Ka, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
-                pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+                if (HB) pull_rate_sums<real>(Kb, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
             } else {
                 pull_rate_sums<real>(A.C, Ga, ya, pa1, pa2, pa3, yh0, yh1, yh2, ka, share);
-                pull_rate_sums<real>(B.C, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
+                if (HB) pull_rate_sums<real>(B.C, Gb, yb, pb1, pb2, pb3, yh0, yh1, yh2, kb, sb);
             }
+            if (HB) {
 #pragma unroll
-            for (int i = 0; i < 6; ++i) share[i] += sb[i];
+                for (int i = 0; i < 6; ++i) share[i] += sb[i];
+            }
         }
         // own consumption of a hub owner in a hub-only reaction, read in finalize.  Stored between
         // the barriers: B orders it before this step's reads, the next A orders those reads
@@ -715,7 +725,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         real inva = 0, invb = 0;  // reciprocal factors of the dt candidates, off the critical path
         if (ADAPT) {
             inva = rcp_pos(ya > y_floor ? eps_y * ya : yfl_eps);
-            invb = rcp_pos(yb > y_floor ? eps_y * yb : yfl_eps);
+            if (HB) invb = rcp_pos(yb > y_floor ? eps_y * yb : yfl_eps);
             if (!plain_a) inva = 0;  // hub owners are judged on their full rows in finalize
             if (!plain_b) invb = 0;
         }
@@ -811,16 +821,18 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         const real h = static_cast<real>(hd), qr = static_cast<real>(q);
 
         // ---- S4: update (Eq. (3)), Eq. (3) as (y q + F+) / (q + k) -----------
-        real yna, ynb;
+        real yna, ynb = yb;
         {
             const real aa = fma(ya, qr, Fpa) * rcp_pos(qr + ka);
-            const real ab = fma(yb, qr, Fpb) * rcp_pos(qr + kb);
-            const real ea = fma(h, cha, ya), eb = fma(h, chb, yb);
+            const real ea = fma(h, cha, ya);
             yna = (ya > 0 && ka * h >= kappa) ? aa : ea;
-            ynb = (yb > 0 && kb * h >= kappa) ? ab : eb;
-            if (qss) {  // uniform: the QSS variant, one formula for every species
+            if (qss)  // uniform: the QSS variant, one formula for every species
                 yna = fma(cha, rcp_pos(qr + qss_alpha_k(ya > 0 ? ka : static_cast<real>(0), h)), ya);
-                ynb = fma(chb, rcp_pos(qr + qss_alpha_k(yb > 0 ? kb : static_cast<real>(0), h)), yb);
+            if (HB) {
+                const real ab = fma(yb, qr, Fpb) * rcp_pos(qr + kb);
+                const real eb = fma(h, chb, yb);
+                ynb = (yb > 0 && kb * h >= kappa) ? ab : eb;
+                if (qss) ynb = fma(chb, rcp_pos(qr + qss_alpha_k(yb > 0 ? kb : static_cast<real>(0), h)), yb);
             }
         }
         {  // hub species, on lanes 0..nbs-1 of every warp: Y (Y q + F+) / (Y q + F-)
@@ -854,7 +866,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
     {
         bool done;
         if (BRF && NW > 1 && p.stair) {  // warp-uniform
-            done = stair_dispatch<NW, CPA, CPB>(warp, substeps);
+            done = stair_dispatch<NW, CPA, CPB>(warp, p.stair == 2, substeps);
         } else {
             done = substeps(std::integral_constant<int, CPA>{}, std::integral_constant<int, CPB>{});
         }
