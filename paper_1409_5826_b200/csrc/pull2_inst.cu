@@ -24,14 +24,18 @@ int pull2_stair_class(const PullSchedule& P) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2) || P.T / 64 < 2) return 0;
     const int nw = P.T / 64, cap_a = pull2_cap_a(sa);
-    bool b0_empty = true;
+    int cls = 1 | 2;
     for (int t = 0; t < P.T; ++t) {
         const int vw = t / 32;
-        const int cap = vw < nw ? pull2_stair_a(cap_a, vw) : pull2_stair_b(kPull2CapB, nw, 2 * nw - 1 - vw);
-        if (P.n_slots[t] > cap) return 0;
-        if (vw == 2 * nw - 1 && P.owner[t] >= 0) b0_empty = false;
+        if (vw < nw) {
+            if (P.n_slots[t] > pull2_stair_a(cap_a, vw)) return 0;
+        } else {
+            const int w = 2 * nw - 1 - vw;
+            if (P.n_slots[t] > pull2_stair_b(kPull2CapB, nw, w)) cls |= 1 << (8 + w);
+            if (w == 0 && P.owner[t] >= 0) cls &= ~2;
+        }
     }
-    return b0_empty ? 2 : 1;
+    return cls;
 }
 #endif
 

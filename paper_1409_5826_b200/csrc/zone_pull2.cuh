@@ -84,8 +84,9 @@ __host__ __device__ constexpr int pull2_stair_a(int cap_a, int w) { return cap_a
 __host__ __device__ constexpr int pull2_stair_b(int cap_b, int nw, int w) {
     return cap_b - 4 * (nw - 1 - w) > 4 ? cap_b - 4 * (nw - 1 - w) : 4;
 }
-// KPull.stair: 0 = no fit, 1 = fits, 2 = fits and warp 0 plays no species on side b (N <= 32 (2 NW - 1)):
-// its copy of the loop then has none of that side's work (capacity 0)
+// KPull.stair: 0 = side a does not fit (every warp runs the instantiation's capacities); else bit 0 set, bit 1 =
+// warp 0 plays no species on side b (N <= 32 (2 NW - 1)): its copy of the loop then has none of that side's
+// work (capacity 0); bit 8 + w = warp w's side b does not fit its step and runs the full capacity
 int pull2_stair_class(const PullSchedule& P);
 // method = net_params_t.method (1 = the QSS instantiations)
 pull_fn pull2_kernel_f64_adaptive(const PullSchedule& P, int method);
@@ -256,12 +257,15 @@ __device__ __forceinline__ void pull_rate_sums(const real (&C)[kPullCoefs - kPul
 
 // warp w runs f with its step of the staircase as compile-time capacities
 template <int NW, int CPA, int CPB, int W = 0, typename F>
-__device__ __forceinline__ bool stair_dispatch(int warp, bool b0_empty, F& f) {
+__device__ __forceinline__ bool stair_dispatch(int warp, int cls, F& f) {
     if constexpr (W + 1 < NW) {
-        if (warp != W) return stair_dispatch<NW, CPA, CPB, W + 1>(warp, b0_empty, f);
+        if (warp != W) return stair_dispatch<NW, CPA, CPB, W + 1>(warp, cls, f);
     }
     if constexpr (W == 0) {
-        if (b0_empty) return f(std::integral_constant<int, pull2_stair_a(CPA, 0)>{}, std::integral_constant<int, 0>{});
+        if (cls & 2) return f(std::integral_constant<int, pull2_stair_a(CPA, 0)>{}, std::integral_constant<int, 0>{});
+    }
+    if constexpr (pull2_stair_b(CPB, NW, W) < CPB) {
+        if (cls >> (8 + W) & 1) return f(std::integral_constant<int, pull2_stair_a(CPA, W)>{}, std::integral_constant<int, CPB>{});
     }
     return f(std::integral_constant<int, pull2_stair_a(CPA, W)>{}, std::integral_constant<int, pull2_stair_b(CPB, NW, W)>{});
 }
@@ -866,7 +870,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
     {
         bool done;
         if (BRF && NW > 1 && p.stair) {  // warp-uniform
-            done = stair_dispatch<NW, CPA, CPB>(warp, p.stair == 2, substeps);
+            done = stair_dispatch<NW, CPA, CPB>(warp, p.stair, substeps);
         } else {
             done = substeps(std::integral_constant<int, CPA>{}, std::integral_constant<int, CPB>{});
         }
