@@ -229,6 +229,12 @@ typedef struct {
                             kernel 1, 2 * threads for kernel 2 (a thread plays two of them) */
     int pull_nslots;     /* longest per-thread N-slot list (reactions with two non-hub reactants);
                             0 = the network has none                                    */
+    int pull_stair;      /* two-species kernel: 0 = every warp runs the instantiation's slot
+                            capacities; else bit 0 set = each warp runs its own copy of the sub-step
+                            loop, compiled for its step of the staircase of live slots (side a:
+                            max(cap_a - 4 w, 12), side b: max(12 - 4 (warps - 1 - w), 4) for warp w);
+                            bit 1 = warp 0 plays no species on side b (capacity 0 there); bit 8 + w =
+                            warp w's side b does not fit its step and runs the full capacity     */
 } net_schedule_info_t;
 
 int net_schedule_info(const net_t *net, net_schedule_info_t *info);

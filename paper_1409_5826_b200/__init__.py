@@ -41,7 +41,8 @@ class net_schedule_info_t(C.Structure):
         "n_species", "n_reactions", "threads", "flux_slots", "slots_2body", "slots_3body",
         "n_entries", "n_big_species", "n_entries_big", "small_max", "readback_max", "smem_bytes",
         "zones_per_sm", "kernel", "pull_ok", "pull_hubs", "pull_slots", "pull_slots2",
-        "pull_agg_max", "pull_wavefronts", "pull_wavefronts_ideal", "pull_threads", "pull_nslots")]
+        "pull_agg_max", "pull_wavefronts", "pull_wavefronts_ideal", "pull_threads", "pull_nslots",
+        "pull_stair")]
 
 
 class KinnetError(RuntimeError):

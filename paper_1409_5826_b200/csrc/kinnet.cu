@@ -1107,6 +1107,7 @@ int net_schedule_info(const net_t* n, net_schedule_info_t* info) {
     info->pull_wavefronts_ideal = static_cast<int>(n->PS.ideal_wavefronts);
     info->pull_threads = n->PS.ok ? n->PS.T : 0;
     info->pull_nslots = n->PS.ok ? n->PS.nslots : 0;
+    info->pull_stair = n->pull2 ? n->pull2_stair : 0;
     return NET_OK;
 }
 

@@ -292,3 +292,40 @@ def test_pull_schedule_small_and_unsupported_networks(g16):
     # kernel = 1 forces the generic kernel even when the network qualifies
     info = K.Net(network("hub150"), K.NetParams(kernel=1), host_only=True).schedule_info()
     assert info["pull_ok"] == 1 and info["kernel"] == 0
+
+
+def test_staircase_class_of_the_two_species_schedule():
+    """S0 host logic behind KPull.stair (include/kinnet.h, net_schedule_info_t.pull_stair): the class is
+    recomputed here from the schedule tables alone.  hub150: every side fits its step and warp 0 plays
+    no species on side b; hub150hh: warp 1's side b (up to 10 slots) overflows its step of 8; g16 does
+    not run on the two-species kernel at all."""
+    from gen.configs import network
+
+    def want(kn, info, cap_b=12):
+        n, own = kn.schedule_table("pull_n_slots"), kn.schedule_table("pull_owner")
+        nw = info["pull_threads"] // 64
+        cap_a = 20 if n[: 32 * nw].max() <= 20 else 24
+        cls = 1 | 2
+        for t, (slots, o) in enumerate(zip(n, own)):
+            vw = t // 32
+            if vw < nw:
+                if slots > max(cap_a - 4 * vw, 12):
+                    return 0
+            else:
+                w = 2 * nw - 1 - vw
+                if slots > max(cap_b - 4 * (nw - 1 - w), 4):
+                    cls |= 1 << (8 + w)
+                if w == 0 and o >= 0:
+                    cls &= ~2
+        return cls
+
+    seen = {}
+    for name in ("hub150", "hub150hh", "hub365"):
+        kn = K.Net(network(name), host_only=True)
+        info = kn.schedule_info()
+        assert info["kernel"] == 2 and info["pull_ok"] == 1
+        assert info["pull_stair"] == want(kn, info), name
+        seen[name] = info["pull_stair"]
+    assert seen["hub150"] == 3                      # fits, warp 0 one-sided
+    assert seen["hub150hh"] == 3 | 1 << 9           # warp 1's side b at full capacity
+    assert K.Net(network("g16"), host_only=True).schedule_info()["pull_stair"] == 0
