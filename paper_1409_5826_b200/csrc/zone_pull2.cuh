@@ -277,7 +277,7 @@ __device__ __forceinline__ bool stair_dispatch(int warp, int cls, F& f) {
 // its sub-step is 17 % shorter in a lone CTA (0.72 us against 0.87 us): every batch that does not fill
 // the SMs gains.  160-thread blocks, whose K stays in shared memory, run three CTAs at 128 registers.
 // With fp32 state the rates take half the registers: 128 registers, four warps per scheduler, five
-// 96-thread CTAs (318k zone-networks/s on configs[3]).
+// 96-thread CTAs (318k zone-networks/s on configs[3] at that commit, 365k with the branch-free loop).
 // NS = 4 compiles the N-slots in (networks with heavy + heavy reactions, schedule.h): four more
 // gathers per side into k, skipped by the warps none of whose species has one, and the hub
 // owners' own P-slot sums (heavy + heavy reactions that emit a hub) joined to their rows.
