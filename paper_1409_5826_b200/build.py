@@ -29,11 +29,11 @@ UNITS = [
       f"-DPULL_FN=pull_kernel_f{bits}_{mode}"])
     for bits, real in ((64, "double"), (32, "float")) for mode in ("adaptive", "fixed")
 ] + [
-    (f"pull2_f{bits}_{mode}.o", "pull2_inst.cu",
+    (f"pull2_f{bits}_{mode}_cap{cap}.o", "pull2_inst.cu",
      [f"-DPULL_REAL={real}", f"-DPULL_ADAPT={int(mode == 'adaptive')}",
-      f"-DPULL_FN=pull2_kernel_f{bits}_{mode}",
+      f"-DPULL_FN=pull2_kernel_f{bits}_{mode}", f"-DPULL_CAP={cap}",
       *(["-DPULL2_DEFINE_SUPPORTED"] if (bits, mode) == (64, "adaptive") else [])])
-    for bits, real in ((64, "double"), (32, "float")) for mode in ("adaptive", "fixed")
+    for bits, real in ((64, "double"), (32, "float")) for mode in ("adaptive", "fixed") for cap in (20, 24)
 ]
 
 

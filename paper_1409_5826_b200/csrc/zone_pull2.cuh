@@ -936,24 +936,21 @@ pull_fn pick_pull2_j2(int s2, int ns, bool qss) {
     if (s2 <= 4) return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 4, 0, ADAPT, false, S0>;
     return zone_kernel_pull2<real, TB, CPA, SA, CB, SB, 8, 0, ADAPT, false, S0>;
 }
-template <typename real, int TB, bool ADAPT>
-pull_fn pick_pull2_cap(int sa, int s2, int ns, bool qss) {
-    if (pull2_cap_a(sa) == 20) return pick_pull2_j2<real, TB, 20, ADAPT>(s2, ns, qss);
-    return pick_pull2_j2<real, TB, 24, ADAPT>(s2, ns, qss);
-}
-template <typename real, bool ADAPT>
+// CPA = the side-a capacity this translation unit instantiates (20 or 24; pull2_inst.cu is compiled once per
+// capacity so that the two halves build in parallel); nullptr for a schedule of the other capacity
+template <typename real, int CPA, bool ADAPT>
 pull_fn pick_pull2(const PullSchedule& P, int method = 0) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2)) return nullptr;
-    if (sa > 24 || sb > kPull2CapB || s2 > kJ2C) return nullptr;
+    if (sa > 24 || sb > kPull2CapB || s2 > kJ2C || pull2_cap_a(sa) != CPA) return nullptr;
     const bool qss = method == 1;
     switch (P.T / 2) {
-        case 32: return pick_pull2_cap<real, 32, ADAPT>(sa, s2, P.nslots, qss);
-        case 64: return pick_pull2_cap<real, 64, ADAPT>(sa, s2, P.nslots, qss);
-        case 96: return pick_pull2_cap<real, 96, ADAPT>(sa, s2, P.nslots, qss);
-        case 128: return pick_pull2_cap<real, 128, ADAPT>(sa, s2, P.nslots, qss);
-        case 160: return pick_pull2_cap<real, 160, ADAPT>(sa, s2, P.nslots, qss);
-        case 192: return pick_pull2_cap<real, 192, ADAPT>(sa, s2, P.nslots, qss);
+        case 32: return pick_pull2_j2<real, 32, CPA, ADAPT>(s2, P.nslots, qss);
+        case 64: return pick_pull2_j2<real, 64, CPA, ADAPT>(s2, P.nslots, qss);
+        case 96: return pick_pull2_j2<real, 96, CPA, ADAPT>(s2, P.nslots, qss);
+        case 128: return pick_pull2_j2<real, 128, CPA, ADAPT>(s2, P.nslots, qss);
+        case 160: return pick_pull2_j2<real, 160, CPA, ADAPT>(s2, P.nslots, qss);
+        case 192: return pick_pull2_j2<real, 192, CPA, ADAPT>(s2, P.nslots, qss);
         default: return nullptr;
     }
 }
