@@ -1,7 +1,9 @@
 """Compile csrc/ into paper_1409_5826_b200/libkinnet.so for sm_100a (in-tree).
 
 Objects are built in parallel (the pull kernel is instantiated once per state
-type and mode, csrc/pull_inst.cu) and cached under csrc/build/ by mtime.
+type and mode, csrc/pull_inst.cu; the two-species kernel once per state type,
+mode and side-a slot capacity, csrc/pull2_inst.cu) and cached under csrc/build/
+by mtime.
 """
 from __future__ import annotations
 
