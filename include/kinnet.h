@@ -153,6 +153,51 @@ int net_integrate_energy(net_t *net, int zones, const double *T9, const double *
                          double t_hydro, double *dt, int *n_steps, int *status, double *energy,
                          void *cuda_stream);
 
+/*
+ * net_integrate for callers that must not allocate device memory while they run.
+ *
+ * Who this is for.  net_create reserves the launch-order workspaces of net_integrate with
+ * cudaMalloc, and net_reserve grows them the same way.  Some hosts of this library cannot
+ * afford that: a hydro code that has handed the whole of HBM to its own pool allocator (a
+ * later cudaMalloc fails, or fragments the pool), a code whose time loop lives in a region
+ * where the runtime forbids allocation (cudaMalloc synchronises the device and is illegal
+ * while a stream is being captured), and real-time or certified drivers in which every byte
+ * must be accounted for before the run starts.  For them the one piece of scratch this
+ * entry point needs -- the counting sort that launches the hottest zones first (PAPER.md
+ * L200 leaves the load balance of unequal networks open) -- lives in a fixed
+ * array inside the library image instead of the heap:
+ *   (2048 + NET_STATIC_MAX_ZONES) ints = 264 KB of device memory, held by every GPU that
+ *   loads libkinnet.so from the moment the CUDA module is loaded until the process exits,
+ *   whether or not this function is ever called.
+ *
+ * Arguments, layouts, units and results are those of net_integrate: the same zone kernel runs
+ * on the same inputs, and the order only decides when a zone runs, so the outputs are bit
+ * for bit net_integrate's.  The caller still owns and passes every input and output array
+ * (device memory).  Differences:
+ *   - zones > NET_STATIC_MAX_ZONES fails with NET_EINVAL and a message naming the limit;
+ *     nothing is launched.  Split the batch into several calls on ONE stream.
+ *   - The call itself performs no cudaMalloc / cudaFree and calls no allocating routine.  It
+ *     enqueues a memset of the sort's 8 KB header (counts and cursors must start at zero; the
+ *     order itself is fully rewritten by every call, so the previous call's contents never
+ *     leak), two small order kernels and the zone kernel on `cuda_stream`, and returns.
+ *   - The FIRST call on each device looks the array's device address up
+ *     (cudaGetSymbolAddress, with the net_t's device current) and caches it for the life of
+ *     the process.  Make that first call at set-up time, before any stream capture begins; a
+ *     call with zones = 0 is enough and launches nothing.
+ *   - There is ONE array per device, shared by every net_t, stream and host thread.  Two
+ *     calls whose GPU work can overlap (calls on different streams with no event between
+ *     them, whichever host thread issues them) race on it: zones may then be skipped or
+ *     integrated twice.  Issue all calls on a device into one stream, or order them with
+ *     events.  net_integrate has per-stream workspaces and no such rule; prefer it
+ *     whenever allocation at net_create time is acceptable.
+ * The net_t itself is still built by net_create, which allocates its tables: do that during
+ * set-up, where allocation is allowed.
+ */
+#define NET_STATIC_MAX_ZONES 65536
+int net_integrate_static(net_t *net, int zones, const double *T9, const double *rho, void *Y,
+                         double t_hydro, double *dt, int *n_steps, int *status,
+                         void *cuda_stream);
+
 /* Exactly n_steps sub-steps of size dt_fixed for every zone (parity mode). */
 int net_integrate_fixed(net_t *net, int zones, const double *T9, const double *rho, void *Y,
                         double dt_fixed, long long n_steps, void *cuda_stream);

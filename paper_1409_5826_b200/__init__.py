@@ -19,12 +19,13 @@ LIB_PATH = os.path.join(_HERE, "libkinnet.so")
 
 NET_OK, NET_EINVAL, NET_ENOMEM, NET_ECUDA = 0, -1, -2, -3
 NET_STATUS_MAX_STEPS, NET_STATUS_NONFINITE = 1, 2
+NET_STATIC_MAX_ZONES = 65536  # largest batch of net_integrate_static (include/kinnet.h)
 
 EXPORTS = (
     "net_default_params", "net_create", "net_create_host", "net_destroy", "net_integrate",
     "net_integrate_fixed", "net_integrate_host", "net_integrate_host_async", "net_wait", "net_reserve",
     "net_set_binding_energy", "net_integrate_energy", "net_rates", "net_rhs", "net_schedule_info",
-    "net_schedule_table", "net_last_error",
+    "net_schedule_table", "net_last_error", "net_integrate_static",
 )
 
 
@@ -65,6 +66,7 @@ def _load() -> C.CDLL:
     lib.net_destroy.argtypes = [vp]
     lib.net_destroy.restype = None
     lib.net_integrate.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp]
+    lib.net_integrate_static.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp]
     lib.net_set_binding_energy.argtypes = [vp, dp]
     lib.net_integrate_energy.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp, vp, vp]
     lib.net_integrate_fixed.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, C.c_longlong, vp]
@@ -185,6 +187,18 @@ class Net:
                       stream=None):
         _check(lib.net_integrate(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y), float(t_hydro),
                                  _ptr(dt), _ptr(n_steps), _ptr(status), _stream(stream)))
+
+    def net_integrate_static(self, zones, T9, rho, Y, t_hydro, dt=None, n_steps=None, status=None,
+                             stream=None):
+        """net_integrate without any device allocation behind it, for callers that may not
+        allocate while they run (their own pool owns the GPU's memory, or they sit in a region
+        where cudaMalloc is illegal): the launch-order scratch is a fixed 264 KB array in the
+        library.  At most NET_STATIC_MAX_ZONES zones per call; one call at a time per device
+        (calls that overlap on the GPU race on the array); make the first call on a device
+        before any stream capture.  Same arguments and bit-identical results (include/kinnet.h)."""
+        _check(lib.net_integrate_static(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(Y),
+                                        float(t_hydro), _ptr(dt), _ptr(n_steps), _ptr(status),
+                                        _stream(stream)))
 
     def net_set_binding_energy(self, B):
         B = np.ascontiguousarray(B, np.float64)

@@ -945,6 +945,93 @@ int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rh
     return launch<kAdaptive>(n, zones, k, stream);
 }
 
+// ---------------------------------------------------------------------------------------
+// net_integrate_static (include/kinnet.h): net_integrate for hosts that may not allocate once
+// they are running -- codes whose own pool owns all of HBM, time loops inside a capture or
+// another region where cudaMalloc is illegal, drivers that must account for every byte up
+// front.  The launch-order workspace (the only scratch of the adaptive path) is this array in
+// the library image rather than a cudaMalloc'ed lane: [0, 1024) bucket counts, [1024, 2048)
+// bucket cursors, then the order of up to NET_STATIC_MAX_ZONES zones; 264 KB on every GPU
+// that loads the module, until the process exits.
+//
+// In HOST code the name g_static_order is only the host-side shadow of the symbol: it is not
+// a device address, and a kernel handed `g_static_order` directly would fault or, on a system
+// where the GPU can reach host memory, quietly scribble on the shadow.  Host code therefore
+// asks the runtime for the device address once per device (static_order_ptr below) and
+// passes that pointer to the kernels.
+static __device__ __align__(256) int g_static_order[kLaneHeader + NET_STATIC_MAX_ZONES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+int* g_static_ptr[kStaticMaxDevices] = {};  // device address of g_static_order, per device ordinal
+
+// Device address of the array on `device`, which must be the calling thread's current device
+// (check_net has verified that).  The first call per device does the lookup; later calls
+// read the cache.
+int static_order_ptr(int device, int** out) {
+    *out = nullptr;
+    if (device < 0 || device >= kStaticMaxDevices)
+        return fail(NET_EINVAL, "net_integrate_static supports device ordinals 0.." +
+                                    std::to_string(kStaticMaxDevices - 1));
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_order);
+        if (e != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            return fail(NET_ECUDA, std::string("cudaGetSymbolAddress(static launch-order array): ") +
+                                       (e != cudaSuccess ? cudaGetErrorString(e) : "null address"));
+        }
+        g_static_ptr[device] = static_cast<int*>(p);
+    }
+    *out = g_static_ptr[device];
+    return NET_OK;
+}
+
+}  // namespace
+
+int net_integrate_static(net_t* n, int zones, const double* T9, const double* rho, void* Y,
+                         double t_hydro, double* dt, int* n_steps, int* status, void* stream) {
+    if (int rc = check_net(n)) return rc;
+    if (zones < 0) return fail(NET_EINVAL, "zones < 0");
+    if (zones > NET_STATIC_MAX_ZONES)
+        return fail(NET_EINVAL, "net_integrate_static: " + std::to_string(zones) +
+                                    " zones exceed the static launch-order array (NET_STATIC_MAX_ZONES = " +
+                                    std::to_string(NET_STATIC_MAX_ZONES) +
+                                    "); split the batch into several calls on one stream");
+    int* ws = nullptr;  // set-up on the first call per device, also for zones == 0
+    if (int rc = static_order_ptr(n->device, &ws)) return rc;
+    if (zones == 0) return NET_OK;
+    if (!Y) return fail(NET_EINVAL, "null Y");
+    if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
+    if (!std::isfinite(t_hydro)) return fail(NET_EINVAL, "t_hydro is not finite");
+    // hottest-first order of this batch in the static array: counts and cursors start at zero,
+    // the scatter then writes every one of order[0, zones) -- nothing of the last call is read
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int ctas = (zones + kOrderZonesPerCta - 1) / kOrderZonesPerCta;
+    CUDA_TRY(cudaMemsetAsync(ws, 0, sizeof(int) * kLaneHeader, s));
+    zone_hist_kernel<<<ctas, kOrderThreads, 0, s>>>(T9, zones, ws);
+    zone_scatter_kernel<<<ctas, kOrderThreads, 0, s>>>(T9, zones, ws, ws + kOrderBuckets, ws + kLaneHeader);
+    CUDA_TRY(cudaGetLastError());
+    if (use_pull_kernel(n)) {
+        KPull q;
+        fill_pull(n, q);
+        q.mode = kAdaptive;
+        q.T9 = T9; q.rho = rho; q.Y = Y; q.dt = dt; q.n_steps = n_steps; q.status = status;
+        q.t_hydro = t_hydro;
+        q.order = ws + kLaneHeader;
+        return launch_pull(n, zones, q, stream);
+    }
+    KParams k;
+    fill_params(n, k);
+    k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
+    k.t_hydro = t_hydro;
+    k.order = ws + kLaneHeader;
+    return launch<kAdaptive>(n, zones, k, stream);
+}
+
 int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                         double dt_fixed, long long n_steps, void* stream) {
     if (int rc = check_net(n)) return rc;
