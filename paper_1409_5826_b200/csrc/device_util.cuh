@@ -4,6 +4,19 @@
 
 namespace kinnet {
 
+// Barrier 0 over the whole CTA, written as the PTX instruction itself.  In the staircase of the
+// two-species kernel (zone_pull2.cuh) every warp of a CTA runs its own compiled copy of the
+// sub-step loop, so the warps meet at barrier call sites that differ from warp to warp.  That is
+// what PTX defines: a barrier resource counts the warps that arrive, whatever their program
+// counter, and .aligned only asks that all threads of ONE warp execute the same instance (they
+// do: the copy is chosen per warp).  CUDA C++ makes no such promise for __syncthreads() under a
+// condition that differs across the block, so the design's contract is spelled out here instead
+// of resting on how __syncthreads() happens to compile.  The contract the callers keep: every
+// copy executes the same number of barriers per sub-step (two: A behind the publishes, B before
+// the finalize) and leaves the loop on values read from shared memory after B, identical in
+// every warp.
+__device__ __forceinline__ void cta_barrier() { asm volatile("barrier.sync.aligned 0;" ::: "memory"); }
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

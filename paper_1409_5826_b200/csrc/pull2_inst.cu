@@ -37,6 +37,7 @@ bool pull2_supported(const PullSchedule& P, int* spill) {
 int pull2_stair_class(const PullSchedule& P) {
     int sa, sb, s2;
     if (!pull2_sides(P, sa, sb, s2) || P.T / 64 < 2) return 0;
+    if (P.T / 2 > 128) return 0;  // 160/192-thread blocks run the branching loop (zone_pull2.cuh: BRF), no per-warp copies
     const int nw = P.T / 64, cap_a = pull2_cap_a(sa);
     int cls = 1 | 2;
     for (int t = 0; t < P.T; ++t) {

@@ -519,7 +519,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
         // barrier A, right behind the publishes: what follows up to barrier B (rate sums, gathers, butterfly)
         // needs no further hand-shake, so the warps' skews over it add up once, at B, instead of being
         // waited out twice
-        __syncthreads();
+        cta_barrier();
         // ---- rate sums: k = F-/y (Eq. (1)) and the hub-row shares, added over the two ----------
         real ka, kb = 0, share[6];
         {
@@ -739,7 +739,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
             const double c = warp_max_pos(static_cast<double>(qa > qb ? qa : qb));
             if (lane == 0) sts(s_redq + warp * 8, c);
         }
-        __syncthreads();
+        cta_barrier();
         if (KT) {  // the next sub-step's first two coefficient chunks: in flight during the finalize
             tm_ld(pf0, tm_at(0));
             tm_ld(pf1, tm_at(8 * RW));
@@ -794,7 +794,7 @@ __global__ void __launch_bounds__(TB, (sizeof(real) == 4 || ST == kStoreTmemKs ?
                     tm_wait(pf0);
                     tm_touch(pf1);
                 }
-                __syncthreads();
+                cta_barrier();
                 if (warp == 0)
                     tm_free();
             }
