@@ -445,6 +445,43 @@ def test_dt_controller_contract():
     assert out["n_steps"][0] == 0 and out["dt"][0] == 0.3 and out["Y"][0, 0] == 1.0
 
 
+def test_nonfinite_status_bit_worked_by_hand():
+    """P:L110 / SURVEY 8(b): status bit 2 = a non-finite abundance was produced (O9's check).
+
+    Overflow, every step known.  A -> B with k = 1, Y_A = Y_B = 1.5e308, eps_Y = 0.25,
+    t_hydro = 10, no trial dt.  Step 1: F_A = -1.5e308, F_B = +1.5e308, so c_A = c_B =
+    0.25 * 1.5e308 / 1.5e308 = 0.25 < growth * t_hydro: dt = 0.25, k_A dt = 0.25 < kappa,
+    Euler on both: Y_A = 1.5e308 * 0.75 and Y_B = 1.5e308 * 1.25 = 1.875e308 > DBL_MAX = +inf.
+    From then on Y_B = inf has F- = 0 (k = 0, Euler, stays inf) and an infinite candidate;
+    Y_A keeps c_A = 0.25 and loses a quarter per step.  0.25 is a binary fraction, so t hits
+    10 exactly on step 40 (the last one through the 1e-12 guard): n_steps = 40, dt = 0.25,
+    Y_A = 1.5e308 * 0.75^40, status = 2 and NOT 1 | 2."""
+    o = Oracle(decay_net(1.0), OracleParams(eps_y=0.25))
+    out = o.integrate(1.0, 1.0, [1.5e308, 1.5e308], 10.0)
+    assert out["status"][0] == 2 and out["n_steps"][0] == 40 and out["dt"][0] == 0.25
+    assert np.isposinf(out["Y"][0, 1])
+    assert out["Y"][0, 0] == pytest.approx(1.5e308 * 0.75**40, rel=1e-13)
+    # a start whose total Y_A + Y_B = 1.6e308 stays below DBL_MAX never overflows: bit 2 stays clear
+    out = o.integrate(1.0, 1.0, [0.8e308, 0.8e308], 10.0)
+    assert out["status"][0] == 0 and np.isfinite(out["Y"]).all() and out["n_steps"][0] == 40
+    # fixed-dt mode overflows the same way: one Euler step of dt = 0.5 from 1.5e308 overflows B
+    out = o.integrate_fixed(1.0, 1.0, [1.5e308, 1.5e308], 0.5, 1)
+    assert np.isposinf(out["Y"][0, 1]) and out["Y"][0, 0] == 0.75e308
+    # NaN from the inputs: T9 < 0 makes ln T9 (a6 term) NaN whenever a6 != 0, every rate of such a
+    # reaction NaN, every flux NaN; a NaN candidate never wins the dt minimum ('<' is false), so the
+    # zone takes ONE step of the whole t_hydro, returns dt = growth * t_hydro, and flags bit 2;
+    # zones beside it in the batch are untouched
+    c = build_config(3, zones=3)
+    good = Oracle(c["network"]).integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    T9 = c["T9"].copy()
+    T9[1] = -1.0
+    bad = Oracle(c["network"]).integrate(T9, c["rho"], c["Y0"], c["t_hydro"])
+    assert bad["status"].tolist() == [0, 2, 0] and bad["n_steps"][1] == 1
+    assert bad["dt"][1] == 2.0 * c["t_hydro"] and np.isnan(bad["Y"][1]).any()
+    for z in (0, 2):
+        assert np.array_equal(bad["Y"][z], good["Y"][z]) and bad["n_steps"][z] == good["n_steps"][z]
+
+
 def test_zero_abundance_species_use_euler():
     """S:Q8: Y_i = 0 => k_i = 0 => Euler: Y_i' = dt F+_i, however large dt is."""
     o = Oracle(make_toy([1, 1, 1], [((0,), (1,)), ((1,), (2,))], [2.0, 1e6]))
