@@ -28,13 +28,22 @@
  *     capture (every operation they enqueue is a kernel launch or a memset node).
  *   - One net_t may be driven from several streams (and host threads) at once.  The only
  *     per-call device state is the launch-order workspace of net_integrate (4 bytes per
- *     zone + 8 KB): the net_t holds 8 of them ("lanes", 65536 zones each after
- *     net_create, grown by net_reserve), one per stream that calls with >= 1024 zones.
- *     A call that finds no lane (a ninth stream, or more zones than reserved) still runs
- *     and returns the same results bit for bit; it only launches the zones in caller
- *     order instead of hottest first.  A captured call keeps the lane of the stream it
- *     was captured on: graphs that may replay concurrently must be captured on
- *     different streams.
+ *     zone + 8 KB): the net_t holds 16 of them ("lanes", 65536 zones each after
+ *     net_create, grown by net_reserve) and hands one to every call with >= 1024 zones:
+ *       eager calls   the lane the stream used last (stream order serialises its users), else
+ *                     a free one, else the least recently used lane whose last zone kernel
+ *                     has finished -- streams may come and go, lanes are recycled;
+ *       captured calls  a lane of its own per stream capture, never handed out again: the
+ *                     graph holds pointers into it and may replay at any time, on any
+ *                     stream, beside eager calls and beside other graphs of the same net_t.
+ *                     It stays valid until net_destroy.  Every capture that contains a call
+ *                     of >= 1024 zones therefore uses up one of the 16 lanes for good.
+ *     A call that finds no lane (every lane busy or pinned by a capture, or more zones than
+ *     reserved) still runs and returns the same results bit for bit; it only launches the
+ *     zones in caller order instead of hottest first (net_launch_stats counts such calls).
+ *     No two launches ever share a lane concurrently.  What remains the caller's business:
+ *     two replays of the SAME graph must not overlap on the GPU (they would share every
+ *     buffer, the lane included), as for any CUDA graph that writes memory.
  *   - A net_t belongs to the CUDA device that was current in net_create; calls with
  *     another device current fail with NET_EINVAL.
  *   - net_integrate_host / net_integrate_host_async take HOST buffers (end to end).
@@ -198,16 +207,29 @@ int net_integrate_static(net_t *net, int zones, const double *T9, const double *
                          double t_hydro, double *dt, int *n_steps, int *status,
                          void *cuda_stream);
 
-/* Exactly n_steps sub-steps of size dt_fixed for every zone (parity mode). */
+/* Exactly n_steps sub-steps of size dt_fixed for every zone (parity mode).  dt_fixed must be
+ * finite and > 0 (NET_EINVAL otherwise). */
 int net_integrate_fixed(net_t *net, int zones, const double *T9, const double *rho, void *Y,
                         double dt_fixed, long long n_steps, void *cuda_stream);
 
 /*
  * Grow every launch-order lane to hold max_zones zones (see "Conventions").  Synchronises the
  * device and reallocates: call it at set-up time, never inside a capture or with launches
- * in flight on other host threads.  Shrinks nothing.
+ * in flight on other host threads.  Shrinks nothing.  Fails with NET_EINVAL (and changes
+ * nothing) once a stream capture has taken a lane of this net_t: the captured graph holds
+ * pointers into the workspaces this call would free.  Reserve first, capture afterwards.
  */
 int net_reserve(net_t *net, int max_zones);
+
+/*
+ * Launch-order bookkeeping since net_create (host-side counters; any pointer may be NULL):
+ *   sorted_calls    calls of >= 1024 zones that launched hottest first
+ *   unsorted_calls  such calls that found no lane and launched in caller order (same bits,
+ *                   10-20 % slower on a batch with a wide spread of temperatures)
+ *   lanes_pinned    lanes held for good by stream captures, of 16
+ */
+int net_launch_stats(net_t *net, long long *sorted_calls, long long *unsorted_calls,
+                     int *lanes_pinned);
 
 /*
  * End-to-end variants: every array is a HOST buffer -- the 154-in / 152-out float exchange of
@@ -220,12 +242,17 @@ int net_reserve(net_t *net, int max_zones);
  *     hottest-first order is kept.  No device scratch.
  *   - Any other host memory: staged through device scratch owned by the net_t (grown on
  *     demand: that call then synchronises the internal streams and allocates), in chunks of
- *     params.host_chunk zones over three internal streams, so that the upload of one chunk, the
- *     kernels of the previous one and the download of the one before overlap; the launch order
- *     then applies within a chunk.
+ *     params.host_chunk zones over three internal streams; the launch order then applies
+ *     within a chunk.  Copies between PAGEABLE memory and the device block the host thread
+ *     (an upload until the data are in the driver's staging buffer, a download until it has
+ *     finished), so the upload and the kernels of chunk c are enqueued before the download of
+ *     chunk c-1: the GPU integrates chunk c while chunk c-1 comes back.  With pageable
+ *     buffers net_integrate_host_async therefore returns only when all but the last download
+ *     are done; it is asynchronous for pinned buffers (either path).
  *   net_integrate_host_async  enqueues everything and returns; the host buffers must stay
  *                             valid and untouched until net_wait returns.  One batch in
- *                             flight per net_t.
+ *                             flight per net_t: a second call before net_wait fails with
+ *                             NET_EINVAL and touches nothing.
  *   net_wait                  blocks until the batch enqueued last is back in the host buffers
  *   net_integrate_host        = net_integrate_host_async + net_wait
  * Results are bit for bit those of net_integrate on the same zones, on either path.
@@ -275,7 +302,8 @@ typedef struct {
     int pull_nslots;     /* longest per-thread N-slot list (reactions with two non-hub reactants);
                             0 = the network has none                                    */
     int pull_stair;      /* two-species kernel: 0 = every warp runs the instantiation's slot
-                            capacities; else bit 0 set = each warp runs its own copy of the sub-step
+                            capacities (always so for blocks of more than 128 threads, i.e. more
+                            than 256 species); else bit 0 set = each warp runs its own copy of the sub-step
                             loop, compiled for its step of the staircase of live slots (side a:
                             max(cap_a - 4 w, 12), side b: max(12 - 4 (warps - 1 - w), 4) for warp w);
                             bit 1 = warp 0 plays no species on side b (capacity 0 there); bit 8 + w =

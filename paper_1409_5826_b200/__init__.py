@@ -25,7 +25,7 @@ EXPORTS = (
     "net_default_params", "net_create", "net_create_host", "net_destroy", "net_integrate",
     "net_integrate_fixed", "net_integrate_host", "net_integrate_host_async", "net_wait", "net_reserve",
     "net_set_binding_energy", "net_integrate_energy", "net_rates", "net_rhs", "net_schedule_info",
-    "net_schedule_table", "net_last_error", "net_integrate_static",
+    "net_schedule_table", "net_last_error", "net_integrate_static", "net_launch_stats",
 )
 
 
@@ -55,7 +55,7 @@ class KinnetError(RuntimeError):
 def _load() -> C.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(
-            f"{LIB_PATH} is missing: build it with `python -m paper_1409_5826_b200.build` "
+            f"{LIB_PATH} is missing: build it with `python paper_1409_5826_b200/build.py` "
             "(there is no CPU fallback)")
     lib = C.CDLL(LIB_PATH)
     vp, ip, dp = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double)
@@ -74,6 +74,7 @@ def _load() -> C.CDLL:
     lib.net_integrate_host_async.argtypes = [vp, C.c_int, vp, vp, vp, C.c_double, vp, vp, vp]
     lib.net_wait.argtypes = [vp]
     lib.net_reserve.argtypes = [vp, C.c_int]
+    lib.net_launch_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), ip]
     lib.net_rates.argtypes = [vp, C.c_int, vp, vp, vp, vp]
     lib.net_rhs.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp]
     lib.net_schedule_info.argtypes = [vp, C.POINTER(net_schedule_info_t)]
@@ -228,6 +229,11 @@ class Net:
 
     def net_reserve(self, max_zones):
         _check(lib.net_reserve(self._h, int(max_zones)))
+
+    def net_launch_stats(self) -> dict:
+        a, b, c = C.c_longlong(), C.c_longlong(), C.c_int()
+        _check(lib.net_launch_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return {"sorted_calls": a.value, "unsorted_calls": b.value, "lanes_pinned": c.value}
 
     def net_rates(self, zones, T9, rho, R, stream=None):
         _check(lib.net_rates(self._h, int(zones), _ptr(T9), _ptr(rho), _ptr(R), _stream(stream)))

@@ -413,8 +413,9 @@ struct DeviceTables {
 }  // namespace
 
 // Launch-order workspaces ("lanes"): one per stream that has a sorted launch in flight on
-// this net_t.  [0, 1024) bucket counts, [1024, 2048) bucket cursors, then the order itself.
-constexpr int kLanes = 8;
+// this net_t, and one per stream capture (a graph may replay at any time, beside anything).
+// [0, 1024) bucket counts, [1024, 2048) bucket cursors, then the order itself.
+constexpr int kLanes = 16;
 constexpr int kLaneHeader = 2 * kOrderBuckets;
 constexpr int kDefaultReserve = 65536;  // zones per lane allocated by net_create
 constexpr int kHostStreams = 3;         // internal streams of net_integrate_host_async
@@ -439,6 +440,13 @@ struct net {
     int* lane_buf[kLanes] = {};
     cudaStream_t lane_stream[kLanes] = {};
     bool lane_used[kLanes] = {};
+    bool lane_captured[kLanes] = {};              // handed to a stream capture: that graph's for good
+    unsigned long long lane_capture[kLanes] = {}; // ... the capture's id
+    cudaEvent_t lane_done[kLanes] = {};           // recorded behind the last eager zone kernel on the lane
+    unsigned long long lane_tick[kLanes] = {};    // value of `tick` at the lane's last use
+    unsigned long long tick = 0;
+    long long sorted_calls = 0, unsorted_calls = 0;  // calls of >= kOrderMinZones zones with / without a lane
+    bool host_in_flight = false;                  // net_integrate_host_async without its net_wait
     // device scratch and streams of net_integrate_host_async
     cudaStream_t host_stream[kHostStreams] = {};
     int scratch_zones = 0;
@@ -560,43 +568,89 @@ int alloc_lanes(net* n, int cap) {
         n->lane_buf[l] = nullptr;
     }
     n->lane_cap = 0;
-    for (int l = 0; l < kLanes; ++l)
+    for (int l = 0; l < kLanes; ++l) {
         CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&n->lane_buf[l]),
                             sizeof(int) * (static_cast<size_t>(kLaneHeader) + cap)));
+        if (!n->lane_done[l]) CUDA_TRY(cudaEventCreateWithFlags(&n->lane_done[l], cudaEventDisableTiming));
+    }
     n->lane_cap = cap;
     return NET_OK;
 }
 
-// The lane of this stream, or of no stream yet; NULL when the batch is larger than the lanes
-// or every lane belongs to another stream (the launch then runs in caller order).
-int* pick_lane(net* n, cudaStream_t stream, int zones) {
-    if (zones > n->lane_cap) return nullptr;
-    std::lock_guard<std::mutex> lock(n->mu);
-    for (int l = 0; l < kLanes; ++l)
-        if (n->lane_used[l] && n->lane_stream[l] == stream) return n->lane_buf[l];
-    for (int l = 0; l < kLanes; ++l)
-        if (!n->lane_used[l]) {
-            n->lane_used[l] = true;
-            n->lane_stream[l] = stream;
-            return n->lane_buf[l];
+// Index of the lane this call may use, or -1 (the launch then runs in caller order: same bits).
+// Called with n->mu held.  The rule that keeps concurrency off a lane:
+//   * an eager call reuses the lane its stream used last (stream order serialises the two),
+//     else takes a lane nobody holds, else steals the least recently used eager lane whose
+//     last zone kernel has finished (lane_done, recorded by release_lane);
+//   * a call under stream capture gets a lane of its own per (capture, stream): the graph keeps
+//     pointers into it and may replay at any time, beside eager calls on the stream it was
+//     captured on and beside any other graph, so the lane is never handed out again.  No event
+//     query here: cudaEventQuery is not legal while a capture is under way.
+int pick_lane(net* n, cudaStream_t stream, int zones) {
+    if (zones > n->lane_cap) return -1;
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    unsigned long long id = 0;
+    if (cudaStreamGetCaptureInfo(stream, &st, &id) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return -1;
+    }
+    if (st == cudaStreamCaptureStatusInvalidated) return -1;
+    const bool capturing = (st == cudaStreamCaptureStatusActive);
+    int pick = -1;
+    for (int l = 0; l < kLanes && pick < 0; ++l)
+        if (n->lane_used[l] && n->lane_stream[l] == stream && n->lane_captured[l] == capturing &&
+            (!capturing || n->lane_capture[l] == id))
+            pick = l;
+    for (int l = 0; l < kLanes && pick < 0; ++l)
+        if (!n->lane_used[l]) pick = l;
+    if (pick < 0 && !capturing) {
+        for (int l = 0; l < kLanes; ++l) {
+            if (n->lane_captured[l] || (pick >= 0 && n->lane_tick[l] >= n->lane_tick[pick])) continue;
+            if (cudaEventQuery(n->lane_done[l]) == cudaSuccess) pick = l;
+            else (void)cudaGetLastError();  // cudaErrorNotReady: still running
         }
-    return nullptr;
+    }
+    if (pick < 0) return -1;
+    n->lane_used[pick] = true;
+    n->lane_stream[pick] = stream;
+    n->lane_captured[pick] = capturing;
+    n->lane_capture[pick] = id;
+    n->lane_tick[pick] = ++n->tick;
+    return pick;
 }
 
-// Enqueue the counting sort of the zones by falling T9; returns the order (device) or NULL.
-int enqueue_order(net* n, int zones, const double* T9, cudaStream_t stream, const int** order) {
+// Enqueue the counting sort of the zones by falling T9; returns the order (device) or NULL,
+// and the lane it lives in (-1 = none).  Called with n->mu held from the first operation on the
+// lane to release_lane behind the zone kernel, so that no other host thread can steal or share
+// the lane in between.
+int enqueue_order(net* n, int zones, const double* T9, cudaStream_t stream, const int** order, int* lane_out) {
     *order = nullptr;
+    *lane_out = -1;
     if (zones < kOrderMinZones) return NET_OK;  // fewer zones than a couple of waves
-    int* lane = pick_lane(n, stream, zones);
-    if (!lane) return NET_OK;
+    const int l = pick_lane(n, stream, zones);
+    if (l < 0) {
+        ++n->unsorted_calls;
+        return NET_OK;
+    }
+    int* lane = n->lane_buf[l];
     const int ctas = (zones + kOrderZonesPerCta - 1) / kOrderZonesPerCta;
     CUDA_TRY(cudaMemsetAsync(lane, 0, sizeof(int) * kLaneHeader, stream));
     zone_hist_kernel<<<ctas, kOrderThreads, 0, stream>>>(T9, zones, lane);
     zone_scatter_kernel<<<ctas, kOrderThreads, 0, stream>>>(T9, zones, lane, lane + kOrderBuckets,
                                                            lane + kLaneHeader);
     CUDA_TRY(cudaGetLastError());
+    ++n->sorted_calls;
     *order = lane + kLaneHeader;
+    *lane_out = l;
     return NET_OK;
+}
+
+// Behind the zone kernel that read the lane: an eager lane becomes stealable once this event
+// has completed.  A captured lane stays with its graph (and an event record would only add a
+// node to it).
+void release_lane(net* n, int l, cudaStream_t stream) {
+    if (l < 0 || n->lane_captured[l]) return;
+    if (cudaEventRecord(n->lane_done[l], stream) != cudaSuccess) (void)cudaGetLastError();
 }
 
 // Entry-point checks shared by everything that launches.
@@ -881,7 +935,10 @@ void net_destroy(net_t* n) {
         cudaFree(n->D.p_agg_ptr); cudaFree(n->D.p_agg_ent); cudaFree(n->D.bind);
         cudaFree(n->sT9); cudaFree(n->srho); cudaFree(n->sdt); cudaFree(n->sY);
         cudaFree(n->ssteps); cudaFree(n->sstatus);
-        for (int l = 0; l < kLanes; ++l) cudaFree(n->lane_buf[l]);
+        for (int l = 0; l < kLanes; ++l) {
+            cudaFree(n->lane_buf[l]);
+            if (n->lane_done[l]) cudaEventDestroy(n->lane_done[l]);
+        }
         for (cudaStream_t s : n->host_stream)
             if (s) cudaStreamDestroy(s);
     }
@@ -891,10 +948,28 @@ void net_destroy(net_t* n) {
 int net_reserve(net_t* n, int max_zones) {
     if (int rc = check_net(n)) return rc;
     if (max_zones < 0) return fail(NET_EINVAL, "max_zones < 0");
-    if (max_zones <= n->lane_cap) return NET_OK;
-    CUDA_TRY(cudaDeviceSynchronize());  // nothing in flight may still read the old workspaces
     std::lock_guard<std::mutex> lock(n->mu);
+    if (max_zones <= n->lane_cap) return NET_OK;
+    for (int l = 0; l < kLanes; ++l)
+        if (n->lane_captured[l])
+            return fail(NET_EINVAL,
+                        "net_reserve after a stream capture of net_integrate on this net_t: the captured "
+                        "graph holds pointers into the launch-order workspaces that would be freed; "
+                        "reserve before capturing");
+    CUDA_TRY(cudaDeviceSynchronize());  // nothing in flight may still read the old workspaces
     return alloc_lanes(n, max_zones);
+}
+
+int net_launch_stats(net_t* n, long long* sorted_calls, long long* unsorted_calls, int* lanes_pinned) {
+    if (!n) return fail(NET_EINVAL, "null net");
+    std::lock_guard<std::mutex> lock(n->mu);
+    if (sorted_calls) *sorted_calls = n->sorted_calls;
+    if (unsorted_calls) *unsorted_calls = n->unsorted_calls;
+    if (lanes_pinned) {
+        *lanes_pinned = 0;
+        for (int l = 0; l < kLanes; ++l) *lanes_pinned += n->lane_captured[l] ? 1 : 0;
+    }
+    return NET_OK;
 }
 
 int net_set_binding_energy(net_t* n, const double* B) {
@@ -924,8 +999,14 @@ int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rh
     if (!Y) return fail(NET_EINVAL, "null Y");
     if (!T9 || !rho) return fail(NET_EINVAL, "null T9/rho");
     if (!std::isfinite(t_hydro)) return fail(NET_EINVAL, "t_hydro is not finite");
+    // sorted launches: lane choice, order kernels, zone kernel and the lane's event are one
+    // host-side critical section per net_t (a few launches; nothing in it waits for the GPU)
+    std::unique_lock<std::mutex> lock(n->mu, std::defer_lock);
+    if (zones >= kOrderMinZones) lock.lock();
     const int* order = nullptr;
-    if (int rc = enqueue_order(n, zones, T9, static_cast<cudaStream_t>(stream), &order)) return rc;
+    int lane = -1;
+    if (int rc = enqueue_order(n, zones, T9, static_cast<cudaStream_t>(stream), &order, &lane)) return rc;
+    int rc;
     if (use_pull_kernel(n)) {
         KPull q;
         fill_pull(n, q);
@@ -934,15 +1015,18 @@ int net_integrate_energy(net_t* n, int zones, const double* T9, const double* rh
         q.t_hydro = t_hydro;
         q.bind = n->D.bind; q.energy = energy;
         q.order = order;
-        return launch_pull(n, zones, q, stream);
+        rc = launch_pull(n, zones, q, stream);
+    } else {
+        KParams k;
+        fill_params(n, k);
+        k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
+        k.t_hydro = t_hydro;
+        k.bind = n->D.bind; k.energy = energy;
+        k.order = order;
+        rc = launch<kAdaptive>(n, zones, k, stream);
     }
-    KParams k;
-    fill_params(n, k);
-    k.T9 = T9; k.rho = rho; k.Y = Y; k.dt = dt; k.n_steps = n_steps; k.status = status;
-    k.t_hydro = t_hydro;
-    k.bind = n->D.bind; k.energy = energy;
-    k.order = order;
-    return launch<kAdaptive>(n, zones, k, stream);
+    release_lane(n, lane, static_cast<cudaStream_t>(stream));
+    return rc;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -1037,6 +1121,8 @@ int net_integrate_fixed(net_t* n, int zones, const double* T9, const double* rho
     if (int rc = check_net(n)) return rc;
     if (zones > 0 && !Y) return fail(NET_EINVAL, "null Y");
     if (n_steps < 0 || n_steps > 2000000000LL) return fail(NET_EINVAL, "n_steps out of range [0, 2e9]");
+    if (!std::isfinite(dt_fixed) || !(dt_fixed > 0.0))
+        return fail(NET_EINVAL, "dt_fixed must be finite and > 0");
     if (use_pull_kernel(n)) {
         if (zones < 0) return fail(NET_EINVAL, "zones < 0");
         if (zones == 0) return NET_OK;
@@ -1091,14 +1177,27 @@ int net_rhs(net_t* n, int zones, const double* T9, const double* rho, const void
 //     when it ends (S6 out): one launch over the whole batch in the global hottest-first order,
 //     every transfer overlapped with the integration of the other zones, no staging copy.
 //   * Anything else (pageable memory): staged through net-owned device scratch in chunks over
-//     three internal streams (upload of chunk c, kernels of c-1 and download of c-2 overlap;
-//     the launch order then applies within a chunk).
+//     three internal streams; the launch order then applies within a chunk.  A copy between
+//     pageable memory and the device is not asynchronous to the host: the upload returns once
+//     the data sit in the driver's staging buffer, the download only when it has finished.  So
+//     the loop enqueues the upload and the kernels of chunk c BEFORE the download of chunk
+//     c-1: while the host thread sits in that download, the GPU already integrates chunk c, and
+//     the download of c-1 overlaps it.  (In the opposite order every chunk ran alone: upload,
+//     kernels, download, GPU idle during the copies.)  The call returns when all but the last
+//     download have finished, i.e. it is asynchronous only for pinned buffers.
 int net_integrate_host_async(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                              double t_hydro, double* dt, int* n_steps, int* status) {
     if (int rc = check_net(n)) return rc;
     if (zones < 0) return fail(NET_EINVAL, "zones < 0");
     if (zones == 0) return NET_OK;
     if (!T9 || !rho || !Y) return fail(NET_EINVAL, "null T9/rho/Y");
+    {
+        std::lock_guard<std::mutex> lock(n->mu);
+        if (n->host_in_flight)
+            return fail(NET_EINVAL, "net_integrate_host_async: a batch is in flight on this net_t "
+                                    "(its scratch and streams are shared): call net_wait first");
+        n->host_in_flight = true;  // until net_wait, also when this call fails half-way
+    }
     for (cudaStream_t& s : n->host_stream)
         if (!s) CUDA_TRY(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
     if (n->P.host_chunk >= 0) {  // < 0 forces the staged path
@@ -1131,7 +1230,19 @@ int net_integrate_host_async(net_t* n, int zones, const double* T9, const double
     const int chunk = n->P.host_chunk != 0
                           ? std::abs(n->P.host_chunk)
                           : std::max(kHostMinChunk, (zones + kHostMaxChunks - 1) / kHostMaxChunks);
-    int c = 0;
+    auto download = [&](int lo, int m, cudaStream_t s) -> int {
+        char* Yh = static_cast<char*>(Y) + ysz * lo;
+        char* Yd = static_cast<char*>(n->sY) + ysz * lo;
+        CUDA_TRY(cudaMemcpyAsync(Yh, Yd, ysz * m, cudaMemcpyDeviceToHost, s));
+        if (dt) CUDA_TRY(cudaMemcpyAsync(dt + lo, n->sdt + lo, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
+        if (n_steps)
+            CUDA_TRY(cudaMemcpyAsync(n_steps + lo, n->ssteps + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
+        if (status)
+            CUDA_TRY(cudaMemcpyAsync(status + lo, n->sstatus + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
+        return NET_OK;
+    };
+    int c = 0, prev_lo = -1, prev_m = 0;
+    cudaStream_t prev_s = nullptr;
     for (int lo = 0; lo < zones; lo += chunk, ++c) {
         const int m = std::min(chunk, zones - lo);
         cudaStream_t s = n->host_stream[c % kHostStreams];
@@ -1145,26 +1256,41 @@ int net_integrate_host_async(net_t* n, int zones, const double* T9, const double
         if (int rc = net_integrate(n, m, n->sT9 + lo, n->srho + lo, Yd, t_hydro, n->sdt + lo,
                                    n->ssteps + lo, n->sstatus + lo, s))
             return rc;
-        CUDA_TRY(cudaMemcpyAsync(Yh, Yd, ysz * m, cudaMemcpyDeviceToHost, s));
-        if (dt) CUDA_TRY(cudaMemcpyAsync(dt + lo, n->sdt + lo, sizeof(double) * m, cudaMemcpyDeviceToHost, s));
-        if (n_steps)
-            CUDA_TRY(cudaMemcpyAsync(n_steps + lo, n->ssteps + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
-        if (status)
-            CUDA_TRY(cudaMemcpyAsync(status + lo, n->sstatus + lo, sizeof(int) * m, cudaMemcpyDeviceToHost, s));
+        // chunk c is queued: now the download of chunk c-1 (which blocks the host for pageable
+        // buffers) cannot leave the GPU idle
+        if (prev_lo >= 0)
+            if (int rc = download(prev_lo, prev_m, prev_s)) return rc;
+        prev_lo = lo; prev_m = m; prev_s = s;
     }
+    if (prev_lo >= 0)
+        if (int rc = download(prev_lo, prev_m, prev_s)) return rc;
     return NET_OK;
 }
 
 int net_wait(net_t* n) {
     if (int rc = check_net(n)) return rc;
+    cudaError_t first = cudaSuccess;
     for (cudaStream_t s : n->host_stream)
-        if (s) CUDA_TRY(cudaStreamSynchronize(s));
+        if (s) {
+            const cudaError_t e = cudaStreamSynchronize(s);
+            if (first == cudaSuccess) first = e;
+        }
+    {
+        std::lock_guard<std::mutex> lock(n->mu);
+        n->host_in_flight = false;
+    }
+    if (first != cudaSuccess) return fail(NET_ECUDA, std::string("net_wait: ") + cudaGetErrorString(first));
     return NET_OK;
 }
 
 int net_integrate_host(net_t* n, int zones, const double* T9, const double* rho, void* Y,
                        double t_hydro, double* dt, int* n_steps, int* status) {
-    if (int rc = net_integrate_host_async(n, zones, T9, rho, Y, t_hydro, dt, n_steps, status)) return rc;
+    if (int rc = net_integrate_host_async(n, zones, T9, rho, Y, t_hydro, dt, n_steps, status)) {
+        const std::string keep = g_last_error;  // drain what was enqueued, report the first error
+        if (n && n->has_device && keep.find("a batch is in flight") == std::string::npos) net_wait(n);
+        g_last_error = keep;
+        return rc;
+    }
     return net_wait(n);
 }
 

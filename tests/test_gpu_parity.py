@@ -443,6 +443,45 @@ def test_max_steps_status(g16):
     assert g["status"][0] == K.NET_STATUS_MAX_STEPS == ref["status"][0]
 
 
+@pytest.mark.parametrize("kernel", [0, 2, 1])
+def test_nonfinite_status_bit(hub150, kernel):
+    """include/kinnet.h NET_STATUS_NONFINITE (what the kernel hands back; SURVEY
+    8(b) status bits).  A zone with T9 = -1 has ln T9 = NaN in every rate with a6 != 0: every flux
+    is NaN, a NaN candidate never wins the dt minimum, so the zone takes one step of the whole
+    t_hydro, reports dt = growth * t_hydro, NaN abundances and status 2 -- on the oracle
+    (tests/test_oracle_pins.py::test_nonfinite_status_bit_worked_by_hand) and on every kernel.  The
+    zones beside it in the batch are bit for bit what they are without it."""
+    c = build_config(3, zones=9)
+    kn, o = K.Net(hub150, K.NetParams(kernel=kernel)), Oracle(hub150)
+    good = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
+    T9 = c["T9"].copy()
+    T9[[2, 7]] = [-1.0, np.nan]
+    g = gpu_integrate(kn, T9, c["rho"], c["Y0"], c["t_hydro"])
+    ref = o.integrate(T9, c["rho"], c["Y0"], c["t_hydro"])
+    assert ref["status"].tolist() == [0, 0, 2, 0, 0, 0, 0, 2, 0]
+    assert g["status"].tolist() == ref["status"].tolist()
+    for z in (2, 7):
+        assert g["n_steps"][z] == ref["n_steps"][z] == 1
+        assert g["dt"][z] == ref["dt"][z] == 2.0 * c["t_hydro"]
+        assert np.array_equal(np.isnan(g["Y"][z]), np.isnan(ref["Y"][z])) and np.isnan(g["Y"][z]).any()
+    for z in (0, 1, 3, 4, 5, 6, 8):
+        for key in ("Y", "dt", "n_steps", "status"):
+            assert np.array_equal(g[key][z], good[key][z]), (z, key)
+
+
+def test_integrate_fixed_rejects_a_bad_step(g16):
+    kn = K.Net(g16)
+    c = build_config(1)
+    Y = dev(c["Y0"])
+    before = Y.clone()
+    for bad in (0.0, -1e-10, float("nan"), float("inf")):
+        with pytest.raises(K.KinnetError) as e:
+            kn.net_integrate_fixed(1, dev(c["T9"]), dev(c["rho"]), Y, bad, 10)
+        assert e.value.code == K.NET_EINVAL and "dt_fixed" in str(e.value)
+    torch.cuda.synchronize()
+    assert torch.equal(Y, before)
+
+
 def test_bitwise_run_to_run_determinism(hub150):
     """Fixed schedule, no atomics: two runs must agree bit for bit."""
     c = build_config(3)
@@ -533,6 +572,94 @@ def test_one_net_two_streams(hub150):
         assert torch.equal(got, ref)
 
 
+def test_two_graphs_of_one_net_replay_concurrently(hub150):
+    """include/kinnet.h "Conventions": a captured call gets a launch-order lane of its own per
+    capture.  torch.cuda.graph captures every graph on the same capture stream, so lanes keyed by
+    stream alone would give both graphs (and eager calls on that stream) ONE lane; replayed side by
+    side on two streams, one graph's order kernels would then rewrite the order the other's zone
+    kernel is reading, and zones would be skipped or run twice.  Two graphs over disjoint halves of
+    the batch, replayed together three times with an eager call of a third range beside them, return
+    the eager single-call bits; the net_t reports two pinned lanes and refuses net_reserve."""
+    z, h = 6144, 2048
+    c = build_config(4, zones=z)
+    kn = K.Net(hub150)
+    T9, rho, Y, dt, steps, status = _state(c, z)
+    kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status)
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (Y, dt, steps, status)]
+    Y0 = dev(c["Y0"])
+    graphs = []
+    for lo in (0, h):
+        sl = slice(lo, lo + h)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            kn.net_integrate(h, T9[sl], rho[sl], Y[sl], c["t_hydro"], dt[sl], steps[sl], status[sl])
+        graphs.append(g)
+    assert kn.net_launch_stats()["lanes_pinned"] == 2
+    s1, s2, s3 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    sl3 = slice(2 * h, 3 * h)
+    for _ in range(3):
+        Y.copy_(Y0)
+        dt.zero_()
+        steps.zero_()
+        status.fill_(-1)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s1):
+            graphs[0].replay()
+        with torch.cuda.stream(s2):
+            graphs[1].replay()
+        kn.net_integrate(h, T9[sl3], rho[sl3], Y[sl3], c["t_hydro"], dt[sl3], steps[sl3], status[sl3], s3)
+        torch.cuda.synchronize()
+        for got, ref in zip((Y, dt, steps, status), want):
+            assert torch.equal(got, ref)
+    st = kn.net_launch_stats()
+    assert st["unsorted_calls"] == 0 and st["sorted_calls"] >= 6
+    with pytest.raises(K.KinnetError) as e:  # the graphs hold pointers into the lanes
+        kn.net_reserve(100_000)
+    assert e.value.code == K.NET_EINVAL and "capture" in str(e.value)
+    graphs[0].replay()  # still valid
+    torch.cuda.synchronize()
+
+
+def test_launch_order_lanes_are_recycled(hub150):
+    """Streams come and go (a fresh stream per hydro step, a stream pool): more distinct streams
+    than the net_t has lanes must keep the hottest-first launch -- a lane whose last zone kernel
+    has finished is handed on.  40 fresh streams in turn, then 20 at once (no lane can be stolen
+    while its kernel runs: those that find none fall back to caller order, same bits)."""
+    z = 1024
+    c = build_config(4, zones=z)
+    kn = K.Net(hub150)
+    T9, rho, Y, dt, steps, status = _state(c, z)
+    kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status)
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (Y, dt, steps, status)]
+    base = kn.net_launch_stats()
+    assert base == {"sorted_calls": 1, "unsorted_calls": 0, "lanes_pinned": 0}
+    Y0 = dev(c["Y0"])
+    for _ in range(40):
+        s = torch.cuda.Stream()
+        Y.copy_(Y0)
+        dt.zero_()
+        torch.cuda.synchronize()
+        kn.net_integrate(z, T9, rho, Y, c["t_hydro"], dt, steps, status, s)
+        torch.cuda.synchronize()
+        for got, ref in zip((Y, dt, steps, status), want):
+            assert torch.equal(got, ref)
+    st = kn.net_launch_stats()
+    assert st["sorted_calls"] == 41 and st["unsorted_calls"] == 0
+    states = [_state(c, z) for _ in range(20)]
+    streams = [torch.cuda.Stream() for _ in range(20)]
+    torch.cuda.synchronize()
+    for stt, s in zip(states, streams):
+        kn.net_integrate(z, *stt[:3], c["t_hydro"], *stt[3:], s)
+    torch.cuda.synchronize()
+    for stt in states:
+        for got, ref in zip(stt[2:], want):
+            assert torch.equal(got, ref)
+    st = kn.net_launch_stats()
+    assert st["sorted_calls"] + st["unsorted_calls"] == 61 and st["sorted_calls"] >= 41 + 16
+
+
 def test_tensor_memory_kernels_share_the_sms():
     """Three zone kernels with different tensor-memory footprints (fp64 hub150: 128 columns per CTA,
     fp32 hub150: 64, fp64 hub365: 256) on three streams at once, each batch large enough to fill the
@@ -605,6 +732,9 @@ def test_host_entry_points_match_device_path(hub150, zones, host_chunk):
     kn.net_integrate_host_async(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"], dt.numpy(),
                                 steps.numpy(), status.numpy())
     busy = float(np.linalg.norm(np.random.default_rng(0).standard_normal((300, 300)) @ np.eye(300)))
+    with pytest.raises(K.KinnetError) as e:  # one batch in flight per net_t: refused, nothing touched
+        kn.net_integrate_host_async(z, T9.numpy(), rho.numpy(), Y.numpy(), c["t_hydro"])
+    assert e.value.code == K.NET_EINVAL and "in flight" in str(e.value)
     kn.net_wait()
     assert busy > 0 and (Y.numpy() == a["Y"]).all() and (steps.numpy() == a["n_steps"]).all()
     assert (dt.numpy() == a["dt"]).all() and (status.numpy() == 0).all()
