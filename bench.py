@@ -34,6 +34,7 @@ PROFILE_SEED = 4
 # exact configuration; any other run reports null.
 DRAM_BYTES_PER_LAUNCH = 20477184
 DRAM_BYTES_SOURCE = "profiles/r02d_pull2_kernel.md"
+SURVEY_FP64_PER_ZONE_SUBSTEP = 13000  # SURVEY.md 8(d), 150 species / 1604 reactions
 
 # Algorithmic work per zone per sub-step: one multiply per
 # reactant of every reaction, one add per F+/F- entry, ~10 flops per species for
@@ -123,9 +124,11 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU, name: str = "hub150"):
+def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU, name: str = "hub150",
+             shard: str = "contiguous"):
     """Weak scaling: the global batch is world x 16384 zones of one seeded profile;
-    rank r integrates the contiguous shard r (no data-path collective)."""
+    rank r integrates the contiguous shard r, or with shard = "t9" the zones dealt to it by
+    falling temperature (shard.zone_shard_balanced); no data-path collective either way."""
     from gen import perturbed_co_start, zone_profile
     from gen.configs import network
 
@@ -134,11 +137,14 @@ def workload(rank: int, world: int, zones_per_gpu: int = ZONES_PER_GPU, name: st
     if world == 1:  # (the reference arm comes through here: it must not load the product library)
         lo, hi = 0, total
     else:
-        from paper_1409_5826_b200.shard import zone_shard
+        from paper_1409_5826_b200.shard import zone_shard, zone_shard_balanced
 
         lo, hi = zone_shard(total, rank, world)
     T9, rho = zone_profile(total, PROFILE_SEED)
     Y0 = perturbed_co_start(net, total, seed=1000 + PROFILE_SEED)
+    if world > 1 and shard == "t9":
+        idx = zone_shard_balanced(T9, rank, world)
+        return net, T9[idx].copy(), rho[idx].copy(), Y0[idx].copy()
     return net, T9[lo:hi].copy(), rho[lo:hi].copy(), Y0[lo:hi].copy()
 
 
@@ -234,7 +240,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
 
-    net, T9h, rhoh, Y0h = workload(rank, world, args.zones, args.network)
+    net, T9h, rhoh, Y0h = workload(rank, world, args.zones, args.network, args.shard)
     z, N = Y0h.shape
     method = {"asymptotic": 0, "qss": 1}[args.method]
     kn = K.Net(net, K.NetParams(precision=args.precision, kernel=args.kernel, method=method))
@@ -371,6 +377,63 @@ def run_ours(args):
                             "ns_per_zone_substep": best5 * 1e6 / sub5,
                             "kernel": k5.schedule_info()["kernel"], "threads_per_zone": k5.schedule_info()["threads"]}
 
+        # the secondary claims on the configs[3] batch itself, one launch each, best of 3 (VERDICT r02
+        # item 5: a regression on any of them must show in the driver's line)
+        def variant(label, what, network_name="hub150", **params):
+            vnet, Yvh = (net, Y0h) if network_name == "hub150" else workload(0, 1, z, network_name)[::3]
+            prec = params.get("precision", 64)
+            kv = K.Net(vnet, K.NetParams(**params))
+            Yv0 = torch.from_numpy(np.ascontiguousarray(Yvh.astype(np.float64 if prec == 64 else np.float32))).to(dev)
+            Yv, dtv = torch.empty_like(Yv0), torch.zeros(z, dtype=torch.float64, device=dev)
+            stv = torch.zeros(z, dtype=torch.int32, device=dev)
+            sv = torch.zeros(z, dtype=torch.int32, device=dev)
+            best = None
+            for it in range(3):
+                Yv.copy_(Yv0)
+                dtv.zero_()
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                kv.net_integrate(z, T9, rho, Yv, T_HYDRO, dtv, stv, sv, stream)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                best = ms if best is None else min(best, ms)
+            sub = int(stv.sum().item())
+            vi = kv.schedule_info()
+            extra[label] = {"what": what + f", {z} zones, one hydro step (best of 3)", "ms": best,
+                            "zone_networks_per_s": z / (best * 1e-3), "sub_steps": sub,
+                            "ns_per_zone_substep": best * 1e6 / sub, "kernel": vi["kernel"],
+                            "threads_per_zone": vi["threads"], "status_max": int(sv.max().item())}
+            kv.close()
+
+        variant("hub150hh", "hub150 + 16 heavy + heavy fusion pairs and inverses (N-slots)", "hub150hh")
+        variant("qss", "QSS variant of the update (net_params_t.method = 1)", method=1)
+        variant("fp32", "single-precision study (PAPER.md L132)", precision=32)
+        variant("kernel2", "forced one-species-per-thread pull kernel (params.kernel = 2)", kernel=2)
+        variant("kernel1", "forced generic flux-array kernel (params.kernel = 1)", kernel=1)
+
+        # pageable host buffers through the staged pipeline in 4 chunks (kinnet.h: upload and kernels
+        # of chunk c are enqueued before the blocking download of chunk c-1)
+        kn_page = K.Net(net, K.NetParams(host_chunk=-(z // 4)))
+        best_p = None
+        for it in range(3):
+            Ypg, dtpg = Y0h.copy(), np.zeros(z)
+            stpg, sspg = np.zeros(z, np.int32), np.zeros(z, np.int32)
+            flush.zero_()
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            kn_page.net_integrate_host(z, T9h, rhoh, Ypg, T_HYDRO, dtpg, stpg, sspg)
+            el = time.perf_counter() - t1
+            if it > 0:
+                best_p = el if best_p is None else min(best_p, el)
+        assert int(sspg.max()) == 0 and int(stpg.sum()) == substeps
+        extra["host_pageable_4chunks"] = {
+            "what": "net_integrate_host on PAGEABLE numpy buffers, staged path in 4 chunks of "
+                    f"{z // 4} zones over three streams (host wall clock, best of 2 after one warm-up)",
+            "ms": best_p * 1e3, "zone_networks_per_s": z / best_p}
+        kn_page.close()
+
     # ---- max over ranks ---------------------------------------------------
     from paper_1409_5826_b200.shard import reduce_job
 
@@ -414,7 +477,8 @@ def run_ours(args):
             "sub_steps_per_zone": {"min": int(steps_host.min()), "median": float(np.median(steps_host)),
                                    "p99": float(np.percentile(steps_host, 99)), "max": int(steps_host.max())},
             "l2": "256 MB buffer written between timed iterations (L2 flush)",
-            "parallelism": f"zones sharded contiguously over {world} GPU(s), no collective",
+            "parallelism": (f"zones sharded contiguously over {world} GPU(s), no collective" if args.shard == "contiguous"
+                            else f"zones dealt by falling T9 over {world} GPU(s) (zone_shard_balanced), no collective"),
             "threads_per_zone": info["threads"], "zones_per_sm": info["zones_per_sm"],
         },
         "ms_per_step_best": best_ms, "ms_per_step_median": median_ms,
@@ -435,6 +499,12 @@ def run_ours(args):
         "roofline": {
             "bound": "alu", "kernel": kname, "achieved": fp64_ach,
             "peak": fp64_peak, "unit": "Tinstr/s", "frac": fp64_ach / fp64_peak, "traffic": traffic,
+            "traffic_source": (f"constant from the ncu capture in {DRAM_BYTES_SOURCE}, not measured by this run"
+                               if default_run else None),
+            # SURVEY 8(d) quotes ~13 k FP64 instructions per zone-substep for the 150/1604 network; the
+            # count above is the stricter one this file derives from the tables
+            "frac_survey_count": (SURVEY_FP64_PER_ZONE_SUBSTEP * per_launch_substeps / (k_ms * 1e-3) / 1e12 / fp64_peak
+                                  if args.network == "hub150" else None),
             "what": f"{flops} algorithmic FP64 instructions (FMA = 1) per zone-substep x {per_launch_substeps} "
                     f"zone-substeps per launch / {k_ms:.2f} ms; peak = FP64 issue rate, {peak_src}; "
                     f"traffic = dram bytes of one launch from the ncu capture in {DRAM_BYTES_SOURCE}"
@@ -538,6 +608,8 @@ def main():
     ap.add_argument("--method", default="asymptotic", choices=["asymptotic", "qss"],
                     help="qss = the explicit quasi-steady-state variant of the update (PAPER.md L217-219, "
                          "DESIGN.md reading Q20); the metric is quoted on the paper's asymptotic method")
+    ap.add_argument("--shard", default="contiguous", choices=["contiguous", "t9"],
+                    help="N > 1: contiguous zone ranges, or zones dealt to ranks by falling T9 (balanced step counts)")
     ap.add_argument("--sweep", choices=["zones", "size"],
                     help="SURVEY 8(f) NEXT 1: saturation curve over the zone count (Fig. 8 analogue) or "
                          "time per sub-step over the network size (Fig. 6a analogue); one JSON line per point")
