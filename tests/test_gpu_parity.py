@@ -161,6 +161,12 @@ def oracle_with_arbiter(net, T9, rho, Y0, t_hydro, dt=None, seeds=(101, 202), pa
 ARBITER_FACTOR = 4.0
 
 
+def say(capsys, *a):
+    """Into the driver's log, past pytest's capture: the arbitration figures are evidence."""
+    with capsys.disabled():
+        print("\n[parity]", *a)
+
+
 def check_adaptive(g, ref, arbiter, A, label="", min_direct=0.75, positive=True):
     """north_star: mass fractions above 1e-12 within 1e-6 of the oracle, step counts within
     1 %.  Every zone must either meet that directly against the fp64 oracle, or -- DESIGN.md
@@ -186,24 +192,50 @@ def check_adaptive(g, ref, arbiter, A, label="", min_direct=0.75, positive=True)
     np.testing.assert_allclose(g["dt"][m], ref["dt"][m], rtol=1e-6)
     arbitrated = ~direct
     ratio = err_a[arbitrated] / np.maximum(e_o[arbitrated], ADAPT_TOL / ARBITER_FACTOR)
-    return dict(zones=int(err.size), max_err_direct=float(err[direct].max()) if direct.any() else 0.0,
+    check_adaptive.last_arbitrated = np.nonzero(arbitrated)[0]
+    return dict(zones=int(err.size), direct_frac=float(direct.mean()),
+                max_err_direct=float(err[direct].max()) if direct.any() else 0.0,
                 n_arbitrated=int(arbitrated.sum()),
                 worst_gpu_vs_arbiter=float(err_a[arbitrated].max()) if arbitrated.any() else 0.0,
                 worst_oracle_vs_arbiter=float(e_o.max()),
                 worst_ratio=float(ratio.max()) if arbitrated.any() else 0.0)
 
 
-def test_config2_adaptive_long(hub150):
+def without_dt_feedback(kn, o, T9, rho, Y0, t_hydro, n_steps, A, zones):
+    """the zones check_adaptive sends to the arbiter, run again with the
+    feedback cut.  Zone z takes exactly n_steps[z] sub-steps (the count of its adaptive run) of
+    the FIXED size t_hydro / n_steps[z] (its mean adaptive dt) on the GPU and on the oracle.
+    Without the controller a rounding difference cannot change dt, so the north_star's fixed-dt
+    bar (1e-9 on mass fractions above 1e-12) must hold on exactly these zones: that separates
+    "dt feedback amplified an ulp" from "the kernel is off on this zone".  Returns the worst
+    error; the caller asserts."""
+    worst = 0.0
+    for z in zones:
+        n = int(n_steps[z])
+        dt = t_hydro / n
+        ref = o.integrate_fixed(T9[z], rho[z], Y0[z:z + 1], dt, n)
+        Yg = gpu_fixed(kn, T9[z:z + 1], rho[z:z + 1], Y0[z:z + 1], dt, n)
+        assert np.isfinite(ref["Y"]).all() and np.isfinite(Yg).all(), z
+        err, _ = max_rel_err(Yg, ref["Y"], A)
+        worst = max(worst, err)
+    return worst
+
+
+def test_config2_adaptive_long(hub150, capsys):
     c = build_config(2)
-    kn = K.Net(hub150)
+    kn, o = K.Net(hub150), Oracle(hub150)
     ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     assert ref["n_steps"][0] > 10_000
     # one zone, ~29 000 sub-steps: the fp64 oracle itself sits ~3e-7 from the arbiter
-    print("config2", check_adaptive(g, ref, arb, hub150.A, "config2", min_direct=0.0))
+    say(capsys, "config2", check_adaptive(g, ref, arb, hub150.A, "config2", min_direct=0.0))
+    # the same zone over the same number of steps with the feedback cut, arbitrated or not
+    w = without_dt_feedback(kn, o, c["T9"], c["rho"], c["Y0"], c["t_hydro"], ref["n_steps"], hub150.A, [0])
+    say(capsys, f"config2 without dt feedback ({int(ref['n_steps'][0])} fixed steps): max rel err {w:.2e}")
+    assert w <= FIXED_TOL
 
 
-def test_config3_operator_split_carry_dt(hub150):
+def test_config3_operator_split_carry_dt(hub150, capsys):
     """10 consecutive hydro steps, dt[] carried call to call.  Each call starts
     GPU and oracle from the same (oracle) state so that a call is judged on its
     own; the fully chained GPU trajectory is checked for sanity at the end."""
@@ -214,7 +246,7 @@ def test_config3_operator_split_carry_dt(hub150):
     for call in range(c["calls"]):
         ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], Yo, c["t_hydro"], dto)
         g = gpu_integrate(kn, c["T9"], c["rho"], Yo, c["t_hydro"], dt=dto)
-        print("config3 call", call, check_adaptive(g, ref, arb, hub150.A, f"config3 call {call}"))
+        say(capsys, "config3 call", call, check_adaptive(g, ref, arb, hub150.A, f"config3 call {call}"))
         chained = gpu_integrate(kn, c["T9"], c["rho"], Yg, c["t_hydro"], dt=dtg)
         Yg, dtg = chained["Y"], chained["dt"]
         Yo, dto = ref["Y"], ref["dt"]
@@ -223,34 +255,57 @@ def test_config3_operator_split_carry_dt(hub150):
     assert np.abs((Yg * hub150.A).sum(axis=1) - (Yo * hub150.A).sum(axis=1)).max() < 1e-4
 
 
-def test_config4_full_batch_sampled(hub150):
-    """16384 zones in the launch configuration bench.py times; the oracle checks
-    a seeded sample of 256 zones that includes the 16 longest-running."""
+CONFIG4_MIN_DIRECT = 0.999  # seen: 16381 of 16384 (0.9998), every step count identical
+
+
+def test_config4_full_batch_every_zone(hub150, capsys):
+    """16384 zones in the launch configuration bench.py times, EVERY zone against the fp64
+    oracle (all host cores: ~15 s).  A zone passes directly at 1e-6 / 1 % of the step count; the
+    misses, the 16 longest-running zones and a seeded sample of 64 more go through the
+    long-double arbiter rule of check_adaptive, and the misses are run again without dt feedback
+    (fixed dt, same step count), where 1e-9 must hold."""
     c = build_config(4)
-    kn = K.Net(hub150)
+    kn, o = K.Net(hub150), Oracle(hub150)
     g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     assert (g["status"] == 0).all()
     X = g["Y"] * hub150.A
     assert (g["Y"] >= 0).all() and np.abs(X.sum(axis=1) - 1).max() < 1e-2
+    full = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], n_threads=max_threads())
+    assert (full["status"] == 0).all()
+    err = zone_err(g["Y"], full["Y"], hub150.A)
+    ds = np.abs(g["n_steps"] - full["n_steps"])
+    direct = (err <= ADAPT_TOL) & (ds <= np.maximum(1, full["n_steps"] // 100))
+    miss = np.nonzero(~direct)[0]
+    say(capsys, f"config4 all {c['zones']} zones vs the fp64 oracle: direct {direct.mean():.4f} "
+                f"({miss.size} to the arbiter), max err among direct {err[direct].max():.2e}, "
+                f"median err {np.median(err):.2e}, identical step counts {float((ds == 0).mean()):.4f}")
+    assert direct.mean() >= CONFIG4_MIN_DIRECT
     rng = np.random.default_rng(44)
-    longest = np.argsort(g["n_steps"])[-16:]
-    rest = rng.choice(c["zones"], 240, replace=False)
-    idx = np.unique(np.concatenate([longest, rest]))
+    idx = np.unique(np.concatenate([miss, np.argsort(g["n_steps"])[-16:], rng.choice(c["zones"], 64, replace=False)]))
     ref, arb = oracle_with_arbiter(hub150, c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"])
-    print("config4", check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, hub150.A, "config4"))
+    say(capsys, "config4 misses + longest + sample",
+        check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, hub150.A, "config4", min_direct=0.0))
+    w = without_dt_feedback(kn, o, c["T9"], c["rho"], c["Y0"], c["t_hydro"], full["n_steps"], hub150.A, miss[:64])
+    say(capsys, f"config4 arbitrated zones without dt feedback ({min(miss.size, 64)} zones): max rel err {w:.2e}")
+    assert w <= FIXED_TOL
 
 
-def test_config5_large_network_sampled():
+def test_config5_large_network_sampled(capsys):
     c = build_config(5)
     net = c["network"]
-    kn = K.Net(net)
+    kn, o = K.Net(net), Oracle(net)
     g = gpu_integrate(kn, c["T9"], c["rho"], c["Y0"], c["t_hydro"])
     assert (g["status"] == 0).all()
     rng = np.random.default_rng(55)
     idx = np.unique(np.concatenate([np.argsort(g["n_steps"])[-4:],
                                     rng.choice(c["zones"], 60, replace=False)]))
     ref, arb = oracle_with_arbiter(net, c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"])
-    print("config5", check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, net.A, "config5"))
+    say(capsys, "config5", check_adaptive({k: v[idx] for k, v in g.items()}, ref, arb, net.A, "config5"))
+    zones = check_adaptive.last_arbitrated
+    w = without_dt_feedback(kn, o, c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"], ref["n_steps"], net.A,
+                            zones)
+    say(capsys, f"config5 arbitrated zones without dt feedback ({len(zones)} zones): max rel err {w:.2e}")
+    assert w <= FIXED_TOL
 
 
 def test_every_kernel_on_a_pull_network(hub150):
@@ -769,6 +824,64 @@ def test_fp32_variant_report(hub150, capsys):
               f"{o32['n_steps'].sum()}/{o64['n_steps'].sum()}")
     assert np.median(dev_gpu) < 1e-3 and dev_gpu.max() < 0.2
     assert abs(int(g32["n_steps"].sum()) - int(o32["n_steps"].sum())) < 0.05 * o32["n_steps"].sum()
+    # the same report on the configuration BASELINE.json asks it for (configs[3]: "Run in both fp64
+    # and fp32"): the full 16384-zone launch in fp32, deviations on a seeded sample of 256 zones
+    c = build_config(4)
+    g32 = gpu_integrate(kn32, c["T9"], c["rho"], c["Y0"], c["t_hydro"], precision=32)
+    assert (g32["status"] == 0).all()
+    idx = np.sort(np.random.default_rng(432).choice(c["zones"], 256, replace=False))
+    o32 = o.integrate(c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"], precision=32, n_threads=max_threads())
+    o64 = o.integrate(c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"], n_threads=max_threads())
+    m = (o64["Y"] * hub150.A) > X_MIN
+    dev_gpu = np.abs(g32["Y"][idx][m] / o64["Y"][m] - 1)
+    dev_cpu = np.abs(o32["Y"][m].astype(np.float64) / o64["Y"][m] - 1)
+    with capsys.disabled():
+        print(f"[fp32 study, config 4 sample of 256] GPU fp32 vs oracle fp64: median {np.median(dev_gpu):.2e} "
+              f"max {dev_gpu.max():.2e}; oracle fp32 vs fp64: median {np.median(dev_cpu):.2e} "
+              f"max {dev_cpu.max():.2e}; steps gpu32/cpu32/cpu64 = {g32['n_steps'][idx].sum()}/"
+              f"{o32['n_steps'].sum()}/{o64['n_steps'].sum()}")
+    assert np.median(dev_gpu) < 1e-3 and dev_gpu.max() < 0.2
+    assert abs(int(g32["n_steps"][idx].sum()) - int(o32["n_steps"].sum())) < 0.05 * o32["n_steps"].sum()
+
+
+FP32_U = 2.0 ** -24
+
+
+@pytest.mark.parametrize("case", ["config1", "hub150"])
+def test_fp32_fixed_dt_against_the_fp32_oracle(hub150, case, capsys):
+    """The single-precision study with the dt feedback cut: GPU fp32 against
+    the oracle's fp32 twin over the same n fixed steps.  The paper fixes no bound; the one
+    asserted is derived in DESIGN.md 5 from the arithmetic: both sides evaluate the same update in
+    fp32, each step rounds every abundance a bounded number of times (relative error c u,
+    u = 2^-24), and with no controller the differences of the two evaluation orders add up at
+    most linearly: |GPU - oracle| / oracle <= 8 n u on mass fractions above 1e-12 (measured: a
+    few u sqrt(n), printed).  The fp64 GPU result is printed beside it as the precision
+    comparison itself."""
+    if case == "config1":
+        c = build_config(1)
+        net, T9, rho, Y0, dt, n = c["network"], c["T9"], c["rho"], c["Y0"], 1e-10, 2000
+    else:
+        rng = np.random.default_rng(21)
+        z = 7
+        net, T9, rho = hub150, rng.uniform(2, 9, z), 10 ** rng.uniform(7, 9.5, z)
+        Y0 = np.zeros((z, 150))
+        Y0[:, 3], Y0[:, 15] = 0.5 / 12, 0.5 / 16
+        dt, n = 1e-9, 400
+    o = Oracle(net)
+    kn32, kn64 = K.Net(net, K.NetParams(precision=32)), K.Net(net)
+    ref32 = o.integrate_fixed(T9, rho, Y0, dt, n, precision=32)["Y"].astype(np.float64)
+    ref64 = o.integrate_fixed(T9, rho, Y0, dt, n)["Y"]
+    g32 = gpu_fixed(kn32, T9, rho, Y0, dt, n, precision=32)
+    g64 = gpu_fixed(kn64, T9, rho, Y0, dt, n)
+    m = ref64 * net.A > X_MIN
+    e32 = np.abs(g32[m] / ref32[m] - 1)
+    p32 = np.abs(g32[m] / ref64[m] - 1)
+    e64 = np.abs(g64[m] / ref64[m] - 1)
+    say(capsys, f"fp32 fixed dt, {case}, n = {n}: GPU32 vs oracle32 max {e32.max():.2e} "
+                f"(= {e32.max() / FP32_U:.1f} u, bound {8 * n} u), median {np.median(e32):.2e}; GPU32 vs oracle64 "
+                f"max {p32.max():.2e}; GPU64 vs oracle64 max {e64.max():.2e}")
+    assert e32.max() <= 8 * n * FP32_U
+    assert e64.max() <= FIXED_TOL
 
 
 # ------------------------------------------- every block-size class of the pull kernel
@@ -842,9 +955,16 @@ def test_energy_release_parity(hub150, kernel):
     ref = Oracle(hub150).integrate(c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"],
                                    n_threads=max_threads())
     Eo = Oracle.energy(B, c["Y0"][idx], ref["Y"])
-    same = steps.cpu().numpy()[idx] == ref["n_steps"]  # zones both sides stepped identically
-    assert same.mean() > 0.9
-    assert (np.abs(Eg[idx] - Eo)[same] <= 1e-6 * scale[idx][same]).all()
+    # every sampled zone: directly within the adaptive tolerance of the oracle's energy, or -- the
+    # rule of check_adaptive -- no further from the long-double arbiter's than 4x the oracle is
+    arb = Oracle(hub150).integrate(c["T9"][idx], c["rho"][idx], c["Y0"][idx], c["t_hydro"],
+                                   n_threads=max_threads(), precision=80)
+    Ea = Oracle.energy(B, c["Y0"][idx], arb["Y"])
+    tol = ADAPT_TOL * scale[idx]
+    direct = np.abs(Eg[idx] - Eo) <= tol
+    by_arbiter = np.abs(Eg[idx] - Ea) <= np.maximum(tol, ARBITER_FACTOR * np.abs(Eo - Ea))
+    assert direct.mean() > 0.9
+    assert (direct | by_arbiter).all(), np.nonzero(~(direct | by_arbiter))[0]
     assert (Eg != 0).all()  # (the sign is a property of the synthetic rates and table, not asserted)
 
 
