@@ -334,3 +334,12 @@ def test_staircase_class_of_the_two_species_schedule():
     # class must say so, whatever its slot counts would allow
     assert seen["hub365"] == 0 and K.Net(network("hub365"), host_only=True).schedule_info()["threads"] == 192
     assert K.Net(network("g16"), host_only=True).schedule_info()["pull_stair"] == 0
+    # negative case inside the eligible block sizes: the 250-species network runs 128 threads, but a
+    # side-a row overflows its warp's step -> class 0 (recomputed from the tables above)
+    from gen import make_hub_network
+
+    kn = K.Net(make_hub_network(250, 2900, seed=250), host_only=True)
+    info = kn.schedule_info()
+    assert info["kernel"] == 2 and info["threads"] == 128 and info["pull_stair"] == 0 == want(kn, info)
+    n = kn.schedule_table("pull_n_slots")
+    assert any(n[t] > max(24 - 4 * (t // 32), 12) for t in range(32 * (info["pull_threads"] // 64)))

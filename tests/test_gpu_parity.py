@@ -903,6 +903,12 @@ def test_pull_kernel_block_size_classes(N, M, kernel, runs, threads):
     kn, o = K.Net(net, K.NetParams(kernel=kernel)), Oracle(net)
     info = kn.schedule_info()
     assert info["kernel"] == runs and info["threads"] == threads, info
+    if runs == 2:
+        # the staircase (a copy of the sub-step loop per warp) only where the schedule fits it:
+        # N = 96, 150 fit; N = 250 is the negative case -- 128 threads, eligible by block size, but a
+        # side-a row longer than its warp's step, so class 0: every warp runs the full capacities and
+        # the parity below must hold all the same; 160/192 threads never use it
+        assert (info["pull_stair"] != 0) == (N in (96, 150)), info
     z = 5
     T9, rho = zone_profile(z, 77)
     Y0 = co_start(net, z)
