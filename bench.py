@@ -32,8 +32,8 @@ PROFILE_SEED = 4
 # workload, from the `ncu --set full` capture summarised in the file named beside it (the
 # writes of the last zones are still in L2 when the capture ends).  Reported only for that
 # exact configuration; any other run reports null.
-DRAM_BYTES_PER_LAUNCH = 20477184
-DRAM_BYTES_SOURCE = "profiles/r02d_pull2_kernel.md"
+DRAM_BYTES_PER_LAUNCH = 20466944
+DRAM_BYTES_SOURCE = "profiles/r03a_pull2_kernel.md"
 SURVEY_FP64_PER_ZONE_SUBSTEP = 13000  # SURVEY.md 8(d), 150 species / 1604 reactions
 
 # Algorithmic work per zone per sub-step: one multiply per
