@@ -290,6 +290,24 @@ def test_config4_full_batch_every_zone(hub150, capsys):
     assert w <= FIXED_TOL
 
 
+def test_config4_pre_burned_start(hub150, capsys):
+    """SURVEY 8(d)'s optional variant of config 4 (a strongly burning zone has
+    tens of populated species): every zone starts from its state after one hydro step, dt carried,
+    so that 20-40 species sit above 1e-12 at t = 0 instead of two.  The start state is the ORACLE's
+    (first call on the CPU); the second call is compared, 2048 zones of the config-4 profile in the
+    sorted launch."""
+    c = build_config(4, zones=2048)
+    kn, o = K.Net(hub150), Oracle(hub150)
+    first = o.integrate(c["T9"], c["rho"], c["Y0"], c["t_hydro"], n_threads=max_threads())
+    Y1, dt1 = first["Y"], first["dt"]
+    populated = ((Y1 * hub150.A) > X_MIN).sum(axis=1)
+    assert np.median(populated) >= 20 and (((c["Y0"] * hub150.A) > X_MIN).sum(axis=1) <= 2).all()
+    ref, arb = oracle_with_arbiter(hub150, c["T9"], c["rho"], Y1, c["t_hydro"], dt1)
+    g = gpu_integrate(kn, c["T9"], c["rho"], Y1, c["t_hydro"], dt=dt1)
+    say(capsys, f"config4 pre-burned (median {int(np.median(populated))} species above 1e-12 at the start)",
+        check_adaptive(g, ref, arb, hub150.A, "config4 pre-burned", min_direct=0.95))
+
+
 def test_config5_large_network_sampled(capsys):
     c = build_config(5)
     net = c["network"]
